@@ -1,0 +1,169 @@
+/*
+ * npfem.h - C ABI of the B200-native npFEM solid-solver step.
+ *
+ * The library advances every deformable blood cell (closed triangulated
+ * membranes: RBCs, platelets) of a batch by one implicit-Euler time step h,
+ * exactly as the paper states the solid problem:
+ *
+ *   state {x_n, v_n}, x, v in R^{n x 3}, input F_ext in R^{n x 3} .... PAPER.md:257
+ *   Eqs. (1)-(2) implicit Euler advancement ....................... PAPER.md:259-264
+ *   Eq. (3)  min_x g(x) = 1/(2h^2) ||M~^(1/2)(x - y_n)||^2 + sum_i E_i(x),
+ *            M~ = M + hC ........................................... PAPER.md:266-268
+ *   Eq. (4)  x^{k+1} <- x^k - H~^-1 grad g(x^k), H~ constant ....... PAPER.md:268-272
+ *   material constants ............................................. PAPER.md:226-239
+ *   every cell is independent within a step ........................ PAPER.md:61,63
+ *
+ * The paper defers the energies, H~ and the damping formulas to its ref. [4];
+ * the forms used are the readings R1-R16 listed in DESIGN.md.
+ *
+ * Conventions
+ *   - Units: micrometre, microsecond, femtogram, piconewton.
+ *   - Per-cell user buffers hold the paper's x in R^{n x 3}: `[n_vertices][3]`
+ *     (xyz interleaved), the listed cells back to back in `cell_ids` order;
+ *     `cell_ids == NULL` means all cells in cell-id order 0..n_cells-1.
+ *   - `dtype` of a user buffer is NPFEM_F32 or NPFEM_F64 and is independent of
+ *     the context's compute precision (fp64 I/O on an fp32 context keeps the
+ *     placement of cells far from the origin exact: state is stored in
+ *     cell-local coordinates around a per-cell fp64 origin).
+ *   - `where` says whether a user buffer is a DEVICE pointer (e.g. a torch
+ *     tensor's data_ptr) or a HOST pointer (pinned memory gives async copies).
+ *   - The library never frees caller memory.  All device work is enqueued on
+ *     the stream given at creation; calls with device buffers return without
+ *     synchronising.  Calls that write HOST buffers (get_*) synchronise the
+ *     stream before returning; calls that read HOST buffers return after the
+ *     host data has been consumed.
+ *   - Every call returns NPFEM_OK (0) or a negative code; no exception crosses
+ *     the ABI.  The message of the last failure is kept per context (and per
+ *     thread for npfem_create) and read with npfem_last_error.  CUDA errors
+ *     are sticky: after NPFEM_ECUDA the context only accepts npfem_destroy.
+ *   - There is NO CPU fallback: without a CUDA device every call fails.
+ */
+#ifndef NPFEM_H_
+#define NPFEM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NPFEM_OK       0
+#define NPFEM_EINVAL  -1   /* bad argument */
+#define NPFEM_EMESH   -2   /* mesh not a closed, consistently oriented 2-manifold / degenerate */
+#define NPFEM_ECUDA   -3   /* CUDA runtime failure (sticky) */
+#define NPFEM_ENOMEM  -4   /* host or device allocation failed / workspace too small */
+#define NPFEM_ESTATE  -5   /* call out of order (e.g. step before set_state) / solver setup failed */
+
+#define NPFEM_F32 32
+#define NPFEM_F64 64
+
+#define NPFEM_DEVICE 0
+#define NPFEM_HOST   1
+
+/* options for npfem_set_option */
+#define NPFEM_OPT_DIAGNOSTICS      1  /* 1: record the objective before every iteration (row a5) */
+#define NPFEM_OPT_GLOBAL_STEP_MATH 2  /* fp32 contexts: 0 = TF32 tensor cores (default), 1 = FP32 FFMA */
+#define NPFEM_OPT_LOCAL_STEP_IMPL  3  /* 0 = auto, 1 = generic kernel, 2 = shared-memory persistent kernel */
+
+#define NPFEM_MAX_ITERATIONS 256
+
+typedef struct npfem_ctx npfem_ctx; /* opaque, owned by the library */
+
+/* Material of one cell type. */
+typedef struct npfem_material {
+  double skalak_B;        /* pN/um   shear-type constant of the Skalak law            */
+  double skalak_C;        /* pN/um   area-dilation constant of the Skalak law         */
+  double skalak_D;        /* pN/um   listed by the paper, no formula given: unused    */
+  double k_bending;       /* pN*um   hinge bending stiffness                          */
+  double k_volume;        /* pN/um^2 volume-conservation stiffness                    */
+  double rayleigh_alpha;  /* 1/us    C = alpha M + beta K                             */
+  double rayleigh_beta;   /* us                                                       */
+  double kappa_damping;   /* [0,1]   position-based-dynamics velocity damping, 0=off  */
+  double density;         /* fg/um^3 mass of body incl. interior fluid = density * V0 */
+} npfem_material;
+
+/* One cell type: rest shape (HOST pointers, copied by npfem_create) + material. */
+typedef struct npfem_cell_type {
+  int32_t n_vertices;
+  int32_t n_triangles;
+  const double *rest_positions; /* [n_vertices][3] */
+  const int32_t *triangles;     /* [n_triangles][3], counter-clockwise seen from outside */
+  npfem_material material;
+} npfem_cell_type;
+
+/*
+ * Build a solver for `n_cells` cells; cell c has type `type_of_cell[c]` (HOST array).
+ * Pre-computes, per TYPE: rest data, lumped mass, the one-ring operator of the
+ * Rayleigh/inertia term, and the dense inverse of the constant Hessian
+ * approximation H~ (Eq. 4) on the device.
+ * dt: time step h in us.  precision: NPFEM_F32 or NPFEM_F64 (compute type).
+ * device: CUDA ordinal.  cuda_stream: a cudaStream_t (NULL = legacy default stream).
+ * On failure *out is NULL and npfem_last_error(NULL) holds the message.
+ */
+int npfem_create(npfem_ctx **out, const npfem_cell_type *types, int32_t n_types,
+                 const int32_t *type_of_cell, int64_t n_cells, double dt,
+                 int32_t precision, int32_t device, void *cuda_stream);
+
+/*
+ * Device memory for state and scratch.  Optional: the caller (e.g. torch) may own it.
+ * If no workspace is bound before the first set_state, the library allocates its own.
+ * `dev_ptr` must be 256-byte aligned and stay valid until npfem_destroy.
+ */
+size_t npfem_workspace_bytes(const npfem_ctx *ctx);
+int npfem_bind_workspace(npfem_ctx *ctx, void *dev_ptr, size_t bytes);
+
+/* Runtime switches (NPFEM_OPT_*). */
+int npfem_set_option(npfem_ctx *ctx, int32_t option, int64_t value);
+
+/*
+ * Initial placement: positions x_n and velocities v_n (NULL = zero) of the listed cells,
+ * each `[n_vertices(type)][3]` of `dtype`.  Forces of these cells are reset to zero.
+ */
+int npfem_set_state(npfem_ctx *ctx, const int64_t *cell_ids, int64_t n_ids,
+                    const void *positions, const void *velocities, int32_t dtype, int32_t where);
+
+/*
+ * External forces F_ext(x_n) of the listed cells, pN.  Forces persist
+ * until overwritten (the solid solver may run every >= 2 fluid steps).
+ */
+int npfem_set_forces(npfem_ctx *ctx, const int64_t *cell_ids, int64_t n_ids,
+                     const void *forces, int32_t dtype, int32_t where);
+
+/*
+ * ONE time step h for every cell: prologue (PBD damping, rhs), `n_iterations`
+ * quasi-Newton iterations of Eq. (4) (local step = grad g, global step = apply H~^-1),
+ * epilogue (Eq. 1).  1 <= n_iterations <= NPFEM_MAX_ITERATIONS.  Asynchronous.
+ */
+int npfem_step(npfem_ctx *ctx, int32_t n_iterations);
+
+/* Current {x, v} of the listed cells (either pointer may be NULL). */
+int npfem_get_state(npfem_ctx *ctx, const int64_t *cell_ids, int64_t n_ids,
+                    void *positions, void *velocities, int32_t dtype, int32_t where);
+
+/*
+ * Row (a5) diagnostic (needs NPFEM_OPT_DIAGNOSTICS = 1 before the step): the objective
+ * of Eq. (3) up to its d-independent constant, g(d) = d^T M~ d/(2h^2) - d^T b + E(x_n + d),
+ * per cell, before each iteration of the LAST step and after its final one.
+ * history: fp64 `[n_entries][n_cells]` (cell-id order), n_entries = n_iterations + 1,
+ * at most `max_entries` rows are written.  monotone (may be NULL): int32 per cell,
+ * 1 if the objective never increased.  Both buffers live `where` says.
+ */
+int npfem_get_objective(npfem_ctx *ctx, double *history, int32_t max_entries,
+                        int32_t *n_entries, int32_t *monotone, int32_t where);
+
+/* Number of kernels the library has launched on this context so far. */
+int64_t npfem_launch_count(const npfem_ctx *ctx);
+
+/* Message of the last failure on `ctx` (ctx == NULL: of the last failed npfem_create). */
+const char *npfem_last_error(const npfem_ctx *ctx);
+
+/* "major.minor.patch (sm_100a)" */
+const char *npfem_version(void);
+
+void npfem_destroy(npfem_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NPFEM_H_ */

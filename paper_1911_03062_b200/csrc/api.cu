@@ -1,0 +1,585 @@
+// C ABI of libnpfem_b200.so (include/npfem.h): context, workspace layout, call orchestration.
+// Every arithmetic step of the path runs in the CUDA kernels of this directory; there is no
+// CPU fallback.
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "internal.h"
+
+using namespace npfem;
+
+struct npfem_ctx {
+  int precision = NPFEM_F32, device = 0, n_sm = 148;
+  cudaStream_t stream = nullptr;
+  double dt = 0;
+  int64_t n_cells = 0, total_vertices = 0;
+  std::vector<HostTypeData> host_types;
+  std::vector<TypeDev> types;
+  std::vector<Bucket> buckets;            // one per type
+  std::vector<BucketView> views;
+  std::vector<int32_t> type_of_cell, slot_of_cell;
+  std::vector<int64_t> user_offset_all;   // [n_cells+1] element offsets in all-cells order
+  std::vector<uint8_t> cell_is_set;
+  int64_t n_set = 0;
+  // workspace
+  unsigned char *ws = nullptr;
+  size_t ws_bytes = 0;
+  bool ws_owned = false, ready = false;
+  struct Layout {
+    std::vector<size_t> type_off[11];     // per type: tri, nbr, rest, hinge, corner, vnbr, w, mass, inv_area, Hinv, Hinv_tf32
+    std::vector<size_t> field_off[F_COUNT], origin_off, cellid_off, scratch_off;
+    size_t views_off = 0, refs_all_off = 0, refs_tmp_off = 0, stage_a_off = 0, stage_b_off = 0, total = 0;
+  } lay;
+  BucketView *views_dev = nullptr;
+  CellRef *refs_all_dev = nullptr, *refs_tmp_dev = nullptr;
+  std::vector<int64_t *> cell_id_dev;
+  void *stage_a = nullptr, *stage_b = nullptr;
+  // diagnostics
+  bool diagnostics = false;
+  double *history_dev = nullptr;
+  int history_cap = 0, history_entries = 0;
+  int64_t opt_global_math = 0, opt_local_impl = 0;
+  int64_t launches = 0;
+  bool sticky = false;
+  std::string err;
+};
+
+namespace {
+
+thread_local std::string g_create_error;
+
+size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+size_t esize(int precision) { return precision == NPFEM_F32 ? 4 : 8; }
+
+int fail(npfem_ctx *c, int code, const std::string &msg) {
+  if (c) {
+    c->err = msg;
+    if (code == NPFEM_ECUDA) c->sticky = true;
+  } else {
+    g_create_error = msg;
+  }
+  return code;
+}
+
+#define NPFEM_CUDA(c, call)                                                              \
+  do {                                                                                   \
+    cudaError_t e_ = (call);                                                             \
+    if (e_ != cudaSuccess)                                                               \
+      return fail((c), NPFEM_ECUDA, std::string(#call ": ") + cudaGetErrorString(e_));   \
+  } while (0)
+
+int check_launch(npfem_ctx *c, int n, const char *what) {
+  if (n < 0) return fail(c, NPFEM_ESTATE, std::string(what) + ": unsupported configuration");
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(c, NPFEM_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+  c->launches += n;
+  return NPFEM_OK;
+}
+
+void compute_layout(npfem_ctx *c) {
+  auto &L = c->lay;
+  const size_t es = esize(c->precision);
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    const size_t o = off;
+    off = align_up(off + bytes);
+    return o;
+  };
+  const size_t nt = c->host_types.size();
+  for (auto &v : L.type_off) v.assign(nt, 0);
+  for (int f = 0; f < F_COUNT; ++f) L.field_off[f].assign(nt, 0);
+  L.origin_off.assign(nt, 0);
+  L.cellid_off.assign(nt, 0);
+  L.scratch_off.assign(nt, 0);
+  for (size_t t = 0; t < nt; ++t) {
+    const HostTypeData &h = c->host_types[t];
+    const size_t n = h.n, T = h.T, vm = h.valence_max, np = h.n_pad;
+    L.type_off[0][t] = take(T * sizeof(int4));
+    L.type_off[1][t] = take(T * sizeof(int4));
+    L.type_off[2][t] = take(T * 4 * es);
+    L.type_off[3][t] = take(T * 6 * es);
+    L.type_off[4][t] = take(vm * n * sizeof(int));
+    L.type_off[5][t] = take(vm * n * sizeof(int));
+    L.type_off[6][t] = take((vm + 1) * n * es);
+    L.type_off[7][t] = take(n * es);
+    L.type_off[8][t] = take(n * es);
+    L.type_off[9][t] = take(np * np * es);
+    L.type_off[10][t] = take(c->precision == NPFEM_F32 ? np * np * 4 : 0);
+    const size_t cells = size_t(c->buckets[t].cells);
+    for (int f = 0; f < F_COUNT; ++f) L.field_off[f][t] = take(cells * 3 * np * es);
+    L.origin_off[t] = take(cells * 3 * sizeof(double));
+    L.cellid_off[t] = take(cells * sizeof(int64_t));
+    TypeDev tmp;
+    tmp.n = h.n;
+    tmp.T = h.T;
+    L.scratch_off[t] = take(cells ? local_generic_scratch_bytes(tmp, c->precision, c->n_sm) : 0);
+  }
+  L.views_off = take(nt * sizeof(BucketView));
+  L.refs_all_off = take(size_t(c->n_cells) * sizeof(CellRef));
+  L.refs_tmp_off = take(size_t(c->n_cells) * sizeof(CellRef));
+  L.stage_a_off = take(size_t(c->total_vertices) * 3 * sizeof(double));
+  L.stage_b_off = take(size_t(c->total_vertices) * 3 * sizeof(double));
+  L.total = off;
+}
+
+template <typename T>
+std::vector<T> convert(const std::vector<double> &v) {
+  std::vector<T> out(v.size());
+  for (size_t i = 0; i < v.size(); ++i) out[i] = T(v[i]);
+  return out;
+}
+
+// upload a double vector as the compute type
+int upload_real(npfem_ctx *c, size_t off, const std::vector<double> &v) {
+  if (c->precision == NPFEM_F32) {
+    const std::vector<float> f = convert<float>(v);
+    NPFEM_CUDA(c, cudaMemcpyAsync(c->ws + off, f.data(), f.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  } else {
+    NPFEM_CUDA(c, cudaMemcpyAsync(c->ws + off, v.data(), v.size() * 8, cudaMemcpyHostToDevice, c->stream));
+    NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  }
+  return NPFEM_OK;
+}
+
+template <typename V>
+int upload_raw(npfem_ctx *c, size_t off, const std::vector<V> &v) {
+  if (v.empty()) return NPFEM_OK;
+  NPFEM_CUDA(c, cudaMemcpyAsync(c->ws + off, v.data(), v.size() * sizeof(V), cudaMemcpyHostToDevice, c->stream));
+  NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  return NPFEM_OK;
+}
+
+// Allocate (if not bound) and fill the workspace: type tables, H~^-1, cell tables.
+int ensure_ready(npfem_ctx *c) {
+  if (c->ready) return NPFEM_OK;
+  NPFEM_CUDA(c, cudaSetDevice(c->device));
+  if (!c->ws) {
+    void *p = nullptr;
+    if (cudaMalloc(&p, c->lay.total ? c->lay.total : 256) != cudaSuccess) {
+      cudaGetLastError();
+      return fail(c, NPFEM_ENOMEM, "cannot allocate " + std::to_string(c->lay.total) + " bytes of device workspace");
+    }
+    c->ws = static_cast<unsigned char *>(p);
+    c->ws_bytes = c->lay.total;
+    c->ws_owned = true;
+  }
+  auto &L = c->lay;
+  const size_t nt = c->host_types.size();
+  c->types.assign(nt, TypeDev());
+  c->views.assign(nt, BucketView());
+  c->cell_id_dev.assign(nt, nullptr);
+  for (size_t t = 0; t < nt; ++t) {
+    const HostTypeData &h = c->host_types[t];
+    TypeDev &d = c->types[t];
+    d.n = h.n; d.T = h.T; d.n_pad = h.n_pad; d.valence_max = h.valence_max;
+    int rc;
+    if ((rc = upload_raw(c, L.type_off[0][t], h.tri))) return rc;
+    if ((rc = upload_raw(c, L.type_off[1][t], h.tri_nbr))) return rc;
+    if ((rc = upload_real(c, L.type_off[2][t], h.tri_rest))) return rc;
+    if ((rc = upload_real(c, L.type_off[3][t], h.hinge_rest))) return rc;
+    if ((rc = upload_raw(c, L.type_off[4][t], h.vtx_corner))) return rc;
+    if ((rc = upload_raw(c, L.type_off[5][t], h.vtx_nbr))) return rc;
+    if ((rc = upload_real(c, L.type_off[6][t], h.vtx_w))) return rc;
+    if ((rc = upload_real(c, L.type_off[7][t], h.mass))) return rc;
+    std::vector<double> inv_area(h.n);
+    for (int v = 0; v < h.n; ++v) inv_area[v] = 1.0 / h.area_v[v];
+    if ((rc = upload_real(c, L.type_off[8][t], inv_area))) return rc;
+    d.tri = reinterpret_cast<const int4 *>(c->ws + L.type_off[0][t]);
+    d.tri_nbr = reinterpret_cast<const int4 *>(c->ws + L.type_off[1][t]);
+    d.tri_rest = c->ws + L.type_off[2][t];
+    d.hinge_rest = c->ws + L.type_off[3][t];
+    d.vtx_corner = reinterpret_cast<const int *>(c->ws + L.type_off[4][t]);
+    d.vtx_nbr = reinterpret_cast<const int *>(c->ws + L.type_off[5][t]);
+    d.vtx_w = c->ws + L.type_off[6][t];
+    d.vtx_mass = c->ws + L.type_off[7][t];
+    d.vtx_inv_area = c->ws + L.type_off[8][t];
+    d.Hinv = c->ws + L.type_off[9][t];
+    d.Hinv_tf32 = c->precision == NPFEM_F32 ? c->ws + L.type_off[10][t] : nullptr;
+    const npfem_material &m = h.mat;
+    d.h = h.h;
+    d.B4 = m.skalak_B / 4.0;
+    d.C4 = m.skalak_C / 4.0;
+    d.k_b = m.k_bending;
+    d.kv_over_V0 = m.k_volume / h.V0;
+    d.V0 = h.V0;
+    d.k_mem = m.skalak_B + 2.0 * m.skalak_C;
+    d.beta_over_h = m.rayleigh_beta / h.h;
+    d.inertia_coef = (1.0 + h.h * m.rayleigh_alpha) / (h.h * h.h);
+    d.kappa = m.kappa_damping;
+
+    // dense inverse of H~ on the device (fp64), then cast/pad to the compute type
+    double *H64 = nullptr, *Hinv64 = nullptr;
+    const size_t hb = size_t(h.n) * h.n * sizeof(double);
+    if (cudaMalloc(&H64, hb) != cudaSuccess || cudaMalloc(&Hinv64, hb) != cudaSuccess) {
+      cudaGetLastError();
+      cudaFree(H64);
+      return fail(c, NPFEM_ENOMEM, "cannot allocate the temporaries for the H~ inverse");
+    }
+    cudaError_t e = cudaMemcpyAsync(H64, h.H.data(), hb, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    std::string ierr;
+    double residual = 0;
+    int nl = e == cudaSuccess ? launch_invert_spd(H64, Hinv64, h.n, c->stream, &residual, ierr) : -1;
+    if (nl >= 0) {
+      nl += launch_convert_pad(Hinv64, h.n, c->ws + L.type_off[9][t], h.n_pad, c->precision, c->stream);
+      e = cudaStreamSynchronize(c->stream);
+    }
+    cudaFree(H64);
+    cudaFree(Hinv64);
+    if (e != cudaSuccess) return fail(c, NPFEM_ECUDA, std::string("H~ inverse: ") + cudaGetErrorString(e));
+    if (nl < 0) return fail(c, nl == -2 ? NPFEM_ENOMEM : NPFEM_ESTATE, ierr);
+    c->launches += nl;
+
+    // bucket
+    Bucket &b = c->buckets[t];
+    BucketView &bv = c->views[t];
+    for (int f = 0; f < F_COUNT; ++f) bv.field[f] = b.field[f] = c->ws + L.field_off[f][t];
+    bv.origin = b.origin = reinterpret_cast<double *>(c->ws + L.origin_off[t]);
+    bv.cells = b.cells;
+    bv.n = h.n;
+    bv.n_pad = h.n_pad;
+    b.scratch = c->ws + L.scratch_off[t];
+    c->cell_id_dev[t] = reinterpret_cast<int64_t *>(c->ws + L.cellid_off[t]);
+    std::vector<int64_t> ids;
+    ids.reserve(size_t(b.cells));
+    for (int64_t cell = 0; cell < c->n_cells; ++cell)
+      if (c->type_of_cell[cell] == int(t)) ids.push_back(cell);
+    if ((rc = upload_raw(c, L.cellid_off[t], ids))) return rc;
+  }
+  c->views_dev = reinterpret_cast<BucketView *>(c->ws + L.views_off);
+  c->refs_all_dev = reinterpret_cast<CellRef *>(c->ws + L.refs_all_off);
+  c->refs_tmp_dev = reinterpret_cast<CellRef *>(c->ws + L.refs_tmp_off);
+  c->stage_a = c->ws + L.stage_a_off;
+  c->stage_b = c->ws + L.stage_b_off;
+  int rc;
+  if ((rc = upload_raw(c, L.views_off, c->views))) return rc;
+  std::vector<CellRef> refs(size_t(c->n_cells));
+  for (int64_t cell = 0; cell < c->n_cells; ++cell)
+    refs[cell] = CellRef{c->user_offset_all[cell], c->type_of_cell[cell], c->slot_of_cell[cell]};
+  if ((rc = upload_raw(c, L.refs_all_off, refs))) return rc;
+  c->ready = true;
+  return NPFEM_OK;
+}
+
+// Resolve a cell-id list to device CellRefs; returns element count of the packed user buffer.
+int resolve_refs(npfem_ctx *c, const int64_t *cell_ids, int64_t n_ids, const CellRef **refs_dev,
+                 int64_t *n_refs, int64_t *n_elems, bool mark_set) {
+  if (!cell_ids) {
+    *refs_dev = c->refs_all_dev;
+    *n_refs = c->n_cells;
+    *n_elems = c->total_vertices * 3;
+    if (mark_set) {
+      std::fill(c->cell_is_set.begin(), c->cell_is_set.end(), uint8_t(1));
+      c->n_set = c->n_cells;
+    }
+    return NPFEM_OK;
+  }
+  if (n_ids < 0 || n_ids > c->n_cells) return fail(c, NPFEM_EINVAL, "n_ids out of range");
+  std::vector<CellRef> refs(static_cast<size_t>(n_ids));
+  int64_t off = 0;
+  for (int64_t i = 0; i < n_ids; ++i) {
+    const int64_t id = cell_ids[i];
+    if (id < 0 || id >= c->n_cells) return fail(c, NPFEM_EINVAL, "cell id " + std::to_string(id) + " out of range");
+    const int t = c->type_of_cell[id];
+    refs[i] = CellRef{off, t, c->slot_of_cell[id]};
+    off += int64_t(3) * c->host_types[t].n;
+  }
+  if (mark_set)
+    for (int64_t i = 0; i < n_ids; ++i)
+      if (!c->cell_is_set[cell_ids[i]]) {
+        c->cell_is_set[cell_ids[i]] = 1;
+        ++c->n_set;
+      }
+  if (n_ids) {
+    NPFEM_CUDA(c, cudaMemcpyAsync(c->refs_tmp_dev, refs.data(), refs.size() * sizeof(CellRef),
+                                  cudaMemcpyHostToDevice, c->stream));
+    NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  }
+  *refs_dev = c->refs_tmp_dev;
+  *n_refs = n_ids;
+  *n_elems = off;
+  return NPFEM_OK;
+}
+
+int common_checks(npfem_ctx *c, int32_t dtype, int32_t where) {
+  if (!c) return NPFEM_EINVAL;
+  if (c->sticky) return fail(c, NPFEM_ECUDA, "context is in a sticky CUDA error state: " + c->err);
+  if (dtype != NPFEM_F32 && dtype != NPFEM_F64) return fail(c, NPFEM_EINVAL, "dtype must be NPFEM_F32 or NPFEM_F64");
+  if (where != NPFEM_DEVICE && where != NPFEM_HOST) return fail(c, NPFEM_EINVAL, "where must be NPFEM_DEVICE or NPFEM_HOST");
+  return NPFEM_OK;
+}
+
+}  // namespace
+
+// =============================================================================================
+extern "C" {
+
+const char *npfem_version(void) { return "0.1.0 (sm_100a)"; }
+
+const char *npfem_last_error(const npfem_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+int64_t npfem_launch_count(const npfem_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int npfem_create(npfem_ctx **out, const npfem_cell_type *types, int32_t n_types, const int32_t *type_of_cell,
+                 int64_t n_cells, double dt, int32_t precision, int32_t device, void *cuda_stream) {
+  if (!out) return fail(nullptr, NPFEM_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!types || n_types < 1 || n_cells < 0 || (n_cells > 0 && !type_of_cell))
+    return fail(nullptr, NPFEM_EINVAL, "types/type_of_cell missing or counts invalid");
+  if (precision != NPFEM_F32 && precision != NPFEM_F64)
+    return fail(nullptr, NPFEM_EINVAL, "precision must be NPFEM_F32 or NPFEM_F64");
+  if (!(dt > 0)) return fail(nullptr, NPFEM_EINVAL, "dt must be positive");
+  npfem_ctx *c = new (std::nothrow) npfem_ctx();
+  if (!c) return fail(nullptr, NPFEM_ENOMEM, "out of host memory");
+  c->precision = precision;
+  c->device = device;
+  c->stream = static_cast<cudaStream_t>(cuda_stream);
+  c->dt = dt;
+  c->n_cells = n_cells;
+  try {
+    c->host_types.resize(size_t(n_types));
+    c->buckets.resize(size_t(n_types));
+    for (int t = 0; t < n_types; ++t) {
+      std::string err;
+      const int rc = build_host_type(types[t], dt, c->host_types[t], err);
+      if (rc != NPFEM_OK) {
+        delete c;
+        return fail(nullptr, rc, "cell type " + std::to_string(t) + ": " + err);
+      }
+      c->buckets[t].type = t;
+    }
+    c->type_of_cell.assign(type_of_cell, type_of_cell + n_cells);
+    c->slot_of_cell.resize(size_t(n_cells));
+    c->user_offset_all.resize(size_t(n_cells) + 1);
+    c->cell_is_set.assign(size_t(n_cells), 0);
+    int64_t off = 0;
+    for (int64_t cell = 0; cell < n_cells; ++cell) {
+      const int t = type_of_cell[cell];
+      if (t < 0 || t >= n_types) {
+        delete c;
+        return fail(nullptr, NPFEM_EINVAL, "type_of_cell[" + std::to_string(cell) + "] out of range");
+      }
+      c->slot_of_cell[cell] = int32_t(c->buckets[t].cells++);
+      c->user_offset_all[cell] = off;
+      off += int64_t(3) * c->host_types[t].n;
+    }
+    c->user_offset_all[n_cells] = off;
+    c->total_vertices = off / 3;
+  } catch (const std::bad_alloc &) {
+    delete c;
+    return fail(nullptr, NPFEM_ENOMEM, "out of host memory");
+  }
+  // host-side validation is done; from here on a CUDA device is required
+  int n_dev = 0;
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) {
+    cudaGetLastError();
+    delete c;
+    return fail(nullptr, NPFEM_ECUDA, "no CUDA device available (this library has no CPU fallback)");
+  }
+  if (device < 0 || device >= n_dev) {
+    delete c;
+    return fail(nullptr, NPFEM_EINVAL, "device ordinal out of range");
+  }
+  cudaDeviceProp prop;
+  if (cudaSetDevice(device) != cudaSuccess || cudaGetDeviceProperties(&prop, device) != cudaSuccess) {
+    delete c;
+    return fail(nullptr, NPFEM_ECUDA, "cannot query the CUDA device");
+  }
+  if (prop.major < 10) {
+    delete c;
+    return fail(nullptr, NPFEM_ECUDA, "this library is built for sm_100a (B200) only");
+  }
+  c->n_sm = prop.multiProcessorCount;
+  compute_layout(c);
+  *out = c;
+  return NPFEM_OK;
+}
+
+size_t npfem_workspace_bytes(const npfem_ctx *ctx) { return ctx ? ctx->lay.total : 0; }
+
+int npfem_bind_workspace(npfem_ctx *c, void *dev_ptr, size_t bytes) {
+  if (!c) return NPFEM_EINVAL;
+  if (c->ready || c->ws) return fail(c, NPFEM_ESTATE, "workspace already bound or allocated");
+  if (!dev_ptr || (reinterpret_cast<uintptr_t>(dev_ptr) & 255)) return fail(c, NPFEM_EINVAL, "workspace must be a 256-byte aligned device pointer");
+  if (bytes < c->lay.total) return fail(c, NPFEM_ENOMEM, "workspace too small: need " + std::to_string(c->lay.total) + " bytes");
+  c->ws = static_cast<unsigned char *>(dev_ptr);
+  c->ws_bytes = bytes;
+  c->ws_owned = false;
+  return ensure_ready(c);
+}
+
+int npfem_set_option(npfem_ctx *c, int32_t option, int64_t value) {
+  if (!c) return NPFEM_EINVAL;
+  switch (option) {
+    case NPFEM_OPT_DIAGNOSTICS: c->diagnostics = value != 0; return NPFEM_OK;
+    case NPFEM_OPT_GLOBAL_STEP_MATH:
+      if (value < 0 || value > 1) return fail(c, NPFEM_EINVAL, "global-step math must be 0 (TF32) or 1 (FP32)");
+      c->opt_global_math = value;
+      return NPFEM_OK;
+    case NPFEM_OPT_LOCAL_STEP_IMPL:
+      if (value < 0 || value > 2) return fail(c, NPFEM_EINVAL, "local-step impl must be 0, 1 or 2");
+      c->opt_local_impl = value;
+      return NPFEM_OK;
+    default: return fail(c, NPFEM_EINVAL, "unknown option");
+  }
+}
+
+int npfem_set_state(npfem_ctx *c, const int64_t *cell_ids, int64_t n_ids, const void *positions,
+                    const void *velocities, int32_t dtype, int32_t where) {
+  int rc = common_checks(c, dtype, where);
+  if (rc) return rc;
+  if (!positions) return fail(c, NPFEM_EINVAL, "positions is NULL");
+  if ((rc = ensure_ready(c))) return rc;
+  PackArgs a{};
+  int64_t n_elems = 0;
+  if ((rc = resolve_refs(c, cell_ids, n_ids, &a.refs, &a.n_refs, &n_elems, true))) return rc;
+  a.io_dtype = dtype;
+  a.src_a = positions;
+  a.src_b = velocities;
+  if (where == NPFEM_HOST && n_elems) {
+    const size_t bytes = size_t(n_elems) * (dtype == NPFEM_F32 ? 4 : 8);
+    NPFEM_CUDA(c, cudaMemcpyAsync(c->stage_a, positions, bytes, cudaMemcpyHostToDevice, c->stream));
+    a.src_a = c->stage_a;
+    if (velocities) {
+      NPFEM_CUDA(c, cudaMemcpyAsync(c->stage_b, velocities, bytes, cudaMemcpyHostToDevice, c->stream));
+      a.src_b = c->stage_b;
+    }
+  }
+  if ((rc = check_launch(c, launch_set_state(c->views_dev, a, c->precision, c->stream), "set_state"))) return rc;
+  if (where == NPFEM_HOST) NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  return NPFEM_OK;
+}
+
+int npfem_set_forces(npfem_ctx *c, const int64_t *cell_ids, int64_t n_ids, const void *forces, int32_t dtype,
+                     int32_t where) {
+  int rc = common_checks(c, dtype, where);
+  if (rc) return rc;
+  if (!forces) return fail(c, NPFEM_EINVAL, "forces is NULL");
+  if ((rc = ensure_ready(c))) return rc;
+  PackArgs a{};
+  int64_t n_elems = 0;
+  if ((rc = resolve_refs(c, cell_ids, n_ids, &a.refs, &a.n_refs, &n_elems, false))) return rc;
+  a.io_dtype = dtype;
+  a.src_a = forces;
+  if (where == NPFEM_HOST && n_elems) {
+    const size_t bytes = size_t(n_elems) * (dtype == NPFEM_F32 ? 4 : 8);
+    NPFEM_CUDA(c, cudaMemcpyAsync(c->stage_a, forces, bytes, cudaMemcpyHostToDevice, c->stream));
+    a.src_a = c->stage_a;
+  }
+  if ((rc = check_launch(c, launch_set_forces(c->views_dev, a, c->precision, c->stream), "set_forces"))) return rc;
+  if (where == NPFEM_HOST) NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  return NPFEM_OK;
+}
+
+int npfem_get_state(npfem_ctx *c, const int64_t *cell_ids, int64_t n_ids, void *positions, void *velocities,
+                    int32_t dtype, int32_t where) {
+  int rc = common_checks(c, dtype, where);
+  if (rc) return rc;
+  if (!c->ready || c->n_set != c->n_cells) return fail(c, NPFEM_ESTATE, "get_state before every cell has been given a state");
+  PackArgs a{};
+  int64_t n_elems = 0;
+  if ((rc = resolve_refs(c, cell_ids, n_ids, &a.refs, &a.n_refs, &n_elems, false))) return rc;
+  a.io_dtype = dtype;
+  a.dst_a = positions;
+  a.dst_b = velocities;
+  if (where == NPFEM_HOST) {
+    a.dst_a = positions ? c->stage_a : nullptr;
+    a.dst_b = velocities ? c->stage_b : nullptr;
+  }
+  if ((rc = check_launch(c, launch_get_state(c->views_dev, a, c->precision, c->stream), "get_state"))) return rc;
+  if (where == NPFEM_HOST) {
+    const size_t bytes = size_t(n_elems) * (dtype == NPFEM_F32 ? 4 : 8);
+    if (positions && bytes) NPFEM_CUDA(c, cudaMemcpyAsync(positions, c->stage_a, bytes, cudaMemcpyDeviceToHost, c->stream));
+    if (velocities && bytes) NPFEM_CUDA(c, cudaMemcpyAsync(velocities, c->stage_b, bytes, cudaMemcpyDeviceToHost, c->stream));
+    NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  }
+  return NPFEM_OK;
+}
+
+int npfem_step(npfem_ctx *c, int32_t n_iterations) {
+  if (!c) return NPFEM_EINVAL;
+  if (c->sticky) return fail(c, NPFEM_ECUDA, "context is in a sticky CUDA error state: " + c->err);
+  if (n_iterations < 1 || n_iterations > NPFEM_MAX_ITERATIONS) return fail(c, NPFEM_EINVAL, "n_iterations out of range");
+  if (!c->ready || c->n_set != c->n_cells) return fail(c, NPFEM_ESTATE, "step before every cell has been given a state");
+  int rc;
+  const size_t nb = c->buckets.size();
+  if (c->diagnostics) {
+    const int need = n_iterations + 1;
+    if (need > c->history_cap) {
+      if (c->history_dev) NPFEM_CUDA(c, cudaFree(c->history_dev));
+      c->history_dev = nullptr;
+      c->history_cap = 0;
+      void *p = nullptr;
+      if (cudaMalloc(&p, size_t(need) * size_t(c->n_cells ? c->n_cells : 1) * sizeof(double)) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, NPFEM_ENOMEM, "cannot allocate the objective history");
+      }
+      c->history_dev = static_cast<double *>(p);
+      c->history_cap = need;
+    }
+    c->history_entries = need;
+  } else {
+    c->history_entries = 0;
+  }
+  auto diag = [&](int row) -> int {
+    for (size_t t = 0; t < nb; ++t) {
+      const int r = check_launch(c, launch_objective(c->types[t], c->views[t], c->cell_id_dev[t],
+                                                     c->history_dev + size_t(row) * c->n_cells, c->precision, c->stream),
+                                 "objective");
+      if (r) return r;
+    }
+    return NPFEM_OK;
+  };
+  for (size_t t = 0; t < nb; ++t)
+    if ((rc = check_launch(c, launch_prologue(c->types[t], c->views[t], c->precision, c->stream), "prologue"))) return rc;
+  for (int k = 0; k < n_iterations; ++k) {
+    if (c->diagnostics && (rc = diag(k))) return rc;
+    for (size_t t = 0; t < nb; ++t) {
+      if ((rc = check_launch(c, launch_local_generic(c->types[t], c->views[t], c->buckets[t].scratch, c->precision,
+                                                     c->n_sm, c->stream), "local step")))
+        return rc;
+      if ((rc = check_launch(c, launch_global_simt(c->types[t], c->views[t], c->precision, c->stream), "global step")))
+        return rc;
+    }
+  }
+  if (c->diagnostics && (rc = diag(n_iterations))) return rc;
+  for (size_t t = 0; t < nb; ++t)
+    if ((rc = check_launch(c, launch_epilogue(c->types[t], c->views[t], c->precision, c->stream), "epilogue"))) return rc;
+  return NPFEM_OK;
+}
+
+int npfem_get_objective(npfem_ctx *c, double *history, int32_t max_entries, int32_t *n_entries, int32_t *monotone,
+                        int32_t where) {
+  int rc = common_checks(c, NPFEM_F64, where);
+  if (rc) return rc;
+  if (!c->history_entries) return fail(c, NPFEM_ESTATE, "no objective history: enable NPFEM_OPT_DIAGNOSTICS before npfem_step");
+  const int rows = std::min<int>(max_entries, c->history_entries);
+  if (n_entries) *n_entries = c->history_entries;
+  const cudaMemcpyKind kind = where == NPFEM_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+  if (history && rows > 0 && c->n_cells)
+    NPFEM_CUDA(c, cudaMemcpyAsync(history, c->history_dev, size_t(rows) * c->n_cells * sizeof(double), kind, c->stream));
+  if (monotone && c->n_cells) {
+    int32_t *flags = where == NPFEM_HOST ? static_cast<int32_t *>(c->stage_a) : monotone;
+    if ((rc = check_launch(c, launch_monotone_flags(c->history_dev, c->history_entries, c->n_cells, flags, c->stream), "monotone")))
+      return rc;
+    if (where == NPFEM_HOST)
+      NPFEM_CUDA(c, cudaMemcpyAsync(monotone, flags, size_t(c->n_cells) * sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
+  }
+  if (where == NPFEM_HOST) NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  return NPFEM_OK;
+}
+
+void npfem_destroy(npfem_ctx *c) {
+  if (!c) return;
+  cudaSetDevice(c->device);
+  cudaStreamSynchronize(c->stream);
+  if (c->ws_owned && c->ws) cudaFree(c->ws);
+  if (c->history_dev) cudaFree(c->history_dev);
+  cudaGetLastError();
+  delete c;
+}
+
+}  // extern "C"

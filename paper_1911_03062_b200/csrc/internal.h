@@ -1,0 +1,98 @@
+// Internal declarations shared by the translation units of libnpfem_b200.so.
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/npfem.h"
+#include "host_setup.hpp"
+
+namespace npfem {
+
+// Number of state fields kept per bucket, each [cells][3][n_pad] of the compute type.
+enum Field { F_X = 0, F_V, F_F, F_B, F_D, F_G, F_COUNT };
+
+// Device view of one cell type (pointers into the workspace; element type = compute type).
+struct TypeDev {
+  int n = 0, T = 0, n_pad = 0, valence_max = 0;
+  const int4 *tri = nullptr;         // [T]  v0 v1 v2 0
+  const int4 *tri_nbr = nullptr;     // [T]  t0 t1 t2 0
+  const void *tri_rest = nullptr;    // [T][4]  a b c A0
+  const void *hinge_rest = nullptr;  // [T][6]  (cos, sin) theta0 per edge
+  const int *vtx_corner = nullptr;   // [valence_max][n]
+  const int *vtx_nbr = nullptr;      // [valence_max][n]
+  const void *vtx_w = nullptr;       // [valence_max+1][n]
+  const void *vtx_mass = nullptr;    // [n]  m_v
+  const void *vtx_inv_area = nullptr;// [n]  1/A_v
+  const void *Hinv = nullptr;        // [n_pad][n_pad] dense inverse of H~ (compute type)
+  const void *Hinv_tf32 = nullptr;   // fp32 contexts: same, rounded to TF32, tiled for tcgen05 (may be null)
+  // scalars (double; converted at launch)
+  double h = 0, B4 = 0, C4 = 0, k_b = 0, kv_over_V0 = 0, V0 = 0, k_mem = 0, beta_over_h = 0;
+  double inertia_coef = 0;           // (1 + h alpha) / h^2, multiplies m_v
+  double kappa = 0;
+};
+
+// One bucket = all cells of one type, contiguous slots.
+struct Bucket {
+  int type = 0;
+  int64_t cells = 0;
+  void *field[F_COUNT] = {};         // each [cells][3][n_pad]
+  double *origin = nullptr;          // [cells][3] fp64 per-cell origin of the local coordinates
+  double *objective = nullptr;       // [NPFEM_MAX_ITERATIONS+1][cells] (diagnostics; lazily allocated)
+  void *scratch = nullptr;           // generic local step: per-CTA normals + corner forces when they do not fit smem
+};
+
+// Per listed cell: where its block sits in the user buffer and where it lives in the workspace.
+struct CellRef {
+  int64_t user_offset;   // element offset of the cell's [n][3] block in the user buffer
+  int32_t bucket;
+  int32_t slot;
+};
+
+// ---- launchers (each enqueues on `stream`, returns the number of kernels launched or <0) -------
+int launch_invert_spd(const double *H_dev, double *Hinv_dev, int n, cudaStream_t stream,
+                      double *residual_out, std::string &err);
+
+int launch_convert_pad(const double *X, int n, void *out, int n_pad, int precision, cudaStream_t s);
+
+// implemented per operation in pack.cu
+struct PackArgs {
+  const CellRef *refs;     // device
+  int64_t n_refs;
+  const void *src_a;       // positions / forces (device, io dtype) or nullptr
+  const void *src_b;       // velocities or nullptr
+  void *dst_a;             // get_state outputs
+  void *dst_b;
+  int io_dtype;
+};
+
+struct BucketView {       // what kernels need of a bucket, passed by value
+  void *field[F_COUNT];
+  double *origin;
+  int64_t cells;
+  int n, n_pad;
+};
+
+int launch_set_state(const BucketView *views_dev, const PackArgs &a, int precision, cudaStream_t s);
+int launch_set_forces(const BucketView *views_dev, const PackArgs &a, int precision, cudaStream_t s);
+int launch_get_state(const BucketView *views_dev, const PackArgs &a, int precision, cudaStream_t s);
+
+int launch_prologue(const TypeDev &td, const BucketView &bv, int precision, cudaStream_t s);
+int launch_epilogue(const TypeDev &td, const BucketView &bv, int precision, cudaStream_t s);
+
+// local step: g = M~ d/h^2 - b + grad E(x_n + d)
+size_t local_generic_scratch_bytes(const TypeDev &td, int precision, int n_sm);
+int launch_local_generic(const TypeDev &td, const BucketView &bv, void *scratch, int precision, int n_sm,
+                         cudaStream_t s);
+int launch_objective(const TypeDev &td, const BucketView &bv, const int64_t *cell_id_dev, double *objective_row,
+                     int precision, cudaStream_t s);
+
+// global step: d <- d - g Hinv   ([3 cells x n_pad] . [n_pad x n_pad])
+int launch_global_simt(const TypeDev &td, const BucketView &bv, int precision, cudaStream_t s);
+
+int launch_monotone_flags(const double *history, int n_entries, int64_t cells, int32_t *flags, cudaStream_t s);
+
+}  // namespace npfem

@@ -1,0 +1,156 @@
+// Step prologue (row a1) and epilogue (row a4).
+//
+// Prologue, once per time step and cell (readings R3, R12):
+//   1. position-based-dynamics damping of v_n (paper's ref. [6]):
+//        v <- v + kappa (v_cm + omega x r - v),  r = x - x_cm,
+//        omega = I^-1 sum r x (m v),  I = sum m (|r|^2 Id - r r^T)
+//   2. b = M v/h + F_ext  (so that grad g = M~ d/h^2 - b + grad E),  d^0 = h v.
+//   It also re-centres the cell-local coordinates when the mass centre has drifted.
+// Epilogue (Eq. 1): x_{n+1} = x_n + d, v_{n+1} = d/h.
+#include "internal.h"
+
+namespace npfem {
+namespace {
+
+template <int N>
+__device__ __forceinline__ void block_sum_n(double (&v)[N], double *red /* [8][N] */) {
+#pragma unroll
+  for (int k = 0; k < N; ++k)
+    for (int o = 16; o > 0; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
+  const int w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0)
+#pragma unroll
+    for (int k = 0; k < N; ++k) red[w * N + k] = v[k];
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < N; ++k) {
+    double s = 0.0;
+    for (int i = 0; i < nw; ++i) s += red[i * N + k];
+    v[k] = s;
+  }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+prologue_kernel(BucketView bv, const T *__restrict__ mass, double kappa, double h) {
+  __shared__ double red[8 * 9];
+  const int n = bv.n, n_pad = bv.n_pad;
+  for (int64_t cell = blockIdx.x; cell < bv.cells; cell += gridDim.x) {
+    const size_t base = size_t(cell) * 3 * n_pad;
+    T *x = static_cast<T *>(bv.field[F_X]) + base;
+    T *v = static_cast<T *>(bv.field[F_V]) + base;
+    const T *f = static_cast<const T *>(bv.field[F_F]) + base;
+    T *b = static_cast<T *>(bv.field[F_B]) + base;
+    T *d = static_cast<T *>(bv.field[F_D]) + base;
+
+    double s[7] = {};   // sum m, sum m x, sum m v
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+      const double m = double(mass[i]);
+      s[0] += m;
+      for (int k = 0; k < 3; ++k) {
+        s[1 + k] += m * double(x[k * n_pad + i]);
+        s[4 + k] += m * double(v[k * n_pad + i]);
+      }
+    }
+    block_sum_n<7>(s, red);
+    const double xc[3] = {s[1] / s[0], s[2] / s[0], s[3] / s[0]};
+    const double vc[3] = {s[4] / s[0], s[5] / s[0], s[6] / s[0]};
+
+    double om[3] = {0.0, 0.0, 0.0};
+    if (kappa > 0.0) {
+      double q[9] = {};   // angular momentum (3), inertia xx yy zz xy xz yz
+      for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const double m = double(mass[i]);
+        const double r0 = double(x[i]) - xc[0], r1 = double(x[n_pad + i]) - xc[1], r2 = double(x[2 * n_pad + i]) - xc[2];
+        const double p0 = m * double(v[i]), p1 = m * double(v[n_pad + i]), p2 = m * double(v[2 * n_pad + i]);
+        q[0] += r1 * p2 - r2 * p1;
+        q[1] += r2 * p0 - r0 * p2;
+        q[2] += r0 * p1 - r1 * p0;
+        q[3] += m * (r1 * r1 + r2 * r2);
+        q[4] += m * (r0 * r0 + r2 * r2);
+        q[5] += m * (r0 * r0 + r1 * r1);
+        q[6] -= m * r0 * r1;
+        q[7] -= m * r0 * r2;
+        q[8] -= m * r1 * r2;
+      }
+      block_sum_n<9>(q, red);
+      // omega = I^-1 L, symmetric 3x3 inverse by the adjugate
+      const double a = q[3], bb = q[4], c = q[5], dxy = q[6], dxz = q[7], dyz = q[8];
+      const double A00 = bb * c - dyz * dyz, A01 = dxz * dyz - dxy * c, A02 = dxy * dyz - dxz * bb;
+      const double A11 = a * c - dxz * dxz, A12 = dxy * dxz - a * dyz, A22 = a * bb - dxy * dxy;
+      const double det = a * A00 + dxy * A01 + dxz * A02;
+      om[0] = (A00 * q[0] + A01 * q[1] + A02 * q[2]) / det;
+      om[1] = (A01 * q[0] + A11 * q[1] + A12 * q[2]) / det;
+      om[2] = (A02 * q[0] + A12 * q[1] + A22 * q[2]) / det;
+    }
+
+    // re-centre the local frame when the mass centre drifted (exact binary shift, rare)
+    double shift[3] = {0.0, 0.0, 0.0};
+    const bool recentre = fabs(xc[0]) > 0.5 || fabs(xc[1]) > 0.5 || fabs(xc[2]) > 0.5;
+    if (recentre) {
+      for (int k = 0; k < 3; ++k) shift[k] = rint(xc[k] * 1024.0) / 1024.0;
+      if (threadIdx.x < 3) bv.origin[size_t(cell) * 3 + threadIdx.x] += shift[threadIdx.x];
+    }
+
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+      const double m = double(mass[i]);
+      double xi[3], vi[3];
+      for (int k = 0; k < 3; ++k) {
+        xi[k] = double(x[k * n_pad + i]);
+        vi[k] = double(v[k * n_pad + i]);
+      }
+      if (kappa > 0.0) {
+        const double r0 = xi[0] - xc[0], r1 = xi[1] - xc[1], r2 = xi[2] - xc[2];
+        const double w[3] = {om[1] * r2 - om[2] * r1, om[2] * r0 - om[0] * r2, om[0] * r1 - om[1] * r0};
+        for (int k = 0; k < 3; ++k) vi[k] += kappa * (vc[k] + w[k] - vi[k]);
+      }
+      for (int k = 0; k < 3; ++k) {
+        if (recentre) x[k * n_pad + i] = T(xi[k] - shift[k]);
+        v[k * n_pad + i] = T(vi[k]);
+        b[k * n_pad + i] = T(m * vi[k] / h + double(f[k * n_pad + i]));
+        d[k * n_pad + i] = T(h * vi[k]);
+      }
+    }
+    __syncthreads();
+  }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+epilogue_kernel(BucketView bv, T inv_h) {
+  T *x = static_cast<T *>(bv.field[F_X]);
+  T *v = static_cast<T *>(bv.field[F_V]);
+  const T *d = static_cast<const T *>(bv.field[F_D]);
+  const size_t total = size_t(bv.cells) * 3 * bv.n_pad;
+  for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < total; i += size_t(gridDim.x) * blockDim.x) {
+    const T di = d[i];
+    x[i] += di;
+    v[i] = di * inv_h;
+  }
+}
+
+}  // namespace
+
+int launch_prologue(const TypeDev &td, const BucketView &bv, int precision, cudaStream_t s) {
+  if (bv.cells == 0) return 0;
+  const unsigned grid = unsigned(bv.cells < 148 * 16 ? bv.cells : 148 * 16);
+  if (precision == NPFEM_F32)
+    prologue_kernel<float><<<grid, 256, 0, s>>>(bv, static_cast<const float *>(td.vtx_mass), td.kappa, td.h);
+  else
+    prologue_kernel<double><<<grid, 256, 0, s>>>(bv, static_cast<const double *>(td.vtx_mass), td.kappa, td.h);
+  return 1;
+}
+
+int launch_epilogue(const TypeDev &td, const BucketView &bv, int precision, cudaStream_t s) {
+  if (bv.cells == 0) return 0;
+  const size_t total = size_t(bv.cells) * 3 * bv.n_pad;
+  const unsigned grid = unsigned((total + 255) / 256 < 148 * 16 ? (total + 255) / 256 : 148 * 16);
+  if (precision == NPFEM_F32)
+    epilogue_kernel<float><<<grid, 256, 0, s>>>(bv, float(1.0 / td.h));
+  else
+    epilogue_kernel<double><<<grid, 256, 0, s>>>(bv, 1.0 / td.h);
+  return 1;
+}
+
+}  // namespace npfem

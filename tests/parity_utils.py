@@ -1,0 +1,72 @@
+"""Shared helpers of the GPU parity tests: run a workloads.Population through the C-ABI binding
+and through the fp64 oracle on the SAME seeded arrays, and compare."""
+import numpy as np
+
+from oracle import npfem_oracle as orc
+
+
+def run_oracle(pop, n_steps=None, n_iterations=None):
+    """-> per-type (x, v) after the run, fp64."""
+    n_steps = pop.n_steps if n_steps is None else n_steps
+    n_iterations = pop.n_iterations if n_iterations is None else n_iterations
+    out = []
+    for t, ct in enumerate(pop.types):
+        if pop.positions[t].shape[0] == 0:
+            out.append((pop.positions[t].copy(), pop.velocities[t].copy()))
+            continue
+        td = orc.make_type(ct, pop.dt)
+        out.append(orc.run(pop.positions[t], pop.velocities[t], lambda s, t=t: pop.forces(s)[t], td,
+                           n_steps, n_iterations))
+    return out
+
+
+def run_gpu(pop, precision, n_steps=None, n_iterations=None, io="fp64", where="device", options=()):
+    """-> per-type (x, v) after the run as fp64 numpy, plus the solver (still open)."""
+    import torch
+    from paper_1911_03062_b200 import Solver
+    n_steps = pop.n_steps if n_steps is None else n_steps
+    n_iterations = pop.n_iterations if n_iterations is None else n_iterations
+    np_dt = np.float32 if io == "fp32" else np.float64
+    solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision=precision)
+    for opt, val in options:
+        solver.set_option(opt, val)
+
+    def to_buf(per_type):
+        flat = pop.packed(per_type, dtype=np_dt)
+        return torch.from_numpy(flat).cuda() if where == "device" else flat
+
+    solver.set_state(to_buf(pop.positions), to_buf(pop.velocities))
+    const_forces = None if pop.redraw_noise_each_step else to_buf(pop.forces(0))
+    for s in range(n_steps):
+        solver.set_forces(const_forces if const_forces is not None else to_buf(pop.forces(s)))
+        solver.step(n_iterations)
+    x, v = solver.get_state(dtype=io, where=where)
+    if where == "device":
+        x, v = x.cpu().numpy(), v.cpu().numpy()
+    xs, vs = pop.unpack(x.astype(np.float64)), pop.unpack(v.astype(np.float64))
+    return list(zip(xs, vs)), solver
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def compare(pop, gpu, ref):
+    """Per type: relative L2 error on positions (BASELINE.json's bar), on the displacement
+    x_end - x_0 (sharper) and on velocities."""
+    rows = []
+    for t in range(len(pop.types)):
+        if pop.positions[t].shape[0] == 0:
+            continue
+        xg, vg = gpu[t]
+        xr, vr = ref[t]
+        x0 = pop.positions[t]
+        rows.append({
+            "type": pop.types[t].name,
+            "pos": rel_l2(xg, xr),
+            "disp": rel_l2(xg - x0, xr - x0),
+            "vel": rel_l2(vg, vr),
+            "worst_cell_pos": float(np.max(np.linalg.norm((xg - xr).reshape(xg.shape[0], -1), axis=1)
+                                           / np.linalg.norm(xr.reshape(xr.shape[0], -1), axis=1))),
+        })
+    return rows

@@ -1,0 +1,158 @@
+"""GPU parity: the CUDA path through the C-ABI against the fp64 oracle, element by element on the
+same seeded inputs.  Tolerances (BASELINE.json north_star): relative L2 on positions 1e-10 (fp64)
+and 1e-4 (fp32); the displacement-relative error (sharper) is checked against looser bars derived
+in DESIGN.md ("Tolerances")."""
+import numpy as np
+import pytest
+
+from tests.parity_utils import compare, rel_l2, run_gpu, run_oracle
+from workloads import icosahedron_cell_type, make_config
+from workloads.populations import Population
+
+pytestmark = pytest.mark.gpu
+
+TOL_POS = {"fp64": 1e-10, "fp32": 1e-4}
+TOL_DISP = {"fp64": 1e-8, "fp32": 5e-3}
+
+
+def _check(pop, precision, **kw):
+    gpu, solver = run_gpu(pop, precision, **kw)
+    ref = run_oracle(pop, kw.get("n_steps"), kw.get("n_iterations"))
+    rows = compare(pop, gpu, ref)
+    solver.close()
+    for r in rows:
+        print(precision, r)
+        assert r["pos"] <= TOL_POS[precision], r
+        assert r["worst_cell_pos"] <= TOL_POS[precision], r
+        assert r["disp"] <= TOL_DISP[precision], r
+        assert r["vel"] <= TOL_DISP[precision], r
+    return rows
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_config1_single_rbc(precision):
+    _check(make_config(1), precision)
+
+
+@pytest.mark.parametrize("precision", ["fp32", "fp64"])
+def test_config2_reduced_70_cells_full_schedule(precision):
+    # 70 cells = 210 GEMM rows: several 64-row tiles and a ragged tail; full 10 steps x 10 its
+    _check(make_config(2, n_cells=70), precision)
+
+
+@pytest.mark.parametrize("precision", ["fp32", "fp64"])
+def test_config3_mixed_types_redrawn_forces(precision):
+    pop = make_config(3, n_cells=45)          # 41 RBC-642 + 4 PLT-162, interleaved ids
+    _check(pop, precision, n_steps=4, n_iterations=5)
+
+
+@pytest.mark.parametrize("precision", ["fp32", "fp64"])
+def test_config5_level4_mesh(precision):
+    # 2562 vertices: the shared-memory budget is exceeded -> global-scratch variant of the local step
+    _check(make_config(5, n_cells=3), precision, n_steps=2, n_iterations=3)
+
+
+def test_icosahedron_cell_fp64():
+    ct = icosahedron_cell_type(3.0)
+    rng = np.random.default_rng(0)
+    pos = ct.rest_positions[None] + 0.05 * rng.standard_normal((5, 12, 3)) + rng.uniform(0, 50, (5, 1, 3))
+    pop = Population(name="ico", types=[ct], type_of_cell=np.zeros(5, np.int32), positions=[pos],
+                     velocities=[0.02 * rng.standard_normal(pos.shape)], dt=0.1, n_steps=3, n_iterations=8,
+                     box=(50.0,) * 3, force_sigma=2.0, shear_gamma=0.0, redraw_noise_each_step=False,
+                     _force_seed=np.random.SeedSequence(5), _shear_height=[pos[..., 2]])
+    _check(pop, "fp64")
+
+
+def test_io_paths_agree_and_partial_ids():
+    """Host and device buffers, fp32 and fp64 I/O, full and partial id lists give the same state."""
+    import torch
+    from paper_1911_03062_b200 import Solver
+    pop = make_config(3, n_cells=23)
+    gpu_dev, s1 = run_gpu(pop, "fp32", n_steps=2, n_iterations=3, io="fp64", where="device")
+    gpu_host, s2 = run_gpu(pop, "fp32", n_steps=2, n_iterations=3, io="fp64", where="host")
+    for (xa, va), (xb, vb) in zip(gpu_dev, gpu_host):
+        assert np.array_equal(xa, xb) and np.array_equal(va, vb)
+    ids = np.array([21, 3, 10, 0], dtype=np.int64)          # cell 10 and 21 are platelets
+    xs, vs = s1.get_state(cell_ids=ids)
+    sub = pop.unpack(xs.cpu().numpy(), ids)
+    order_rbc = [3, 0]                                       # list order within each type
+    assert np.array_equal(sub[0][0], gpu_dev[0][0][3]) and np.array_equal(sub[0][1], gpu_dev[0][0][0])
+    assert np.array_equal(sub[1][0], gpu_dev[1][0][1]) and np.array_equal(sub[1][1], gpu_dev[1][0][0])
+    # fp32 read-back is the fp64 read-back rounded once
+    x32, _ = s1.get_state(dtype="fp32")
+    x64, _ = s1.get_state(dtype="fp64")
+    assert torch.equal(x32, x64.to(torch.float32))
+    s1.close()
+    s2.close()
+
+
+def test_partial_set_state_and_forces_persist():
+    from paper_1911_03062_b200 import Solver, NpfemError
+    import torch
+    pop = make_config(2, n_cells=6)
+    solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision="fp64")
+    first, rest = np.array([0, 1, 2]), np.array([5, 4, 3])
+    solver.set_state(torch.from_numpy(pop.packed(pop.positions, first)).cuda(), cell_ids=first)
+    with pytest.raises(NpfemError) as e:
+        solver.step(2)                                        # three cells still have no state
+    assert e.value.code == -5
+    solver.set_state(torch.from_numpy(pop.packed(pop.positions, rest)).cuda(), cell_ids=rest)
+    solver.set_forces(torch.from_numpy(pop.packed(pop.forces(0))).cuda())
+    solver.step(4)
+    solver.step(4)                                            # forces persist until overwritten
+    x, v = solver.get_state()
+    ref = run_oracle(pop, 2, 4)
+    assert rel_l2(pop.unpack(x.cpu().numpy())[0], ref[0][0]) < 1e-10
+    with pytest.raises(NpfemError) as e:
+        solver.step(0)
+    assert e.value.code == -1
+    solver.close()
+
+
+def test_rest_state_stays_at_rest_far_from_origin():
+    """P1 on the GPU: rigidly placed rest shapes, no force -> no motion, even 1000 um out in fp32."""
+    from paper_1911_03062_b200 import Solver
+    import torch
+    pop = make_config(2, n_cells=8)
+    pos = [pop.positions[0] + 1000.0]
+    solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision="fp32")
+    solver.set_state(torch.from_numpy(pop.packed(pos)).cuda())
+    for _ in range(3):
+        solver.step(5)
+    x, v = solver.get_state()
+    disp = x.cpu().numpy() - pop.packed(pos)
+    assert np.abs(disp).max() < 2e-6          # fp32 round-off of the local coordinates only
+    assert np.abs(v.cpu().numpy()).max() < 1e-4
+    solver.close()
+
+
+def test_zero_cells_and_empty_bucket():
+    from paper_1911_03062_b200 import Solver
+    pop = make_config(3, n_cells=5)                           # 5 RBCs, platelet bucket empty
+    gpu, solver = run_gpu(pop, "fp64", n_steps=1, n_iterations=2)
+    ref = run_oracle(pop, 1, 2)
+    assert rel_l2(gpu[0][0], ref[0][0]) < 1e-10
+    solver.close()
+    empty = Solver(pop.types, np.zeros(0, np.int32), pop.dt, precision="fp32")
+    empty.step(3)
+    x, v = empty.get_state()
+    assert x.numel() == 0
+    empty.close()
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_objective_history_matches_oracle(precision):
+    from oracle import npfem_oracle as orc
+    from paper_1911_03062_b200 import binding
+    pop = make_config(2, n_cells=4)
+    gpu, solver = run_gpu(pop, precision, n_steps=1, n_iterations=6,
+                          options=[(binding.OPT_DIAGNOSTICS, 1)])
+    hist, mono = solver.get_objective()
+    solver.close()
+    td = orc.make_type(pop.types[0], pop.dt)
+    _, _, rec = orc.step(pop.positions[0], pop.velocities[0], pop.forces(0)[0], td, 6, record=True)
+    ref = np.array(rec["objective"])                          # [7, 4]
+    assert hist.shape == ref.shape
+    scale = np.abs(ref).max()
+    assert np.abs(hist - ref).max() < (1e-9 if precision == "fp64" else 2e-3) * scale
+    assert np.all(mono == 1)
