@@ -5,7 +5,7 @@ in DESIGN.md ("Tolerances")."""
 import numpy as np
 import pytest
 
-from tests.parity_utils import compare, rel_l2, run_gpu, run_oracle
+from parity_utils import compare, rel_l2, run_gpu, run_oracle
 from workloads import icosahedron_cell_type, make_config
 from workloads.populations import Population
 
