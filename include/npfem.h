@@ -66,6 +66,15 @@ extern "C" {
 #define NPFEM_OPT_GLOBAL_STEP_MATH 2  /* fp32 contexts: 0 = TF32 tensor cores (default), 1 = FP32 FFMA */
 #define NPFEM_OPT_LOCAL_STEP_IMPL  3  /* 0 = auto, 1 = generic kernel, 2 = shared-memory persistent kernel */
 
+#define NPFEM_OPT_KERNEL_TIMING    4  /* 1: bracket every kernel of npfem_step with CUDA events */
+
+/* kernel kinds reported by npfem_get_kernel_times */
+#define NPFEM_KIND_PROLOGUE 0
+#define NPFEM_KIND_LOCAL    1
+#define NPFEM_KIND_GLOBAL   2
+#define NPFEM_KIND_EPILOGUE 3
+#define NPFEM_KIND_COUNT    4
+
 #define NPFEM_MAX_ITERATIONS 256
 
 typedef struct npfem_ctx npfem_ctx; /* opaque, owned by the library */
@@ -151,6 +160,14 @@ int npfem_get_state(npfem_ctx *ctx, const int64_t *cell_ids, int64_t n_ids,
  */
 int npfem_get_objective(npfem_ctx *ctx, double *history, int32_t max_entries,
                         int32_t *n_entries, int32_t *monotone, int32_t where);
+
+/*
+ * Device time per kernel kind since the last reset (needs NPFEM_OPT_KERNEL_TIMING = 1): CUDA
+ * events recorded on the context's stream around every launch of npfem_step.  Synchronises the
+ * stream.  ms[kind][type] and launches[kind][type] are HOST arrays of NPFEM_KIND_COUNT * n_types
+ * entries (either may be NULL); reset != 0 clears the accumulators afterwards.
+ */
+int npfem_get_kernel_times(npfem_ctx *ctx, double *ms, int64_t *launches, int32_t reset);
 
 /* Number of kernels the library has launched on this context so far. */
 int64_t npfem_launch_count(const npfem_ctx *ctx);

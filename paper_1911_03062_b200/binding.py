@@ -13,13 +13,14 @@ import numpy as np
 
 NPFEM_F32, NPFEM_F64 = 32, 64
 NPFEM_DEVICE, NPFEM_HOST = 0, 1
-OPT_DIAGNOSTICS, OPT_GLOBAL_STEP_MATH, OPT_LOCAL_STEP_IMPL = 1, 2, 3
+OPT_DIAGNOSTICS, OPT_GLOBAL_STEP_MATH, OPT_LOCAL_STEP_IMPL, OPT_KERNEL_TIMING = 1, 2, 3, 4
+KIND_NAMES = ("prologue", "local", "global", "epilogue")
 _ERR_NAMES = {-1: "NPFEM_EINVAL", -2: "NPFEM_EMESH", -3: "NPFEM_ECUDA", -4: "NPFEM_ENOMEM", -5: "NPFEM_ESTATE"}
 
 EXPORTED_SYMBOLS = (
     "npfem_create", "npfem_workspace_bytes", "npfem_bind_workspace", "npfem_set_option",
     "npfem_set_state", "npfem_set_forces", "npfem_step", "npfem_get_state", "npfem_get_objective",
-    "npfem_launch_count", "npfem_last_error", "npfem_version", "npfem_destroy",
+    "npfem_get_kernel_times", "npfem_launch_count", "npfem_last_error", "npfem_version", "npfem_destroy",
 )
 
 
@@ -79,6 +80,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.npfem_get_state.restype = C.c_int
     lib.npfem_get_objective.argtypes = [vp, vp, i32, C.POINTER(i32), vp, i32]
     lib.npfem_get_objective.restype = C.c_int
+    lib.npfem_get_kernel_times.argtypes = [vp, vp, vp, i32]
+    lib.npfem_get_kernel_times.restype = C.c_int
     lib.npfem_launch_count.argtypes = [vp]
     lib.npfem_launch_count.restype = i64
     lib.npfem_last_error.argtypes = [vp]
@@ -225,6 +228,15 @@ class Solver:
         self._check(self._lib.npfem_get_objective(self._ctx, C.c_void_p(hist.ctypes.data), 257, C.byref(n_entries),
                                                   C.c_void_p(mono.ctypes.data), NPFEM_HOST))
         return hist[:n_entries.value, :self.n_cells].copy(), mono[:self.n_cells].copy()
+
+    def get_kernel_times(self, reset: bool = True):
+        """{kind: [(ms, launches) per cell type]} accumulated since the last reset (OPT_KERNEL_TIMING)."""
+        ms = np.zeros((len(KIND_NAMES), self.n_types), dtype=np.float64)
+        cnt = np.zeros((len(KIND_NAMES), self.n_types), dtype=np.int64)
+        self._check(self._lib.npfem_get_kernel_times(self._ctx, C.c_void_p(ms.ctypes.data),
+                                                     C.c_void_p(cnt.ctypes.data), 1 if reset else 0))
+        return {k: [(float(ms[i, t]), int(cnt[i, t])) for t in range(self.n_types)]
+                for i, k in enumerate(KIND_NAMES)}
 
     @property
     def launch_count(self) -> int:

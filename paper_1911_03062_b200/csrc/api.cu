@@ -42,6 +42,13 @@ struct npfem_ctx {
   int history_cap = 0, history_entries = 0;
   int64_t opt_global_math = 0, opt_local_impl = 0;
   int64_t launches = 0;
+  // kernel timing (NPFEM_OPT_KERNEL_TIMING)
+  bool timing = false;
+  struct TimedSpan { cudaEvent_t a, b; int kind, type; int launches; };
+  std::vector<TimedSpan> spans;
+  std::vector<cudaEvent_t> event_pool;
+  std::vector<double> kind_ms;
+  std::vector<int64_t> kind_launches;
   bool sticky = false;
   std::string err;
 };
@@ -75,6 +82,52 @@ int check_launch(npfem_ctx *c, int n, const char *what) {
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(c, NPFEM_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
   c->launches += n;
+  return NPFEM_OK;
+}
+
+cudaEvent_t take_event(npfem_ctx *c) {
+  if (!c->event_pool.empty()) {
+    cudaEvent_t e = c->event_pool.back();
+    c->event_pool.pop_back();
+    return e;
+  }
+  cudaEvent_t e = nullptr;
+  cudaEventCreate(&e);
+  return e;
+}
+
+// run `launch()` (returns #kernels or <0), bracketed by events when timing is on
+template <typename F>
+int timed_launch(npfem_ctx *c, int kind, int type, const char *what, F launch) {
+  if (!c->timing) return check_launch(c, launch(), what);
+  npfem_ctx::TimedSpan sp{take_event(c), take_event(c), kind, type, 0};
+  cudaEventRecord(sp.a, c->stream);
+  const int n = launch();
+  cudaEventRecord(sp.b, c->stream);
+  sp.launches = n > 0 ? n : 0;
+  c->spans.push_back(sp);
+  return check_launch(c, n, what);
+}
+
+int drain_spans(npfem_ctx *c) {
+  const size_t nt = c->host_types.size();
+  if (c->kind_ms.size() != NPFEM_KIND_COUNT * nt) {
+    c->kind_ms.assign(NPFEM_KIND_COUNT * nt, 0.0);
+    c->kind_launches.assign(NPFEM_KIND_COUNT * nt, 0);
+  }
+  if (c->spans.empty()) return NPFEM_OK;
+  NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  for (auto &sp : c->spans) {
+    float ms = 0.f;
+    if (sp.launches > 0 && cudaEventElapsedTime(&ms, sp.a, sp.b) == cudaSuccess) {
+      c->kind_ms[sp.kind * nt + sp.type] += ms;
+      c->kind_launches[sp.kind * nt + sp.type] += sp.launches;
+    }
+    c->event_pool.push_back(sp.a);
+    c->event_pool.push_back(sp.b);
+  }
+  c->spans.clear();
+  cudaGetLastError();
   return NPFEM_OK;
 }
 
@@ -423,6 +476,7 @@ int npfem_set_option(npfem_ctx *c, int32_t option, int64_t value) {
       if (value < 0 || value > 2) return fail(c, NPFEM_EINVAL, "local-step impl must be 0, 1 or 2");
       c->opt_local_impl = value;
       return NPFEM_OK;
+    case NPFEM_OPT_KERNEL_TIMING: c->timing = value != 0; return NPFEM_OK;
     default: return fail(c, NPFEM_EINVAL, "unknown option");
   }
 }
@@ -533,21 +587,44 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
     }
     return NPFEM_OK;
   };
+  if (c->spans.size() > 200000 && (rc = drain_spans(c))) return rc;
   for (size_t t = 0; t < nb; ++t)
-    if ((rc = check_launch(c, launch_prologue(c->types[t], c->views[t], c->precision, c->stream), "prologue"))) return rc;
+    if ((rc = timed_launch(c, NPFEM_KIND_PROLOGUE, int(t), "prologue", [&] {
+           return launch_prologue(c->types[t], c->views[t], c->precision, c->stream); })))
+      return rc;
   for (int k = 0; k < n_iterations; ++k) {
     if (c->diagnostics && (rc = diag(k))) return rc;
     for (size_t t = 0; t < nb; ++t) {
-      if ((rc = check_launch(c, launch_local_generic(c->types[t], c->views[t], c->buckets[t].scratch, c->precision,
-                                                     c->n_sm, c->stream), "local step")))
+      if ((rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "local step", [&] {
+             return launch_local_generic(c->types[t], c->views[t], c->buckets[t].scratch, c->precision, c->n_sm,
+                                         c->stream); })))
         return rc;
-      if ((rc = check_launch(c, launch_global_simt(c->types[t], c->views[t], c->precision, c->stream), "global step")))
+      if ((rc = timed_launch(c, NPFEM_KIND_GLOBAL, int(t), "global step", [&] {
+             return launch_global_simt(c->types[t], c->views[t], c->precision, c->stream); })))
         return rc;
     }
   }
   if (c->diagnostics && (rc = diag(n_iterations))) return rc;
   for (size_t t = 0; t < nb; ++t)
-    if ((rc = check_launch(c, launch_epilogue(c->types[t], c->views[t], c->precision, c->stream), "epilogue"))) return rc;
+    if ((rc = timed_launch(c, NPFEM_KIND_EPILOGUE, int(t), "epilogue", [&] {
+           return launch_epilogue(c->types[t], c->views[t], c->precision, c->stream); })))
+      return rc;
+  return NPFEM_OK;
+}
+
+int npfem_get_kernel_times(npfem_ctx *c, double *ms, int64_t *launches, int32_t reset) {
+  if (!c) return NPFEM_EINVAL;
+  if (c->sticky) return fail(c, NPFEM_ECUDA, "context is in a sticky CUDA error state: " + c->err);
+  const int rc = drain_spans(c);
+  if (rc) return rc;
+  const size_t cnt = c->kind_ms.size();
+  if (ms) std::copy(c->kind_ms.begin(), c->kind_ms.end(), ms);
+  if (launches) std::copy(c->kind_launches.begin(), c->kind_launches.end(), launches);
+  if (reset) {
+    std::fill(c->kind_ms.begin(), c->kind_ms.end(), 0.0);
+    std::fill(c->kind_launches.begin(), c->kind_launches.end(), 0);
+  }
+  (void)cnt;
   return NPFEM_OK;
 }
 
@@ -578,6 +655,11 @@ void npfem_destroy(npfem_ctx *c) {
   cudaStreamSynchronize(c->stream);
   if (c->ws_owned && c->ws) cudaFree(c->ws);
   if (c->history_dev) cudaFree(c->history_dev);
+  for (auto &sp : c->spans) {
+    cudaEventDestroy(sp.a);
+    cudaEventDestroy(sp.b);
+  }
+  for (auto e : c->event_pool) cudaEventDestroy(e);
   cudaGetLastError();
   delete c;
 }
