@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py - cells*solver-iterations/s of the npFEM step on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--cells M] [--iterations I]
+  python bench.py --impl reference ...        # times the fp64 CPU oracle on a bounded sample
+
+One "step" = one npfem_step (prologue, I x (local step, global step), epilogue) over the whole
+synthetic population.  Default workload: BASELINE.json configs[3], 100,000 mixed cells (90,000
+RBC-642 + 10,000 PLT-162), 10 iterations per step, fp32 - the configuration the north star
+quotes its target on; it fits one GPU.  Prints ONE JSON line (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cells*solver-iterations/sec"
+UNIT = "cell-iterations/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--cells", type=int, default=None, help="shrink the config to this many cells")
+    ap.add_argument("--iterations", type=int, default=None, help="solver iterations per step")
+    ap.add_argument("--precision", default="fp32", choices=["fp32", "fp64"])
+    ap.add_argument("--global-math", default="tf32", choices=["tf32", "fp32"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    return ap.parse_args()
+
+
+def load_peaks():
+    """Measured roofline denominators (driver-written), else the profiling guide's fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return {"hbm_gbs": float(p["hbm_gbs"]), "bf16_tflops": float(p["bf16_tflops"]),
+                "bf16_tflops_sustained": float(p.get("bf16_tflops_sustained", p["bf16_tflops"])),
+                "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device: int):
+        self.device, self.rows, self._stop, self._thread = device, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.device}", f"--query-gpu={self.QUERY}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
+                if out.returncode == 0 and out.stdout.strip():
+                    self.rows.append([c.strip() for c in out.stdout.strip().splitlines()[0].split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.15)
+
+    def __enter__(self):
+        self._thread = threading.Thread(target=self._run, daemon=True)
+        self._thread.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        self._thread.join(timeout=6)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        sm = sorted(float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit())
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": float(self.rows[0][1]),
+                "power_w_max": max(float(r[2]) for r in self.rows), "samples": len(self.rows), "reasons": reasons}
+
+
+# ---- algorithmic work per cell-iteration -------------
+def algorithmic_bytes(kind: str, n: int, es: int) -> int:
+    """local: read x_n, d, b, write g (4 vec3 fields); global: read g, d, write d (3 fields)."""
+    return {"local": 12 * n * es, "global": 9 * n * es}[kind]
+
+
+def global_flops(n: int) -> int:
+    return 6 * n * n          # [3 x n] . [n x n], multiply-add = 2 flops
+
+
+# ---- the oracle leg (cpu_baseline and --impl reference) --------------------------------------
+def blas_threads() -> int:
+    try:
+        from threadpoolctl import threadpool_info
+        return max([int(p.get("num_threads", 1)) for p in threadpool_info()] or [1])
+    except Exception:
+        return 1
+
+
+def oracle_sample(pop, n_sample: int):
+    """First n_sample cells of the population (same type mix) as their own population."""
+    return pop.subset(np.arange(min(n_sample, pop.n_cells)))
+
+
+def time_oracle(sample, n_iterations: int) -> float:
+    """Seconds for ONE time step of the oracle, as it stands, on the sample."""
+    from oracle import npfem_oracle as orc
+    tds = [orc.make_type(ct, sample.dt) for ct in sample.types]     # setup, not timed (as on the GPU)
+    forces = sample.forces(0)
+    t0 = time.perf_counter()
+    for t, td in enumerate(tds):
+        if sample.positions[t].shape[0]:
+            orc.step(sample.positions[t], sample.velocities[t], forces[t], td, n_iterations)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(pop, n_iterations: int, target_seconds: float):
+    probe = oracle_sample(pop, min(22, pop.n_cells))
+    t_probe = time_oracle(probe, n_iterations)
+    per_cell = max(t_probe / probe.n_cells, 1e-6)
+    n_sample = int(max(probe.n_cells, min(pop.n_cells, target_seconds / per_cell, 4000)))
+    sample = oracle_sample(pop, n_sample)
+    secs = time_oracle(sample, n_iterations)
+    counts = [int(np.sum(sample.type_of_cell == t)) for t in range(len(pop.types))]
+    desc = " + ".join(f"{c} {ct.name}" for c, ct in zip(counts, pop.types) if c)
+    return {
+        "value": sample.n_cells * n_iterations / secs, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+        "sample": f"first {sample.n_cells} cells of the workload ({desc}), 1 step x {n_iterations} iterations, "
+                  f"{secs:.1f} s; numpy element loops are single-threaded, LAPACK solves use `cores` threads",
+    }, sample
+
+
+def run_reference(args, pop, n_iterations: int, config_desc: dict):
+    """--impl reference: the fp64 oracle as it stands, each step a bounded sample of the workload."""
+    info, sample = cpu_baseline(pop, n_iterations, args.cpu_seconds)
+    for _ in range(min(args.warmup, 1)):
+        time_oracle(sample, n_iterations)
+    times = [time_oracle(sample, n_iterations) for _ in range(args.steps)]
+    total = float(np.sum(times))
+    value = sample.n_cells * n_iterations * args.steps / total
+    info["value"] = value
+    return {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": config_desc, "cpu_baseline": info,
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+
+
+# ---- the B200 arm ------------------------------------------------------------------------------
+def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: int):
+    import torch
+    from paper_1911_03062_b200 import Solver, binding
+
+    local_rank = int(os.environ.get("LOCAL_RANK", 0))
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    es = 4 if args.precision == "fp32" else 8
+    np_io = np.float32 if args.precision == "fp32" else np.float64
+    peaks = load_peaks()
+
+    solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision=args.precision, device=local_rank)
+    solver.set_option(binding.OPT_GLOBAL_STEP_MATH, 0 if args.global_math == "tf32" else 1)
+    solver.set_state(torch.from_numpy(pop.packed(pop.positions)).to(dev))
+    forces_host = torch.from_numpy(pop.packed(pop.forces(0), dtype=np_io)).pin_memory()
+    forces_dev = forces_host.to(dev)
+    solver.set_forces(forces_dev)
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: inputs already in HBM -------------------------------------
+    for _ in range(args.warmup):
+        solver.step(n_iterations)
+    solver.set_option(binding.OPT_KERNEL_TIMING, 1)
+    solver.get_kernel_times(reset=True)
+    barrier()
+    launches0 = solver.launch_count
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        ev0.record()
+        for _ in range(args.steps):
+            solver.step(n_iterations)
+        ev1.record()
+        barrier()
+    elapsed_ms = ev0.elapsed_time(ev1)
+    launches = solver.launch_count - launches0
+    ktimes = solver.get_kernel_times(reset=True)
+    solver.set_option(binding.OPT_KERNEL_TIMING, 0)
+    if world > 1:
+        t = torch.tensor([elapsed_ms], device=dev, dtype=torch.float64)
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+        elapsed_ms = float(t.item())
+    cell_iters = pop.n_cells * n_iterations * args.steps
+    value = world * cell_iters / (elapsed_ms * 1e-3)
+
+    # ---- per-kernel rooflines from the live CUDA-event times ---------------------------------
+    kernels, total_kernel_ms = [], sum(ms for v in ktimes.values() for ms, _ in v)
+    for kind in ("local", "global"):
+        for t, ct in enumerate(pop.types):
+            ms, cnt = ktimes[kind][t]
+            cells_t = int(np.sum(pop.type_of_cell == t))
+            if cnt == 0 or cells_t == 0:
+                continue
+            per_launch_s = ms * 1e-3 / cnt
+            bytes_launch = algorithmic_bytes(kind, ct.n_vertices, es) * cells_t
+            row = {"kernel": f"{kind}:{ct.name}", "launches": cnt, "avg_ms": ms / cnt,
+                   "share_of_kernel_time": ms / total_kernel_ms,
+                   "hbm_gbs": bytes_launch / per_launch_s / 1e9,
+                   "hbm_frac": bytes_launch / per_launch_s / 1e9 / peaks["hbm_gbs"]}
+            if kind == "global":
+                tflops = global_flops(ct.n_vertices) * cells_t / per_launch_s / 1e12
+                # TF32 dense peak = measured bf16 peak x nominal ratio 1/2 (B200_PROFILING.md); fp32/fp64 SIMT
+                # paths are reported against the same tensor figure for context only
+                row["tflops"] = tflops
+                row["tensor_frac_tf32"] = tflops / (0.5 * peaks["bf16_tflops_sustained"])
+            kernels.append(row)
+    dominant = max(kernels, key=lambda r: r["share_of_kernel_time"]) if kernels else None
+    roofline = None
+    if dominant:
+        roofline = {"kernel": dominant["kernel"], "bound": "hbm", "achieved": dominant["hbm_gbs"],
+                    "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": dominant["hbm_frac"], "traffic": None,
+                    "peak_source": peaks["source"] + " (MEASURED_PEAKS.json hbm_gbs)"}
+
+    result = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32" if args.precision == "fp32" else "f64",
+        "data": "synthetic", "config": config_desc, "clocks": clocks.summary(), "gpu_launches": launches,
+        "roofline": roofline, "kernels": kernels,
+        "kernel_ms_per_step": {k: sum(ms for ms, _ in v) / args.steps for k, v in ktimes.items()},
+    }
+
+    # ---- end to end through the C-ABI with HOST buffers ------------------------------------
+    if not args.no_e2e:
+        count = 3 * solver.total_vertices
+        pos_host = torch.empty(count, dtype=forces_host.dtype).pin_memory()
+        vel_host = torch.empty(count, dtype=forces_host.dtype).pin_memory()
+        for _ in range(2):
+            solver.set_forces(forces_host)
+            solver.step(n_iterations)
+            solver.get_state(positions=pos_host, velocities=vel_host)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            solver.set_forces(forces_host)                      # H2D of this step's F_ext
+            solver.step(n_iterations)
+            solver.get_state(positions=pos_host, velocities=vel_host)   # D2H of {x, v}
+        e1.record()
+        barrier()
+        e2e_ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
+            torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+            e2e_ms = float(t.item())
+        result["e2e"] = {"value": world * cell_iters / (e2e_ms * 1e-3), "unit": UNIT,
+                         "h2d_bytes_per_step": int(forces_host.numel() * forces_host.element_size()),
+                         "d2h_bytes_per_step": int(2 * count * pos_host.element_size()),
+                         "ms_per_step": e2e_ms / args.steps}
+    solver.close()
+    return result
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    from workloads import CONFIG_NAMES, make_config
+    n_iterations = args.iterations
+
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        args.cpu_seconds = min(args.cpu_seconds, 120.0 / max(args.steps, 1))
+        small = make_config(args.config, n_cells=min(args.cells or 10 ** 9, 4400))
+        full_cells = args.cells or make_config_size(args.config)
+        n_iterations = n_iterations or small.n_iterations
+        desc = config_description(args, small, full_cells, n_iterations)
+        print(json.dumps(run_reference(args, small, n_iterations, desc)), flush=True)
+        return 0
+
+    import torch
+    if world > 1:
+        torch.distributed.init_process_group("nccl")
+    pop = make_config(args.config, n_cells=args.cells)
+    n_iterations = n_iterations or pop.n_iterations
+    desc = config_description(args, pop, pop.n_cells, n_iterations)
+    desc["parallelism"] = f"{world} independent replica(s) of the workload, one per GPU, no collective"
+    result = run_b200(args, pop, n_iterations, desc, rank, world)
+    if rank == 0:
+        if not args.no_cpu_baseline and world == 1:
+            result["cpu_baseline"], _ = cpu_baseline(pop, n_iterations, args.cpu_seconds)
+        print(json.dumps(result), flush=True)
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    return 0
+
+
+def make_config_size(index: int) -> int:
+    return {1: 1, 2: 1000, 3: 22000, 4: 100000, 5: 10000}[index]
+
+
+def config_description(args, pop, n_cells: int, n_iterations: int) -> dict:
+    from workloads import CONFIG_NAMES
+    mix = {ct.name: ct.n_vertices for ct in pop.types}
+    return {"workload": f"BASELINE.json configs[{args.config - 1}]: {CONFIG_NAMES[args.config]}",
+            "cells": int(n_cells), "cell_types_vertices": mix, "iterations_per_step": int(n_iterations),
+            "dt_us": pop.dt, "precision": args.precision, "global_step_math": args.global_math,
+            "l2": "no flush needed: the state touched per iteration (>= 2.9 GB at 100k cells) exceeds the 126 MB L2"}
+
+
+if __name__ == "__main__":
+    sys.exit(main())
