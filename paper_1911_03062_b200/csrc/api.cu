@@ -600,6 +600,10 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
                                          c->stream); })))
         return rc;
       if ((rc = timed_launch(c, NPFEM_KIND_GLOBAL, int(t), "global step", [&] {
+             if (c->precision == NPFEM_F32 && c->opt_global_math == 0) {
+               const int n = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, c->stream);
+               if (n >= 0) return n;
+             }
              return launch_global_simt(c->types[t], c->views[t], c->precision, c->stream); })))
         return rc;
     }

@@ -1,0 +1,290 @@
+// Global step (row a3) on the 5th-generation tensor cores: d <- d - g H~^-1 for a whole type
+// bucket as ONE TF32 GEMM  D[3*cells x n_pad] -= G[3*cells x n_pad] . W[n_pad x n_pad]
+// (Eq. (4), reading R1; x in R^{n x 3}, matrices n x n).
+//
+// Cells of one type share the rest shape, hence the operator: the structure is a dense
+// contraction of one constant matrix against many right-hand sides, which is the only place of
+// the path where tensor cores apply.  Increment form keeps TF32 safe: the rounding lands on the
+// small update g W, not on d.
+//
+// Kernel: persistent, one CTA per SM, warp-specialised.
+//   warp 0   TMA producer : G tile [128 x 32 fp32] and W tile [N_pass x 32] per K chunk, 128B swizzle
+//   warp 1   MMA issuer   : tcgen05.mma.cta_group::1.kind::tf32, M = 128, N <= 256 per instruction,
+//                           accumulators for N_pass <= 512 columns in TMEM; A negated in the
+//                           instruction descriptor so the accumulator is -G W
+//   warps 2-5 epilogue    : tcgen05.ld -> d += acc (vectorised read-modify-write of the d tile)
+// Work item = (M tile, N pass); a CTA takes consecutive items so the G tile of pass 2 is an L2 hit,
+// and the producer runs ahead into the next item while the epilogue drains TMEM.
+#include <cuda.h>
+
+#include "internal.h"
+
+namespace npfem {
+namespace {
+
+constexpr int BM = 128;          // rows per tile (TMEM lanes)
+constexpr int BK = 32;           // fp32 per K chunk = 128 bytes = one swizzle row
+constexpr int UMMA_K = 8;        // K per tcgen05.mma for tf32 (32 bytes)
+constexpr int STAGES = 3;
+constexpr int MAX_NPASS = 336;   // accumulator columns per pass (<= 512, multiple of 16)
+constexpr int A_BYTES = BM * BK * 4;
+constexpr int B_BYTES = MAX_NPASS * BK * 4;
+constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return uint32_t(__cvta_generic_to_shared(p)); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  } while (!done);
+}
+
+__device__ __forceinline__ void tma_load_2d(void *smem_dst, const CUtensorMap *map, int x, int y, uint64_t *bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+      ::"r"(smem_u32(smem_dst)), "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y) : "memory");
+}
+
+// K-major, 128B-swizzled operand tile: 8-row atoms of 1024 bytes (SBO), version 1 (sm_100)
+__device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr) {
+  uint64_t desc = 0;
+  desc |= uint64_t((saddr & 0x3FFFF) >> 4);          // start address, bits [0,14)
+  desc |= uint64_t(1) << 16;                         // leading byte offset (unused for swizzled K-major)
+  desc |= uint64_t(1024 >> 4) << 32;                 // stride byte offset, bits [32,46)
+  desc |= uint64_t(1) << 46;                         // descriptor version for Blackwell
+  desc |= uint64_t(2) << 61;                         // SWIZZLE_128B
+  return desc;
+}
+
+// kind::tf32, fp32 accumulate, A and B K-major, A negated
+__host__ __device__ constexpr uint32_t make_idesc(int M, int N) {
+  return (1u << 4) | (2u << 7) | (2u << 10) | (1u << 13) | (uint32_t(N >> 3) << 17) | (uint32_t(M >> 4) << 24);
+}
+
+__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+                                          uint32_t accumulate) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "setp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n"
+      "}\n" ::"r"(tmem_d), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t *bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
+               : "memory");
+}
+
+struct GemmParams {
+  float *D;            // [rows][n_pad], updated in place
+  int64_t rows;
+  int n_pad;
+  int n_pass;          // accumulator columns per pass (multiple of 16, <= MAX_NPASS)
+  int passes;          // ceil(n_pad / n_pass)
+  int n1, n2;          // columns of the two MMA instructions of a pass (n1 <= 256, n2 may be 0)
+  int k_chunks;        // ceil(n_pad / BK)
+  int64_t m_tiles;
+};
+
+__global__ void __launch_bounds__(192, 1)
+global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_constant__ CUtensorMap map_w1,
+                      const __grid_constant__ CUtensorMap map_w2, const GemmParams p) {
+  extern __shared__ unsigned char smem_raw[];
+  __shared__ uint64_t full_bar[STAGES], empty_bar[STAGES], tmem_full_bar, tmem_empty_bar;
+  __shared__ uint32_t tmem_base_sh;
+  unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t n_items = p.m_tiles * p.passes;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(&full_bar[s], 1);
+      mbar_init(&empty_bar[s], 1);
+    }
+    mbar_init(&tmem_full_bar, 1);
+    mbar_init(&tmem_empty_bar, 128);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) {   // TMEM: 512 columns (the whole SM's, one CTA per SM)
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&tmem_base_sh)));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;");
+  const uint32_t tmem_base = tmem_base_sh;
+
+  if (warp == 0) {
+    // ===== TMA producer =====
+    if (lane == 0) {
+      int stage = 0;
+      uint32_t phase = 0;
+      const uint32_t tx = A_BYTES + uint32_t(p.n1 + p.n2) * BK * 4;
+      for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const int row0 = int((item / p.passes) * BM), col0 = int(item % p.passes) * p.n_pass;
+        for (int kc = 0; kc < p.k_chunks; ++kc) {
+          mbar_wait(&empty_bar[stage], phase ^ 1);
+          unsigned char *sa = smem + stage * STAGE_BYTES, *sb = sa + A_BYTES;
+          mbar_expect_tx(&full_bar[stage], tx);
+          tma_load_2d(sa, &map_g, kc * BK, row0, &full_bar[stage]);
+          tma_load_2d(sb, &map_w1, kc * BK, col0, &full_bar[stage]);
+          if (p.n2) tma_load_2d(sb + p.n1 * BK * 4, &map_w2, kc * BK, col0 + p.n1, &full_bar[stage]);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer =====
+    if (lane == 0) {
+      int stage = 0;
+      uint32_t phase = 0, acc_phase = 0;
+      const uint32_t idesc1 = make_idesc(BM, p.n1), idesc2 = make_idesc(BM, p.n2 ? p.n2 : 16);
+      for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+        mbar_wait(&tmem_empty_bar, acc_phase ^ 1);          // epilogue has drained the accumulator
+        asm volatile("tcgen05.fence::after_thread_sync;");
+        for (int kc = 0; kc < p.k_chunks; ++kc) {
+          mbar_wait(&full_bar[stage], phase);
+          asm volatile("tcgen05.fence::after_thread_sync;");
+          const uint32_t sa = smem_u32(smem + stage * STAGE_BYTES), sb = sa + A_BYTES;
+#pragma unroll
+          for (int k = 0; k < BK / UMMA_K; ++k) {
+            const uint64_t a_desc = make_smem_desc(sa + k * UMMA_K * 4);
+            umma_tf32(tmem_base, a_desc, make_smem_desc(sb + k * UMMA_K * 4), idesc1, (kc | k) != 0);
+            if (p.n2)
+              umma_tf32(tmem_base + p.n1, a_desc, make_smem_desc(sb + p.n1 * BK * 4 + k * UMMA_K * 4), idesc2,
+                        (kc | k) != 0);
+          }
+          umma_commit(&empty_bar[stage]);                   // frees the smem slot when the MMAs retire
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+        umma_commit(&tmem_full_bar);                        // accumulator complete
+        acc_phase ^= 1;
+      }
+    }
+  } else {
+    // ===== epilogue: warps 2..5 own TMEM lanes 32*(warp%4) .. +31 =====
+    const int lane_base = (warp & 3) * 32;
+    uint32_t acc_phase = 0;
+    for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+      const int64_t row = (item / p.passes) * BM + lane_base + lane;
+      const int col0 = int(item % p.passes) * p.n_pass;
+      mbar_wait(&tmem_full_bar, acc_phase);
+      asm volatile("tcgen05.fence::after_thread_sync;");
+      float *drow = p.D + row * p.n_pad;
+      for (int c = 0; c < p.n_pass; c += 16) {
+        uint32_t r[16];
+        const uint32_t taddr = tmem_base + (uint32_t(lane_base) << 16) + uint32_t(c);
+        asm volatile(
+            "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+            : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+              "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+            : "r"(taddr));
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        if (row < p.rows && col0 + c < p.n_pad) {
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            float4 *ptr = reinterpret_cast<float4 *>(drow + col0 + c + 4 * q);
+            float4 v = *ptr;
+            v.x += __uint_as_float(r[4 * q]);
+            v.y += __uint_as_float(r[4 * q + 1]);
+            v.z += __uint_as_float(r[4 * q + 2]);
+            v.w += __uint_as_float(r[4 * q + 3]);
+            *ptr = v;
+          }
+        }
+      }
+      asm volatile("tcgen05.fence::before_thread_sync;");
+      mbar_arrive(&tmem_empty_bar);
+      acc_phase ^= 1;
+    }
+  }
+  __syncthreads();
+  if (warp == 1) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base));
+  }
+}
+
+// ---- host: tensor maps --------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+// 2-D fp32 row-major tensor [rows][cols] (cols contiguous, row pitch `pitch` elements), box [box_rows][32]
+bool make_map(CUtensorMap *map, const void *base, uint64_t rows, uint64_t cols, uint64_t pitch, uint32_t box_rows) {
+  EncodeTiledFn enc = get_encode();
+  if (!enc) return false;
+  const cuuint64_t dims[2] = {cols, rows};
+  const cuuint64_t strides[1] = {pitch * sizeof(float)};
+  const cuuint32_t box[2] = {BK, box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void *>(base), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+// returns #launches, or -1 if the configuration is unsupported (caller falls back to the SIMT GEMM)
+int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s) {
+  if (bv.cells == 0) return 0;
+  GemmParams p{};
+  p.D = static_cast<float *>(bv.field[F_D]);
+  p.rows = bv.cells * 3;
+  p.n_pad = td.n_pad;
+  p.passes = (td.n_pad + MAX_NPASS - 1) / MAX_NPASS;
+  p.n_pass = ((td.n_pad + p.passes - 1) / p.passes + 15) / 16 * 16;
+  if (p.n_pass > MAX_NPASS) return -1;
+  p.n1 = p.n_pass > 256 ? 256 : p.n_pass;
+  p.n2 = p.n_pass - p.n1;
+  p.k_chunks = (td.n_pad + BK - 1) / BK;
+  p.m_tiles = (p.rows + BM - 1) / BM;
+  CUtensorMap map_g, map_w1, map_w2;
+  if (!make_map(&map_g, bv.field[F_G], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), BM)) return -1;
+  if (!make_map(&map_w1, td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n1))) return -1;
+  if (!make_map(&map_w2, td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad),
+                uint32_t(p.n2 ? p.n2 : 16)))
+    return -1;
+  static bool attr = false;
+  if (!attr) {
+    if (cudaFuncSetAttribute(global_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES) != cudaSuccess)
+      return -1;
+    attr = true;
+  }
+  const int64_t items = p.m_tiles * p.passes;
+  // the passes of one M tile are adjacent items: they run on neighbouring CTAs at about the same
+  // time, so the second read of the G tile is an L2 hit
+  const unsigned grid = unsigned(items < n_sm ? items : n_sm);
+  global_tcgen05_kernel<<<grid, 192, SMEM_BYTES, s>>>(map_g, map_w1, map_w2, p);
+  return 1;
+}
+
+}  // namespace npfem

@@ -92,6 +92,8 @@ int launch_objective(const TypeDev &td, const BucketView &bv, const int64_t *cel
 
 // global step: d <- d - g Hinv   ([3 cells x n_pad] . [n_pad x n_pad])
 int launch_global_simt(const TypeDev &td, const BucketView &bv, int precision, cudaStream_t s);
+// fp32 contexts, TF32 tensor cores (tcgen05); returns -1 when the shape is unsupported
+int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
 
 int launch_monotone_flags(const double *history, int n_entries, int64_t cells, int32_t *flags, cudaStream_t s);
 

@@ -156,3 +156,23 @@ def test_objective_history_matches_oracle(precision):
     scale = np.abs(ref).max()
     assert np.abs(hist - ref).max() < (1e-9 if precision == "fp64" else 2e-3) * scale
     assert np.all(mono == 1)
+
+
+def test_tf32_tensor_core_global_step_vs_fp32_ffma():
+    """The tcgen05/TF32 global step and the exact FP32-FFMA global step give the same trajectory up
+    to TF32 rounding of the (small) increment; both stay within the fp32 bar against the oracle."""
+    from paper_1911_03062_b200 import binding
+    pop = make_config(3, n_cells=90)                  # 82 RBC (246 rows: 2 M tiles, ragged) + 8 PLT
+    tf32, s1 = run_gpu(pop, "fp32", n_steps=3, n_iterations=5, options=[(binding.OPT_GLOBAL_STEP_MATH, 0)])
+    ffma, s2 = run_gpu(pop, "fp32", n_steps=3, n_iterations=5, options=[(binding.OPT_GLOBAL_STEP_MATH, 1)])
+    s1.close()
+    s2.close()
+    ref = run_oracle(pop, 3, 5)
+    for t in range(2):
+        x0 = pop.positions[t]
+        d_tf32, d_ffma, d_ref = tf32[t][0] - x0, ffma[t][0] - x0, ref[t][0] - x0
+        print(pop.types[t].name, "tf32 vs ffma", rel_l2(d_tf32, d_ffma), "tf32 vs oracle", rel_l2(d_tf32, d_ref),
+              "ffma vs oracle", rel_l2(d_ffma, d_ref))
+        assert rel_l2(d_tf32, d_ffma) < 2e-3
+        assert rel_l2(tf32[t][0], ref[t][0]) < 1e-4
+        assert rel_l2(d_tf32, d_ref) < 5e-3
