@@ -28,7 +28,7 @@ struct npfem_ctx {
   size_t ws_bytes = 0;
   bool ws_owned = false, ready = false;
   struct Layout {
-    std::vector<size_t> type_off[11];     // per type: tri, nbr, rest, hinge, corner, vnbr, w, mass, inv_area, Hinv, Hinv_tf32
+    std::vector<size_t> type_off[14];     // per type: tri, nbr, rest, hinge, corner, vnbr, w, mass, inv_area, Hinv, Hinv_tf32
     std::vector<size_t> field_off[F_COUNT], origin_off, cellid_off, scratch_off;
     size_t views_off = 0, refs_all_off = 0, refs_tmp_off = 0, stage_a_off = 0, stage_b_off = 0, total = 0;
   } lay;
@@ -160,6 +160,10 @@ void compute_layout(npfem_ctx *c) {
     L.type_off[8][t] = take(n * es);
     L.type_off[9][t] = take(np * np * es);
     L.type_off[10][t] = take(c->precision == NPFEM_F32 ? np * np * 4 : 0);
+    const bool f32 = c->precision == NPFEM_F32;
+    L.type_off[11][t] = take(f32 ? T * 16 : 0);
+    L.type_off[12][t] = take(f32 ? n * 16 : 0);
+    L.type_off[13][t] = take(f32 ? n * 4 : 0);
     const size_t cells = size_t(c->buckets[t].cells);
     for (int f = 0; f < F_COUNT; ++f) L.field_off[f][t] = take(cells * 3 * np * es);
     L.origin_off[t] = take(cells * 3 * sizeof(double));
@@ -262,6 +266,36 @@ int ensure_ready(npfem_ctx *c) {
     d.beta_over_h = m.rayleigh_beta / h.h;
     d.inertia_coef = (1.0 + h.h * m.rayleigh_alpha) / (h.h * h.h);
     d.kappa = m.kappa_damping;
+    d.gamma = d.beta_over_h / (1.0 + d.beta_over_h);
+    if (c->precision == NPFEM_F32 && h.valence_max <= 8 && h.n < 65535 && 3 * h.T + 1 <= 65535) {
+      // packed tables of the shared-memory local step
+      std::vector<uint32_t> tri_pack(size_t(h.T) * 4), vtx_pack(size_t(h.n) * 4);
+      for (int tt = 0; tt < h.T; ++tt) {
+        const int32_t *v = &h.tri[4 * tt], *nb = &h.tri_nbr[4 * tt];
+        tri_pack[4 * tt + 0] = uint32_t(v[0]) | (uint32_t(v[1]) << 16);
+        tri_pack[4 * tt + 1] = uint32_t(v[2]) | (uint32_t(nb[0]) << 16);
+        tri_pack[4 * tt + 2] = uint32_t(nb[1]) | (uint32_t(nb[2]) << 16);
+        tri_pack[4 * tt + 3] = 0;
+      }
+      std::vector<float> coef(h.n);
+      for (int v = 0; v < h.n; ++v) {
+        uint32_t ids[8];
+        for (int q = 0; q < 8; ++q) {
+          const int32_t cid = q < h.valence_max ? h.vtx_corner[size_t(q) * h.n + v] : -1;
+          ids[q] = cid >= 0 ? uint32_t(cid) : uint32_t(3 * h.T);
+        }
+        for (int q = 0; q < 4; ++q) vtx_pack[4 * v + q] = ids[2 * q] | (ids[2 * q + 1] << 16);
+        coef[v] = float((1.0 - d.gamma) * d.inertia_coef * h.mass[v]);
+      }
+      if (h.T < 65536) {
+        if ((rc = upload_raw(c, L.type_off[11][t], tri_pack))) return rc;
+        if ((rc = upload_raw(c, L.type_off[12][t], vtx_pack))) return rc;
+        if ((rc = upload_raw(c, L.type_off[13][t], coef))) return rc;
+        d.tri_pack = c->ws + L.type_off[11][t];
+        d.vtx_pack = c->ws + L.type_off[12][t];
+        d.vtx_coef = c->ws + L.type_off[13][t];
+      }
+    }
 
     // dense inverse of H~ on the device (fp64), then cast/pad to the compute type
     double *H64 = nullptr, *Hinv64 = nullptr;
@@ -595,16 +629,19 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   for (int k = 0; k < n_iterations; ++k) {
     if (c->diagnostics && (rc = diag(k))) return rc;
     for (size_t t = 0; t < nb; ++t) {
+      const bool fast = c->precision == NPFEM_F32 && c->opt_local_impl != 1 && local_smem_supported(c->types[t]);
+      const double d_scale = fast ? 1.0 - c->types[t].gamma : 1.0;
       if ((rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "local step", [&] {
+             if (fast) return launch_local_smem(c->types[t], c->views[t], c->n_sm, c->stream);
              return launch_local_generic(c->types[t], c->views[t], c->buckets[t].scratch, c->precision, c->n_sm,
                                          c->stream); })))
         return rc;
       if ((rc = timed_launch(c, NPFEM_KIND_GLOBAL, int(t), "global step", [&] {
              if (c->precision == NPFEM_F32 && c->opt_global_math == 0) {
-               const int n = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, c->stream);
+               const int n = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, d_scale, c->stream);
                if (n >= 0) return n;
              }
-             return launch_global_simt(c->types[t], c->views[t], c->precision, c->stream); })))
+             return launch_global_simt(c->types[t], c->views[t], c->precision, d_scale, c->stream); })))
         return rc;
     }
   }

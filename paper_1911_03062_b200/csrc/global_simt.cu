@@ -12,7 +12,7 @@ namespace {
 
 template <typename T, int BM, int BN, int BK, int TM, int TN>
 __global__ void __launch_bounds__((BM / TM) * (BN / TN))
-global_simt_kernel(const T *__restrict__ G, const T *__restrict__ W, T *__restrict__ D, int64_t rows, int n_pad) {
+global_simt_kernel(const T *__restrict__ G, const T *__restrict__ W, T *__restrict__ D, int64_t rows, int n_pad, T d_scale) {
   constexpr int NT = (BM / TM) * (BN / TN);
   __shared__ T Gs[BK][BM + 4];
   __shared__ T Ws[BK][BN];
@@ -50,13 +50,13 @@ global_simt_kernel(const T *__restrict__ G, const T *__restrict__ W, T *__restri
     for (int j = 0; j < TN; ++j) {
       const int64_t r = row0 + ty + (BM / TM) * i;
       const int c = col0 + tx + (BN / TN) * j;
-      if (r < rows && c < n_pad) D[r * n_pad + c] -= acc[i][j];
+      if (r < rows && c < n_pad) D[r * n_pad + c] = d_scale * D[r * n_pad + c] - acc[i][j];
     }
 }
 
 }  // namespace
 
-int launch_global_simt(const TypeDev &td, const BucketView &bv, int precision, cudaStream_t s) {
+int launch_global_simt(const TypeDev &td, const BucketView &bv, int precision, double d_scale, cudaStream_t s) {
   if (bv.cells == 0) return 0;
   const int64_t rows = bv.cells * 3;
   constexpr int BM = 64, BN = 64;
@@ -64,11 +64,11 @@ int launch_global_simt(const TypeDev &td, const BucketView &bv, int precision, c
   if (precision == NPFEM_F32)
     global_simt_kernel<float, BM, BN, 16, 4, 4><<<grid, 256, 0, s>>>(
         static_cast<const float *>(bv.field[F_G]), static_cast<const float *>(td.Hinv),
-        static_cast<float *>(bv.field[F_D]), rows, td.n_pad);
+        static_cast<float *>(bv.field[F_D]), rows, td.n_pad, float(d_scale));
   else
     global_simt_kernel<double, BM, BN, 16, 4, 4><<<grid, 256, 0, s>>>(
         static_cast<const double *>(bv.field[F_G]), static_cast<const double *>(td.Hinv),
-        static_cast<double *>(bv.field[F_D]), rows, td.n_pad);
+        static_cast<double *>(bv.field[F_D]), rows, td.n_pad, d_scale);
   return 1;
 }
 

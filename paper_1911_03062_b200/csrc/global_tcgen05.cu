@@ -101,6 +101,7 @@ struct GemmParams {
   int n1, n2;          // columns of the two MMA instructions of a pass (n1 <= 256, n2 may be 0)
   int k_chunks;        // ceil(n_pad / BK)
   int64_t m_tiles;
+  float d_scale;       // d <- d_scale * d + acc
 };
 
 __global__ void __launch_bounds__(192, 1)
@@ -202,10 +203,10 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
           for (int q = 0; q < 4; ++q) {
             float4 *ptr = reinterpret_cast<float4 *>(drow + col0 + c + 4 * q);
             float4 v = *ptr;
-            v.x += __uint_as_float(r[4 * q]);
-            v.y += __uint_as_float(r[4 * q + 1]);
-            v.z += __uint_as_float(r[4 * q + 2]);
-            v.w += __uint_as_float(r[4 * q + 3]);
+            v.x = p.d_scale * v.x + __uint_as_float(r[4 * q]);
+            v.y = p.d_scale * v.y + __uint_as_float(r[4 * q + 1]);
+            v.z = p.d_scale * v.z + __uint_as_float(r[4 * q + 2]);
+            v.w = p.d_scale * v.w + __uint_as_float(r[4 * q + 3]);
             *ptr = v;
           }
         }
@@ -254,7 +255,7 @@ bool make_map(CUtensorMap *map, const void *base, uint64_t rows, uint64_t cols, 
 }  // namespace
 
 // returns #launches, or -1 if the configuration is unsupported (caller falls back to the SIMT GEMM)
-int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s) {
+int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, double d_scale, cudaStream_t s) {
   if (bv.cells == 0) return 0;
   GemmParams p{};
   p.D = static_cast<float *>(bv.field[F_D]);
@@ -267,6 +268,7 @@ int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, cud
   p.n2 = p.n_pass - p.n1;
   p.k_chunks = (td.n_pad + BK - 1) / BK;
   p.m_tiles = (p.rows + BM - 1) / BM;
+  p.d_scale = float(d_scale);
   CUtensorMap map_g, map_w1, map_w2;
   if (!make_map(&map_g, bv.field[F_G], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), BM)) return -1;
   if (!make_map(&map_w1, td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n1))) return -1;

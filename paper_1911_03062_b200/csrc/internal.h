@@ -28,7 +28,12 @@ struct TypeDev {
   const void *vtx_mass = nullptr;    // [n]  m_v
   const void *vtx_inv_area = nullptr;// [n]  1/A_v
   const void *Hinv = nullptr;        // [n_pad][n_pad] dense inverse of H~ (compute type)
-  const void *Hinv_tf32 = nullptr;   // fp32 contexts: same, rounded to TF32, tiled for tcgen05 (may be null)
+  const void *Hinv_tf32 = nullptr;
+  // fp32 shared-memory local step (local_smem.cu)
+  const void *tri_pack = nullptr;    // [T] uint4: v0|v1<<16, v2|n0<<16, n1|n2<<16, 0
+  const void *vtx_pack = nullptr;    // [n] uint4: 8 x u16 corner ids (3T = none)
+  const void *vtx_coef = nullptr;    // [n] float: (1 - gamma)(1 + h alpha) m_v / h^2
+  double gamma = 0;                  // (beta/h) / (1 + beta/h)   // fp32 contexts: same, rounded to TF32, tiled for tcgen05 (may be null)
   // scalars (double; converted at launch)
   double h = 0, B4 = 0, C4 = 0, k_b = 0, kv_over_V0 = 0, V0 = 0, k_mem = 0, beta_over_h = 0;
   double inertia_coef = 0;           // (1 + h alpha) / h^2, multiplies m_v
@@ -91,9 +96,13 @@ int launch_objective(const TypeDev &td, const BucketView &bv, const int64_t *cel
                      int precision, cudaStream_t s);
 
 // global step: d <- d - g Hinv   ([3 cells x n_pad] . [n_pad x n_pad])
-int launch_global_simt(const TypeDev &td, const BucketView &bv, int precision, cudaStream_t s);
+int launch_global_simt(const TypeDev &td, const BucketView &bv, int precision, double d_scale, cudaStream_t s);
 // fp32 contexts, TF32 tensor cores (tcgen05); returns -1 when the shape is unsupported
-int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
+int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, double d_scale, cudaStream_t s);
+
+// fp32 fast local step; writes the reduced gradient (global step must then use d_scale = 1 - gamma)
+bool local_smem_supported(const TypeDev &td);
+int launch_local_smem(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
 
 int launch_monotone_flags(const double *history, int n_entries, int64_t cells, int32_t *flags, cudaStream_t s);
 
