@@ -7,6 +7,7 @@
 #include <new>
 
 #include "internal.h"
+#include "local_schedule.hpp"
 
 using namespace npfem;
 
@@ -16,6 +17,7 @@ struct npfem_ctx {
   double dt = 0;
   int64_t n_cells = 0, total_vertices = 0;
   std::vector<HostTypeData> host_types;
+  std::vector<LocalSchedule> sched;       // fp32 contexts: scheduled local step, per type (may be invalid)
   std::vector<TypeDev> types;
   std::vector<Bucket> buckets;            // one per type
   std::vector<BucketView> views;
@@ -28,7 +30,7 @@ struct npfem_ctx {
   size_t ws_bytes = 0;
   bool ws_owned = false, ready = false;
   struct Layout {
-    std::vector<size_t> type_off[14];     // per type: tri, nbr, rest, hinge, corner, vnbr, w, mass, inv_area, Hinv, Hinv_tf32
+    std::vector<size_t> type_off[18];     // per type: tri, nbr, rest, hinge, corner, vnbr, w, mass, inv_area, Hinv, Hinv_tf32
     std::vector<size_t> field_off[F_COUNT], origin_off, cellid_off, scratch_off;
     size_t views_off = 0, refs_all_off = 0, refs_tmp_off = 0, stage_a_off = 0, stage_b_off = 0, total = 0;
   } lay;
@@ -164,6 +166,11 @@ void compute_layout(npfem_ctx *c) {
     L.type_off[11][t] = take(f32 ? T * 16 : 0);
     L.type_off[12][t] = take(f32 ? n * 16 : 0);
     L.type_off[13][t] = take(f32 ? n * 4 : 0);
+    const LocalSchedule &sc = c->sched[t];
+    L.type_off[14][t] = take(sc.valid ? sc.tri_words.size() * 4 : 0);
+    L.type_off[15][t] = take(sc.valid ? sc.tri_consts.size() * 4 : 0);
+    L.type_off[16][t] = take(sc.valid ? sc.vtx_words.size() * 4 : 0);
+    L.type_off[17][t] = take(sc.valid ? sc.vtx_coef.size() * 4 : 0);
     const size_t cells = size_t(c->buckets[t].cells);
     for (int f = 0; f < F_COUNT; ++f) L.field_off[f][t] = take(cells * 3 * np * es);
     L.origin_off[t] = take(cells * 3 * sizeof(double));
@@ -295,6 +302,21 @@ int ensure_ready(npfem_ctx *c) {
         d.vtx_pack = c->ws + L.type_off[12][t];
         d.vtx_coef = c->ws + L.type_off[13][t];
       }
+    }
+    if (c->sched[t].valid) {
+      const LocalSchedule &sc = c->sched[t];
+      if ((rc = upload_raw(c, L.type_off[14][t], sc.tri_words))) return rc;
+      if ((rc = upload_raw(c, L.type_off[15][t], sc.tri_consts))) return rc;
+      if ((rc = upload_raw(c, L.type_off[16][t], sc.vtx_words))) return rc;
+      if ((rc = upload_raw(c, L.type_off[17][t], sc.vtx_coef))) return rc;
+      SchedDev &sd = d.sched;
+      sd.valid = true;
+      sd.threads = sc.threads; sd.vstride = sc.vstride; sd.tpt = sc.tpt; sd.ttri = sc.ttri; sd.maxv = sc.maxv;
+      sd.n_vslots = sc.n_vslots; sd.n_tslots = sc.n_tslots; sd.n_cslots = sc.n_cslots;
+      sd.tri_words = reinterpret_cast<const uint32_t *>(c->ws + L.type_off[14][t]);
+      sd.tri_consts = reinterpret_cast<const float *>(c->ws + L.type_off[15][t]);
+      sd.vtx_words = reinterpret_cast<const uint32_t *>(c->ws + L.type_off[16][t]);
+      sd.vtx_coef = reinterpret_cast<const float *>(c->ws + L.type_off[17][t]);
     }
 
     // dense inverse of H~ on the device (fp64), then cast/pad to the compute type
@@ -428,6 +450,7 @@ int npfem_create(npfem_ctx **out, const npfem_cell_type *types, int32_t n_types,
   c->n_cells = n_cells;
   try {
     c->host_types.resize(size_t(n_types));
+    c->sched.resize(size_t(n_types));
     c->buckets.resize(size_t(n_types));
     for (int t = 0; t < n_types; ++t) {
       std::string err;
@@ -437,6 +460,11 @@ int npfem_create(npfem_ctx **out, const npfem_cell_type *types, int32_t n_types,
         return fail(nullptr, rc, "cell type " + std::to_string(t) + ": " + err);
       }
       c->buckets[t].type = t;
+      if (precision == NPFEM_F32) {
+        const HostTypeData &h = c->host_types[t];
+        const int tpt = h.T <= 320 ? 1 : 2;
+        build_local_schedule(h, types[t].rest_positions, tpt, c->sched[t]);   // may stay invalid
+      }
     }
     c->type_of_cell.assign(type_of_cell, type_of_cell + n_cells);
     c->slot_of_cell.resize(size_t(n_cells));
@@ -507,7 +535,7 @@ int npfem_set_option(npfem_ctx *c, int32_t option, int64_t value) {
       c->opt_global_math = value;
       return NPFEM_OK;
     case NPFEM_OPT_LOCAL_STEP_IMPL:
-      if (value < 0 || value > 2) return fail(c, NPFEM_EINVAL, "local-step impl must be 0, 1 or 2");
+      if (value < 0 || value > 3) return fail(c, NPFEM_EINVAL, "local-step impl must be 0, 1, 2 or 3");
       c->opt_local_impl = value;
       return NPFEM_OK;
     case NPFEM_OPT_KERNEL_TIMING: c->timing = value != 0; return NPFEM_OK;
@@ -629,9 +657,12 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   for (int k = 0; k < n_iterations; ++k) {
     if (c->diagnostics && (rc = diag(k))) return rc;
     for (size_t t = 0; t < nb; ++t) {
-      const bool fast = c->precision == NPFEM_F32 && c->opt_local_impl != 1 && local_smem_supported(c->types[t]);
-      const double d_scale = fast ? 1.0 - c->types[t].gamma : 1.0;
+      const bool f32 = c->precision == NPFEM_F32;
+      const bool sched = f32 && (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]);
+      const bool fast = f32 && !sched && c->opt_local_impl != 1 && local_smem_supported(c->types[t]);
+      const double d_scale = (sched || fast) ? 1.0 - c->types[t].gamma : 1.0;
       if ((rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "local step", [&] {
+             if (sched) return launch_local_sched(c->types[t], c->views[t], c->n_sm, c->stream);
              if (fast) return launch_local_smem(c->types[t], c->views[t], c->n_sm, c->stream);
              return launch_local_generic(c->types[t], c->views[t], c->buckets[t].scratch, c->precision, c->n_sm,
                                          c->stream); })))

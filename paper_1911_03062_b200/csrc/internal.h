@@ -15,6 +15,16 @@ namespace npfem {
 // Number of state fields kept per bucket, each [cells][3][n_pad] of the compute type.
 enum Field { F_X = 0, F_V, F_F, F_B, F_D, F_G, F_COUNT };
 
+// Device tables of the scheduled fp32 local step (local_schedule.hpp / local_sched.cu).
+struct SchedDev {
+  bool valid = false;
+  int threads = 0, vstride = 0, tpt = 0, ttri = 0, maxv = 0, n_vslots = 0, n_tslots = 0, n_cslots = 0;
+  const uint32_t *tri_words = nullptr;
+  const float *tri_consts = nullptr;
+  const uint32_t *vtx_words = nullptr;
+  const float *vtx_coef = nullptr;
+};
+
 // Device view of one cell type (pointers into the workspace; element type = compute type).
 struct TypeDev {
   int n = 0, T = 0, n_pad = 0, valence_max = 0;
@@ -38,6 +48,7 @@ struct TypeDev {
   double h = 0, B4 = 0, C4 = 0, k_b = 0, kv_over_V0 = 0, V0 = 0, k_mem = 0, beta_over_h = 0;
   double inertia_coef = 0;           // (1 + h alpha) / h^2, multiplies m_v
   double kappa = 0;
+  SchedDev sched;                    // fp32 contexts: scheduled local step (may be invalid)
 };
 
 // One bucket = all cells of one type, contiguous slots.
@@ -103,6 +114,11 @@ int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, dou
 // fp32 fast local step; writes the reduced gradient (global step must then use d_scale = 1 - gamma)
 bool local_smem_supported(const TypeDev &td);
 int launch_local_smem(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
+
+// fp32 scheduled local step (register-resident topology, conflict-free shared-memory slots); same
+// reduced-gradient convention as launch_local_smem
+bool local_sched_supported(const TypeDev &td);
+int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
 
 int launch_monotone_flags(const double *history, int n_entries, int64_t cells, int32_t *flags, cudaStream_t s);
 

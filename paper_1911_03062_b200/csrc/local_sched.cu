@@ -1,0 +1,338 @@
+// Local step (row a2), fp32 "scheduled" path: g = M~ d/h^2 - b + grad E(x_n + d) in its reduced
+// form  r = (1 - gamma) m^ d - b + grad E(x_n + d)  (see local_smem.cu for the derivation; the global
+// step applies the (1 - gamma) factor), Eqs. (3)-(4), energies = readings R5-R9.
+//
+// Design (profiles/r1_ncu_full_v3.md showed shared-memory wavefronts, 37 % of them bank conflicts,
+// and the instruction count binding the previous kernel):
+//   * persistent CTAs, one cell at a time; every thread owns the SAME TPT triangles and the same
+//     vertex for the whole launch, so all per-TYPE constants (connectivity as 16-bit shared-memory
+//     byte offsets, the rest metric R = Dm^-1 Dm^-T, det^2, pre-multiplied material constants,
+//     k_b (cos, sin) theta0 of the three hinges) live in REGISTERS, loaded once per launch;
+//   * the shared-memory slots of vertex positions, unit normals and corner forces are assigned at
+//     create time by graph colouring (local_schedule.hpp): the owner's store and the three gathers
+//     are (nearly) bank-conflict-free;
+//   * membrane gradient from the metric G = [e_i . e_j]:  I1 + 1 = tr(R G) - 1,
+//     I2 = det(Dm^-1)^2 |e1 x e2|^2 - 1,  [g1 g2] = [e1 e2] Q,  Q = 2 A0 (W1 R + W2 det^2 adj G);
+//   * hinges from UNIT normals stored once per triangle (1 rsqrt per triangle instead of 3);
+//   * cell volume: per-warp float partial -> fixed-point shared atomics on two 32-bit digits
+//     (exact, order independent, deterministic);
+//   * x_n, d, b of the next cells stream in through 1-D TMA bulk copies (cp.async.bulk + mbarrier)
+//     into a NSTAGE-deep ring, issued NSTAGE-1 cells ahead.
+// Phases per cell (3 block barriers):
+//   0  stage -> sx[slot(v)] = (x_n + d, 0)                                           | barrier 1
+//   A  per triangle: e1, e2, unit normal, 1/|N| -> sN[slot(t)]; volume partial       | barrier 2
+//   B  per triangle: membrane + 3 hinge sides + volume term -> 3 corner forces in sC | barrier 3
+//   C  per vertex: gather <= MAXV corner forces, r = coef d - b + sum -> global
+#include "internal.h"
+
+namespace npfem {
+namespace {
+
+constexpr int NSTAGE = 3;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return uint32_t(__cvta_generic_to_shared(p)); }
+
+struct SchedParams {
+  int n, T, n_pad, ttri, threads, vstride;
+  int sx_bytes, sN_bytes, sC_bytes;
+  const uint32_t *tri_words;   // [TPT][5][threads]
+  const float *tri_consts;     // [TPT][12][threads]
+  const uint32_t *vtx_words;   // [1 + MAXV/2][vstride]
+  const float *vtx_coef;       // [vstride]
+  double fx_scale, fx_inv;     // fixed-point scale of the 6 V accumulator and its inverse
+  double V0x6, kv_coef;        // 6 V0;  k_v / (36 V0):  vc = kv_coef (6V - 6V0) = k_v (V - V0)/V0 / 6
+  const float *x, *d, *b;      // [cells][3][n_pad]
+  float *g;
+  int64_t cells;
+};
+
+// plain MUFU.RSQ: no denormal rescue (squared edge lengths / areas of a live mesh are normal numbers)
+__device__ __forceinline__ float rsqrt_fast(float x) {
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float4 lds4(const unsigned char *base, uint32_t off) {
+  return *reinterpret_cast<const float4 *>(base + off);
+}
+__device__ __forceinline__ void sts4(unsigned char *base, uint32_t off, float x, float y, float z, float w) {
+  *reinterpret_cast<float4 *>(base + off) = make_float4(x, y, z, w);
+}
+
+template <int TPT, int MAXV, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedParams p) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const int n = p.n, n_pad = p.n_pad, nthreads = p.threads;
+  unsigned char *sx = smem;
+  unsigned char *sN = sx + p.sx_bytes;
+  unsigned char *sC = sN + p.sN_bytes;
+  float *stage = reinterpret_cast<float *>(sC + p.sC_bytes);            // [NSTAGE][3 fields][3][n_pad]
+  int *vacc = reinterpret_cast<int *>(stage + NSTAGE * 9 * n_pad);   // [2 cells][hi, lo] base-2^24 digits of 6V
+  uint64_t *mbar = reinterpret_cast<uint64_t *>(vacc + 4);
+
+  const int tid = threadIdx.x, lane = tid & 31;
+  const uint32_t field_bytes = uint32_t(3 * n_pad) * 4u;
+
+  // ---- per-thread constants: registers for the whole launch ---------------------------------
+  uint32_t tw[TPT][5];
+  float tk[TPT][12];
+  bool act[TPT];
+#pragma unroll
+  for (int j = 0; j < TPT; ++j) {
+    act[j] = tid < p.ttri && j * p.ttri + tid < p.T;
+#pragma unroll
+    for (int q = 0; q < 5; ++q) tw[j][q] = p.tri_words[(j * 5 + q) * nthreads + tid];
+#pragma unroll
+    for (int q = 0; q < 12; ++q) tk[j][q] = p.tri_consts[(j * 12 + q) * nthreads + tid];
+  }
+  uint32_t vw[1 + MAXV / 2];
+#pragma unroll
+  for (int q = 0; q < 1 + MAXV / 2; ++q) vw[q] = p.vtx_words[q * p.vstride + tid];
+  const float coef = p.vtx_coef[tid];
+  const bool vact = tid < n;
+  const int v2 = tid + nthreads;       // a few vertices may need a second pass (n slightly above the CTA size):
+  const bool vact2 = v2 < n;           // their constants stay in global memory (L1/L2 hits)
+
+  auto prefetch = [&](int64_t cell, int st) {   // one thread: arm the barrier, start 3 bulk copies
+    const size_t base = size_t(cell) * 3 * n_pad;
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar + st)),
+                 "r"(3 * field_bytes) : "memory");
+    const float *src[3] = {p.x + base, p.d + base, p.b + base};
+#pragma unroll
+    for (int f = 0; f < 3; ++f)
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                   ::"r"(smem_u32(stage + (st * 9 + f * 3) * n_pad)), "l"(src[f]), "r"(field_bytes),
+                     "r"(smem_u32(mbar + st)) : "memory");
+  };
+
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < NSTAGE; ++s) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(mbar + s)));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    vacc[0] = vacc[1] = vacc[2] = vacc[3] = 0;
+  }
+  if (tid < 8) sts4(sC, uint32_t(p.sC_bytes) - 128u + 16u * tid, 0.f, 0.f, 0.f, 0.f);   // the zero slots
+  __syncthreads();
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < NSTAGE - 1; ++s) {
+      const int64_t c = int64_t(blockIdx.x) + int64_t(s) * gridDim.x;
+      if (c < p.cells) prefetch(c, s);
+    }
+  }
+
+  int it = 0;
+  for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x, ++it) {
+    const int st = it % NSTAGE;
+    const float *sg = stage + st * 9 * n_pad;
+    // ---- phase 0 ----------------------------------------------------------------------------
+    {
+      const uint32_t parity = uint32_t(it / NSTAGE) & 1u;
+      uint32_t done;
+      do {
+        asm volatile(
+            "{\n.reg .pred q;\nmbarrier.try_wait.parity.shared::cta.b64 q, [%1], %2;\nselp.u32 %0, 1, 0, q;\n}\n"
+            : "=r"(done) : "r"(smem_u32(mbar + st)), "r"(parity) : "memory");
+      } while (!done);
+    }
+    if (vact)
+      sts4(sx, vw[0] & 0xffffu, sg[tid] + sg[3 * n_pad + tid], sg[n_pad + tid] + sg[4 * n_pad + tid],
+           sg[2 * n_pad + tid] + sg[5 * n_pad + tid], 0.f);
+    if (vact2)
+      sts4(sx, p.vtx_words[v2] & 0xffffu, sg[v2] + sg[3 * n_pad + v2], sg[n_pad + v2] + sg[4 * n_pad + v2],
+           sg[2 * n_pad + v2] + sg[5 * n_pad + v2], 0.f);
+    if (tid == 0) vacc[2 * ((it + 1) & 1)] = vacc[2 * ((it + 1) & 1) + 1] = 0;
+    __syncthreads();                                   // barrier 1: sx complete
+    if (tid == 0) {   // ring slot (it-1) % NSTAGE was last read in phase C of the previous cell
+      const int64_t nxt = cell + int64_t(NSTAGE - 1) * gridDim.x;
+      if (nxt < p.cells) prefetch(nxt, (it + NSTAGE - 1) % NSTAGE);
+    }
+    // ---- phase A ----------------------------------------------------------------------------
+    float e1[TPT][3], e2[TPT][3], nh[TPT][3], inv[TPT], nn[TPT];
+    float vol = 0.f;
+#pragma unroll
+    for (int j = 0; j < TPT; ++j) {
+      if (act[j]) {
+        const float4 X0 = lds4(sx, tw[j][0] & 0xffffu), X1 = lds4(sx, tw[j][0] >> 16), X2 = lds4(sx, tw[j][1] & 0xffffu);
+        e1[j][0] = X1.x - X0.x; e1[j][1] = X1.y - X0.y; e1[j][2] = X1.z - X0.z;
+        e2[j][0] = X2.x - X0.x; e2[j][1] = X2.y - X0.y; e2[j][2] = X2.z - X0.z;
+        const float Nx = e1[j][1] * e2[j][2] - e1[j][2] * e2[j][1];
+        const float Ny = e1[j][2] * e2[j][0] - e1[j][0] * e2[j][2];
+        const float Nz = e1[j][0] * e2[j][1] - e1[j][1] * e2[j][0];
+        nn[j] = Nx * Nx + Ny * Ny + Nz * Nz;
+        vol += X0.x * Nx + X0.y * Ny + X0.z * Nz;      // 6 x signed tetrahedron volume
+        inv[j] = rsqrt_fast(nn[j]);
+        nh[j][0] = Nx * inv[j]; nh[j][1] = Ny * inv[j]; nh[j][2] = Nz * inv[j];
+        sts4(sN, tw[j][4] >> 16, nh[j][0], nh[j][1], nh[j][2], inv[j]);
+      }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) vol += __shfl_xor_sync(0xffffffffu, vol, o);
+    if (lane == 0) {   // exact, order-independent: fixed point, split into a signed high and a 24-bit low digit
+      const long long v = __double2ll_rn(double(vol) * p.fx_scale);
+      atomicAdd(vacc + 2 * (it & 1), int(v >> 24));
+      atomicAdd(vacc + 2 * (it & 1) + 1, int(v & 0xffffff));
+    }
+    __syncthreads();                                   // barrier 2: sN complete, volume accumulated
+    const int2 vd = *reinterpret_cast<const int2 *>(vacc + 2 * (it & 1));
+    const float vc = float(((double(vd.x) * 16777216.0 + double(vd.y)) * p.fx_inv - p.V0x6) * p.kv_coef);
+    // ---- phase B ----------------------------------------------------------------------------
+#pragma unroll
+    for (int j = 0; j < TPT; ++j) {
+      if (act[j]) {
+        const float *a1 = e1[j], *a2 = e2[j], *nA = nh[j];
+        const float e11 = a1[0] * a1[0] + a1[1] * a1[1] + a1[2] * a1[2];
+        const float e12 = a1[0] * a2[0] + a1[1] * a2[1] + a1[2] * a2[2];
+        const float e22 = a2[0] * a2[0] + a2[1] * a2[1] + a2[2] * a2[2];
+        // membrane (Skalak, readings R5/R7): Q = 2 A0 (W1 R + W2 det^2 adj G)
+        const float R11 = tk[j][0], R12 = tk[j][1], R22 = tk[j][2], J = tk[j][3], tA = tk[j][4], tC = tk[j][5];
+        const float th = fmaf(R12, e12, -0.5f);
+        const float I1p1 = fmaf(R11, e11, fmaf(R22, e22, th + th));      // I1 + 1
+        const float I2 = fmaf(J, nn[j], -1.f);
+        const float W1 = tA * I1p1, W2 = fmaf(tC, I2, -tA * J);
+        const float q11 = fmaf(W2, e22, W1 * R11), q22 = fmaf(W2, e11, W1 * R22), q12 = fmaf(-W2, e12, W1 * R12);
+        // hinges seen from this triangle (reading R8): side s runs from corner s to s+1
+        float w0 = 0.f, w1 = 0.f, w2 = 0.f;
+        {
+          const float4 NB = lds4(sN, tw[j][1] >> 16);
+          const float crx = nA[1] * NB.z - nA[2] * NB.y, cry = nA[2] * NB.x - nA[0] * NB.z, crz = nA[0] * NB.y - nA[1] * NB.x;
+          const float S = crx * a1[0] + cry * a1[1] + crz * a1[2];
+          const float cs = nA[0] * NB.x + nA[1] * NB.y + nA[2] * NB.z;
+          const float L = e11, D = e11 - e12, ie = rsqrt_fast(L);
+          const float q = ie * fmaf(S * ie, tk[j][6], -cs * tk[j][9]);   // dE/dtheta / |e|
+          w0 = fmaf(D, q, w0); w1 = fmaf(L - D, q, w1); w2 = fmaf(-L, q, w2);
+        }
+        {
+          const float4 NB = lds4(sN, tw[j][2] & 0xffffu);
+          const float crx = nA[1] * NB.z - nA[2] * NB.y, cry = nA[2] * NB.x - nA[0] * NB.z, crz = nA[0] * NB.y - nA[1] * NB.x;
+          const float S = crx * (a2[0] - a1[0]) + cry * (a2[1] - a1[1]) + crz * (a2[2] - a1[2]);
+          const float cs = nA[0] * NB.x + nA[1] * NB.y + nA[2] * NB.z;
+          const float L = e11 - 2.f * e12 + e22, D = e22 - e12, ie = rsqrt_fast(L);
+          const float q = ie * fmaf(S * ie, tk[j][7], -cs * tk[j][10]);
+          w1 = fmaf(D, q, w1); w2 = fmaf(L - D, q, w2); w0 = fmaf(-L, q, w0);
+        }
+        {
+          const float4 NB = lds4(sN, tw[j][2] >> 16);
+          const float crx = nA[1] * NB.z - nA[2] * NB.y, cry = nA[2] * NB.x - nA[0] * NB.z, crz = nA[0] * NB.y - nA[1] * NB.x;
+          const float S = -(crx * a2[0] + cry * a2[1] + crz * a2[2]);
+          const float cs = nA[0] * NB.x + nA[1] * NB.y + nA[2] * NB.z;
+          const float L = e22, D = e12, ie = rsqrt_fast(L);
+          const float q = ie * fmaf(S * ie, tk[j][8], -cs * tk[j][11]);
+          w2 = fmaf(D, q, w2); w0 = fmaf(L - D, q, w0); w1 = fmaf(-L, q, w1);
+        }
+        // corner weights along the unit normal: volume term (reading R9) + hinge terms / |N|
+        const float vn = vc * (nn[j] * inv[j]);
+        const float u0 = fmaf(inv[j], w0, vn), u1 = fmaf(inv[j], w1, vn), u2 = fmaf(inv[j], w2, vn);
+        const float us = u0 + u1 + u2;
+        float c0[3], c1[3], c2[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+          c1[k] = fmaf(u1, nA[k], fmaf(q11, a1[k], q12 * a2[k]));
+          c2[k] = fmaf(u2, nA[k], fmaf(q12, a1[k], q22 * a2[k]));
+          c0[k] = fmaf(us, nA[k], -c1[k]) - c2[k];
+        }
+        sts4(sC, tw[j][3] & 0xffffu, c0[0], c0[1], c0[2], 0.f);
+        sts4(sC, tw[j][3] >> 16, c1[0], c1[1], c1[2], 0.f);
+        sts4(sC, tw[j][4] & 0xffffu, c2[0], c2[1], c2[2], 0.f);
+      }
+    }
+    __syncthreads();                                   // barrier 3: corner forces complete
+    // ---- phase C ----------------------------------------------------------------------------
+    if (vact) {
+      float ax = 0.f, ay = 0.f, az = 0.f;
+#pragma unroll
+      for (int q = 0; q < MAXV; ++q) {
+        const uint32_t off = (q & 1) ? (vw[1 + (q >> 1)] >> 16) : (vw[1 + (q >> 1)] & 0xffffu);
+        const float4 f = lds4(sC, off);
+        ax += f.x; ay += f.y; az += f.z;
+      }
+      float *gout = p.g + size_t(cell) * 3 * n_pad + tid;
+      gout[0] = fmaf(coef, sg[3 * n_pad + tid], ax - sg[6 * n_pad + tid]);
+      gout[n_pad] = fmaf(coef, sg[4 * n_pad + tid], ay - sg[7 * n_pad + tid]);
+      gout[2 * n_pad] = fmaf(coef, sg[5 * n_pad + tid], az - sg[8 * n_pad + tid]);
+    }
+    if (vact2) {
+      float ax = 0.f, ay = 0.f, az = 0.f;
+      for (int q = 0; q < MAXV; ++q) {
+        const uint32_t w = p.vtx_words[(1 + (q >> 1)) * p.vstride + v2];
+        const float4 f = lds4(sC, (q & 1) ? (w >> 16) : (w & 0xffffu));
+        ax += f.x; ay += f.y; az += f.z;
+      }
+      const float coef2 = p.vtx_coef[v2];
+      float *gout = p.g + size_t(cell) * 3 * n_pad + v2;
+      gout[0] = fmaf(coef2, sg[3 * n_pad + v2], ax - sg[6 * n_pad + v2]);
+      gout[n_pad] = fmaf(coef2, sg[4 * n_pad + v2], ay - sg[7 * n_pad + v2]);
+      gout[2 * n_pad] = fmaf(coef2, sg[5 * n_pad + v2], az - sg[8 * n_pad + v2]);
+    }
+    // no barrier: the next phase 0 writes sx (last read in phase A) and reads another ring slot;
+    // sN / sC are rewritten only after barriers 1 / 2 of the next cell
+  }
+}
+
+}  // namespace
+
+namespace {
+
+size_t sched_smem_bytes(const SchedDev &s, int n_pad) {
+  return size_t(s.n_vslots + s.n_tslots + s.n_cslots) * 16 + size_t(NSTAGE) * 9 * n_pad * 4 + 4 * 4 + NSTAGE * 8;
+}
+
+template <int TPT, int MAXV, int MAXT, int MINB>
+int launch_variant(const SchedParams &p, size_t smem, int n_sm, int64_t cells, cudaStream_t s) {
+  auto kernel = local_sched_kernel<TPT, MAXV, MAXT, MINB>;
+  static int per_sm = 0;          // per template instance; the smem size of a type never changes
+  static size_t smem_set = 0;
+  if (smem > smem_set) {
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) return -1;
+    smem_set = smem;
+    per_sm = 0;
+  }
+  if (per_sm == 0) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, p.threads, smem) != cudaSuccess || per_sm < 1)
+      return -1;
+  }
+  int64_t grid = int64_t(n_sm) * per_sm;
+  if (grid > cells) grid = cells;
+  kernel<<<unsigned(grid), p.threads, smem, s>>>(p);
+  return 1;
+}
+
+}  // namespace
+
+bool local_sched_supported(const TypeDev &td) {
+  const SchedDev &s = td.sched;
+  if (!s.valid) return false;
+  if (sched_smem_bytes(s, td.n_pad) > 227 * 1024) return false;
+  return (s.tpt == 2 && s.threads <= 640) || (s.tpt == 1 && s.threads <= 320);
+}
+
+int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t stream) {
+  if (bv.cells == 0) return 0;
+  if (!local_sched_supported(td)) return -1;
+  const SchedDev &s = td.sched;
+  SchedParams p;
+  p.n = td.n; p.T = td.T; p.n_pad = td.n_pad; p.ttri = s.ttri; p.threads = s.threads; p.vstride = s.vstride;
+  p.sx_bytes = s.n_vslots * 16; p.sN_bytes = s.n_tslots * 16; p.sC_bytes = s.n_cslots * 16;
+  p.tri_words = s.tri_words; p.tri_consts = s.tri_consts; p.vtx_words = s.vtx_words; p.vtx_coef = s.vtx_coef;
+  // 6V accumulates in fixed point (two 32-bit digits, base 2^24) with room for 64 x the rest volume
+  int k = 0;
+  std::frexp(384.0 * td.V0, &k);                    // 384 V0 < 2^k
+  p.fx_scale = std::ldexp(1.0, 52 - k);
+  p.fx_inv = std::ldexp(1.0, k - 52);
+  p.V0x6 = 6.0 * td.V0;
+  p.kv_coef = td.kv_over_V0 / 36.0;
+  p.x = static_cast<const float *>(bv.field[F_X]);
+  p.d = static_cast<const float *>(bv.field[F_D]);
+  p.b = static_cast<const float *>(bv.field[F_B]);
+  p.g = static_cast<float *>(bv.field[F_G]);
+  p.cells = bv.cells;
+  const size_t smem = sched_smem_bytes(s, td.n_pad);
+  if (s.tpt == 2) {
+    if (s.maxv == 6) return launch_variant<2, 6, 640, 1>(p, smem, n_sm, bv.cells, stream);
+    return launch_variant<2, 8, 640, 1>(p, smem, n_sm, bv.cells, stream);
+  }
+  if (s.maxv == 6) return launch_variant<1, 6, 320, 2>(p, smem, n_sm, bv.cells, stream);
+  return launch_variant<1, 8, 320, 2>(p, smem, n_sm, bv.cells, stream);
+}
+
+}  // namespace npfem
