@@ -52,6 +52,18 @@ __device__ __forceinline__ float rsqrt_fast(float x) {
   asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+// 16-bit halves of a packed offset word.  volatile: re-extracted at every use instead of being kept
+// unpacked in registers for the whole launch (the register budget is what limits this kernel)
+__device__ __forceinline__ uint32_t lo16(uint32_t w) {
+  uint32_t r;
+  asm volatile("and.b32 %0, %1, 0xffff;" : "=r"(r) : "r"(w));
+  return r;
+}
+__device__ __forceinline__ uint32_t hi16(uint32_t w) {
+  uint32_t r;
+  asm volatile("shr.u32 %0, %1, 16;" : "=r"(r) : "r"(w));
+  return r;
+}
 __device__ __forceinline__ float4 lds4(const unsigned char *base, uint32_t off) {
   return *reinterpret_cast<const float4 *>(base + off);
 }
@@ -136,7 +148,7 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
       } while (!done);
     }
     if (vact)
-      sts4(sx, vw[0] & 0xffffu, sg[tid] + sg[3 * n_pad + tid], sg[n_pad + tid] + sg[4 * n_pad + tid],
+      sts4(sx, lo16(vw[0]), sg[tid] + sg[3 * n_pad + tid], sg[n_pad + tid] + sg[4 * n_pad + tid],
            sg[2 * n_pad + tid] + sg[5 * n_pad + tid], 0.f);
     if (vact2)
       sts4(sx, p.vtx_words[v2] & 0xffffu, sg[v2] + sg[3 * n_pad + v2], sg[n_pad + v2] + sg[4 * n_pad + v2],
@@ -152,18 +164,18 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
     float vol = 0.f;
 #pragma unroll
     for (int j = 0; j < TPT; ++j) {
-      if (act[j]) {
-        const float4 X0 = lds4(sx, tw[j][0] & 0xffffu), X1 = lds4(sx, tw[j][0] >> 16), X2 = lds4(sx, tw[j][1] & 0xffffu);
+      {
+        const float4 X0 = lds4(sx, lo16(tw[j][0])), X1 = lds4(sx, hi16(tw[j][0])), X2 = lds4(sx, lo16(tw[j][1]));
         e1[j][0] = X1.x - X0.x; e1[j][1] = X1.y - X0.y; e1[j][2] = X1.z - X0.z;
         e2[j][0] = X2.x - X0.x; e2[j][1] = X2.y - X0.y; e2[j][2] = X2.z - X0.z;
         const float Nx = e1[j][1] * e2[j][2] - e1[j][2] * e2[j][1];
         const float Ny = e1[j][2] * e2[j][0] - e1[j][0] * e2[j][2];
         const float Nz = e1[j][0] * e2[j][1] - e1[j][1] * e2[j][0];
         nn[j] = Nx * Nx + Ny * Ny + Nz * Nz;
-        vol += X0.x * Nx + X0.y * Ny + X0.z * Nz;      // 6 x signed tetrahedron volume
+        vol += act[j] ? X0.x * Nx + X0.y * Ny + X0.z * Nz : 0.f;      // 6 x signed tetrahedron volume
         inv[j] = rsqrt_fast(nn[j]);
         nh[j][0] = Nx * inv[j]; nh[j][1] = Ny * inv[j]; nh[j][2] = Nz * inv[j];
-        sts4(sN, tw[j][4] >> 16, nh[j][0], nh[j][1], nh[j][2], inv[j]);
+        if (act[j]) sts4(sN, hi16(tw[j][4]), nh[j][0], nh[j][1], nh[j][2], inv[j]);
       }
     }
 #pragma unroll
@@ -177,75 +189,92 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
     const int2 vd = *reinterpret_cast<const int2 *>(vacc + 2 * (it & 1));
     const float vc = float(((double(vd.x) * 16777216.0 + double(vd.y)) * p.fx_inv - p.V0x6) * p.kv_coef);
     // ---- phase B ----------------------------------------------------------------------------
+    // all neighbour normals first (independent loads in flight together), then the hinge weights of
+    // every triangle, then membrane + corner forces + stores (stores last: they would fence the loads)
+    float4 NB[TPT][3];
 #pragma unroll
     for (int j = 0; j < TPT; ++j) {
-      if (act[j]) {
-        const float *a1 = e1[j], *a2 = e2[j], *nA = nh[j];
-        const float e11 = a1[0] * a1[0] + a1[1] * a1[1] + a1[2] * a1[2];
-        const float e12 = a1[0] * a2[0] + a1[1] * a2[1] + a1[2] * a2[2];
-        const float e22 = a2[0] * a2[0] + a2[1] * a2[1] + a2[2] * a2[2];
-        // membrane (Skalak, readings R5/R7): Q = 2 A0 (W1 R + W2 det^2 adj G)
-        const float R11 = tk[j][0], R12 = tk[j][1], R22 = tk[j][2], J = tk[j][3], tA = tk[j][4], tC = tk[j][5];
-        const float th = fmaf(R12, e12, -0.5f);
-        const float I1p1 = fmaf(R11, e11, fmaf(R22, e22, th + th));      // I1 + 1
-        const float I2 = fmaf(J, nn[j], -1.f);
-        const float W1 = tA * I1p1, W2 = fmaf(tC, I2, -tA * J);
-        const float q11 = fmaf(W2, e22, W1 * R11), q22 = fmaf(W2, e11, W1 * R22), q12 = fmaf(-W2, e12, W1 * R12);
-        // hinges seen from this triangle (reading R8): side s runs from corner s to s+1
-        float w0 = 0.f, w1 = 0.f, w2 = 0.f;
-        {
-          const float4 NB = lds4(sN, tw[j][1] >> 16);
-          const float crx = nA[1] * NB.z - nA[2] * NB.y, cry = nA[2] * NB.x - nA[0] * NB.z, crz = nA[0] * NB.y - nA[1] * NB.x;
-          const float S = crx * a1[0] + cry * a1[1] + crz * a1[2];
-          const float cs = nA[0] * NB.x + nA[1] * NB.y + nA[2] * NB.z;
-          const float L = e11, D = e11 - e12, ie = rsqrt_fast(L);
-          const float q = ie * fmaf(S * ie, tk[j][6], -cs * tk[j][9]);   // dE/dtheta / |e|
-          w0 = fmaf(D, q, w0); w1 = fmaf(L - D, q, w1); w2 = fmaf(-L, q, w2);
-        }
-        {
-          const float4 NB = lds4(sN, tw[j][2] & 0xffffu);
-          const float crx = nA[1] * NB.z - nA[2] * NB.y, cry = nA[2] * NB.x - nA[0] * NB.z, crz = nA[0] * NB.y - nA[1] * NB.x;
-          const float S = crx * (a2[0] - a1[0]) + cry * (a2[1] - a1[1]) + crz * (a2[2] - a1[2]);
-          const float cs = nA[0] * NB.x + nA[1] * NB.y + nA[2] * NB.z;
-          const float L = e11 - 2.f * e12 + e22, D = e22 - e12, ie = rsqrt_fast(L);
-          const float q = ie * fmaf(S * ie, tk[j][7], -cs * tk[j][10]);
-          w1 = fmaf(D, q, w1); w2 = fmaf(L - D, q, w2); w0 = fmaf(-L, q, w0);
-        }
-        {
-          const float4 NB = lds4(sN, tw[j][2] >> 16);
-          const float crx = nA[1] * NB.z - nA[2] * NB.y, cry = nA[2] * NB.x - nA[0] * NB.z, crz = nA[0] * NB.y - nA[1] * NB.x;
-          const float S = -(crx * a2[0] + cry * a2[1] + crz * a2[2]);
-          const float cs = nA[0] * NB.x + nA[1] * NB.y + nA[2] * NB.z;
-          const float L = e22, D = e12, ie = rsqrt_fast(L);
-          const float q = ie * fmaf(S * ie, tk[j][8], -cs * tk[j][11]);
-          w2 = fmaf(D, q, w2); w0 = fmaf(L - D, q, w0); w1 = fmaf(-L, q, w1);
-        }
-        // corner weights along the unit normal: volume term (reading R9) + hinge terms / |N|
-        const float vn = vc * (nn[j] * inv[j]);
-        const float u0 = fmaf(inv[j], w0, vn), u1 = fmaf(inv[j], w1, vn), u2 = fmaf(inv[j], w2, vn);
-        const float us = u0 + u1 + u2;
-        float c0[3], c1[3], c2[3];
+      NB[j][0] = lds4(sN, hi16(tw[j][1]));
+      NB[j][1] = lds4(sN, lo16(tw[j][2]));
+      NB[j][2] = lds4(sN, hi16(tw[j][2]));
+    }
+    float hw[TPT][3], e11[TPT], e12[TPT], e22[TPT];
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-          c1[k] = fmaf(u1, nA[k], fmaf(q11, a1[k], q12 * a2[k]));
-          c2[k] = fmaf(u2, nA[k], fmaf(q12, a1[k], q22 * a2[k]));
-          c0[k] = fmaf(us, nA[k], -c1[k]) - c2[k];
-        }
-        sts4(sC, tw[j][3] & 0xffffu, c0[0], c0[1], c0[2], 0.f);
-        sts4(sC, tw[j][3] >> 16, c1[0], c1[1], c1[2], 0.f);
-        sts4(sC, tw[j][4] & 0xffffu, c2[0], c2[1], c2[2], 0.f);
+    for (int j = 0; j < TPT; ++j) {
+      const float *a1 = e1[j], *a2 = e2[j], *nA = nh[j];
+      e11[j] = a1[0] * a1[0] + a1[1] * a1[1] + a1[2] * a1[2];
+      e12[j] = a1[0] * a2[0] + a1[1] * a2[1] + a1[2] * a2[2];
+      e22[j] = a2[0] * a2[0] + a2[1] * a2[1] + a2[2] * a2[2];
+      // hinges seen from this triangle (reading R8): side s runs from corner s to s+1
+      float w0 = 0.f, w1 = 0.f, w2 = 0.f;
+      {
+        const float4 B = NB[j][0];
+        const float crx = nA[1] * B.z - nA[2] * B.y, cry = nA[2] * B.x - nA[0] * B.z, crz = nA[0] * B.y - nA[1] * B.x;
+        const float S = crx * a1[0] + cry * a1[1] + crz * a1[2];
+        const float cs = nA[0] * B.x + nA[1] * B.y + nA[2] * B.z;
+        const float L = e11[j], D = e11[j] - e12[j], ie = rsqrt_fast(L);
+        const float q = ie * fmaf(S * ie, tk[j][6], -cs * tk[j][9]);   // dE/dtheta / |e|
+        w0 = fmaf(D, q, w0); w1 = fmaf(L - D, q, w1); w2 = fmaf(-L, q, w2);
+      }
+      {
+        const float4 B = NB[j][1];
+        const float crx = nA[1] * B.z - nA[2] * B.y, cry = nA[2] * B.x - nA[0] * B.z, crz = nA[0] * B.y - nA[1] * B.x;
+        const float S = crx * (a2[0] - a1[0]) + cry * (a2[1] - a1[1]) + crz * (a2[2] - a1[2]);
+        const float cs = nA[0] * B.x + nA[1] * B.y + nA[2] * B.z;
+        const float L = e11[j] - 2.f * e12[j] + e22[j], D = e22[j] - e12[j], ie = rsqrt_fast(L);
+        const float q = ie * fmaf(S * ie, tk[j][7], -cs * tk[j][10]);
+        w1 = fmaf(D, q, w1); w2 = fmaf(L - D, q, w2); w0 = fmaf(-L, q, w0);
+      }
+      {
+        const float4 B = NB[j][2];
+        const float crx = nA[1] * B.z - nA[2] * B.y, cry = nA[2] * B.x - nA[0] * B.z, crz = nA[0] * B.y - nA[1] * B.x;
+        const float S = -(crx * a2[0] + cry * a2[1] + crz * a2[2]);
+        const float cs = nA[0] * B.x + nA[1] * B.y + nA[2] * B.z;
+        const float L = e22[j], D = e12[j], ie = rsqrt_fast(L);
+        const float q = ie * fmaf(S * ie, tk[j][8], -cs * tk[j][11]);
+        w2 = fmaf(D, q, w2); w0 = fmaf(L - D, q, w0); w1 = fmaf(-L, q, w1);
+      }
+      hw[j][0] = w0; hw[j][1] = w1; hw[j][2] = w2;
+    }
+    float cf[TPT][9];
+#pragma unroll
+    for (int j = 0; j < TPT; ++j) {
+      const float *a1 = e1[j], *a2 = e2[j], *nA = nh[j];
+      // membrane (Skalak, readings R5/R7): Q = 2 A0 (W1 R + W2 det^2 adj G)
+      const float R11 = tk[j][0], R12 = tk[j][1], R22 = tk[j][2], J = tk[j][3], tA = tk[j][4], tC = tk[j][5];
+      const float th = fmaf(R12, e12[j], -0.5f);
+      const float I1p1 = fmaf(R11, e11[j], fmaf(R22, e22[j], th + th));      // I1 + 1
+      const float I2 = fmaf(J, nn[j], -1.f);
+      const float W1 = tA * I1p1, W2 = fmaf(tC, I2, -tA * J);
+      const float q11 = fmaf(W2, e22[j], W1 * R11), q22 = fmaf(W2, e11[j], W1 * R22), q12 = fmaf(-W2, e12[j], W1 * R12);
+      // corner weights along the unit normal: volume term (reading R9) + hinge terms / |N|
+      const float vn = vc * (nn[j] * inv[j]);
+      const float u0 = fmaf(inv[j], hw[j][0], vn), u1 = fmaf(inv[j], hw[j][1], vn), u2 = fmaf(inv[j], hw[j][2], vn);
+      const float us = u0 + u1 + u2;
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        cf[j][3 + k] = fmaf(u1, nA[k], fmaf(q11, a1[k], q12 * a2[k]));
+        cf[j][6 + k] = fmaf(u2, nA[k], fmaf(q12, a1[k], q22 * a2[k]));
+        cf[j][k] = fmaf(us, nA[k], -cf[j][3 + k]) - cf[j][6 + k];
       }
     }
+#pragma unroll
+    for (int j = 0; j < TPT; ++j)
+      if (act[j]) {
+        sts4(sC, lo16(tw[j][3]), cf[j][0], cf[j][1], cf[j][2], 0.f);
+        sts4(sC, hi16(tw[j][3]), cf[j][3], cf[j][4], cf[j][5], 0.f);
+        sts4(sC, lo16(tw[j][4]), cf[j][6], cf[j][7], cf[j][8], 0.f);
+      }
     __syncthreads();                                   // barrier 3: corner forces complete
     // ---- phase C ----------------------------------------------------------------------------
     if (vact) {
+      float4 f[MAXV];
+#pragma unroll
+      for (int q = 0; q < MAXV; ++q)
+        f[q] = lds4(sC, (q & 1) ? hi16(vw[1 + (q >> 1)]) : lo16(vw[1 + (q >> 1)]));
       float ax = 0.f, ay = 0.f, az = 0.f;
 #pragma unroll
-      for (int q = 0; q < MAXV; ++q) {
-        const uint32_t off = (q & 1) ? (vw[1 + (q >> 1)] >> 16) : (vw[1 + (q >> 1)] & 0xffffu);
-        const float4 f = lds4(sC, off);
-        ax += f.x; ay += f.y; az += f.z;
-      }
+      for (int q = 0; q < MAXV; ++q) { ax += f[q].x; ay += f[q].y; az += f[q].z; }
       float *gout = p.g + size_t(cell) * 3 * n_pad + tid;
       gout[0] = fmaf(coef, sg[3 * n_pad + tid], ax - sg[6 * n_pad + tid]);
       gout[n_pad] = fmaf(coef, sg[4 * n_pad + tid], ay - sg[7 * n_pad + tid]);
