@@ -80,7 +80,8 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
   unsigned char *sC = sN + p.sN_bytes;
   float *stage = reinterpret_cast<float *>(sC + p.sC_bytes);            // [NSTAGE][3 fields][3][n_pad]
   int *vacc = reinterpret_cast<int *>(stage + NSTAGE * 9 * n_pad);   // [2 cells][hi, lo] base-2^24 digits of 6V
-  uint64_t *mbar = reinterpret_cast<uint64_t *>(vacc + 4);
+  uint64_t *mbar = reinterpret_cast<uint64_t *>(vacc + 4);   // [NSTAGE] TMA ring
+  uint64_t *bars = mbar + NSTAGE;                              // [3] split block barriers B1, B2, B3
 
   const int tid = threadIdx.x, lane = tid & 31;
   const uint32_t field_bytes = uint32_t(3 * n_pad) * 4u;
@@ -120,6 +121,9 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < NSTAGE; ++s) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(mbar + s)));
+#pragma unroll
+    for (int s = 0; s < 3; ++s)
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bars + s)), "r"(nthreads >> 5));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     vacc[0] = vacc[1] = vacc[2] = vacc[3] = 0;
   }
@@ -133,32 +137,52 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
     }
   }
 
-  int it = 0;
-  for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x, ++it) {
-    const int st = it % NSTAGE;
+  // block-wide split barriers (arrive early, wait late) on mbarriers, one arrival per warp
+  auto bar_arrive = [&](int which) {
+    __syncwarp();
+    if (lane == 0)
+      asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bars + which)) : "memory");
+  };
+  auto bar_wait = [&](int which, uint32_t parity) {
+    uint32_t done;
+    do {
+      asm volatile(
+          "{\n.reg .pred q;\nmbarrier.try_wait.parity.shared::cta.b64 q, [%1], %2;\nselp.u32 %0, 1, 0, q;\n}\n"
+          : "=r"(done) : "r"(smem_u32(bars + which)), "r"(parity) : "memory");
+    } while (!done);
+  };
+  // phase 0 of the cell in ring slot `st`: sx[slot(v)] = (x_n + d, 0)
+  auto phase0 = [&](int it0) {
+    const int st = it0 % NSTAGE;
     const float *sg = stage + st * 9 * n_pad;
-    // ---- phase 0 ----------------------------------------------------------------------------
-    {
-      const uint32_t parity = uint32_t(it / NSTAGE) & 1u;
-      uint32_t done;
-      do {
-        asm volatile(
-            "{\n.reg .pred q;\nmbarrier.try_wait.parity.shared::cta.b64 q, [%1], %2;\nselp.u32 %0, 1, 0, q;\n}\n"
-            : "=r"(done) : "r"(smem_u32(mbar + st)), "r"(parity) : "memory");
-      } while (!done);
-    }
+    const uint32_t parity = uint32_t(it0 / NSTAGE) & 1u;
+    uint32_t done;
+    do {
+      asm volatile(
+          "{\n.reg .pred q;\nmbarrier.try_wait.parity.shared::cta.b64 q, [%1], %2;\nselp.u32 %0, 1, 0, q;\n}\n"
+          : "=r"(done) : "r"(smem_u32(mbar + st)), "r"(parity) : "memory");
+    } while (!done);
     if (vact)
       sts4(sx, lo16(vw[0]), sg[tid] + sg[3 * n_pad + tid], sg[n_pad + tid] + sg[4 * n_pad + tid],
            sg[2 * n_pad + tid] + sg[5 * n_pad + tid], 0.f);
     if (vact2)
       sts4(sx, p.vtx_words[v2] & 0xffffu, sg[v2] + sg[3 * n_pad + v2], sg[n_pad + v2] + sg[4 * n_pad + v2],
            sg[2 * n_pad + v2] + sg[5 * n_pad + v2], 0.f);
-    if (tid == 0) vacc[2 * ((it + 1) & 1)] = vacc[2 * ((it + 1) & 1) + 1] = 0;
-    __syncthreads();                                   // barrier 1: sx complete
-    if (tid == 0) {   // ring slot (it-1) % NSTAGE was last read in phase C of the previous cell
-      const int64_t nxt = cell + int64_t(NSTAGE - 1) * gridDim.x;
-      if (nxt < p.cells) prefetch(nxt, (it + NSTAGE - 1) % NSTAGE);
-    }
+  };
+
+  // Software pipeline over the cells of this CTA (B1/B2/B3 = split barriers, parity it & 1):
+  //   wait B1 | phase A | arrive B2 | wait B2 | phase B | arrive B3 | phase 0 of the NEXT cell |
+  //   arrive B1 | wait B3 | phase C
+  // so a warp that is early at a barrier runs ahead into work that does not depend on it.
+  if (int64_t(blockIdx.x) < p.cells) {
+    phase0(0);
+    bar_arrive(0);
+  }
+  int it = 0;
+  for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x, ++it) {
+    const uint32_t par = uint32_t(it) & 1u;
+    const float *sg = stage + (it % NSTAGE) * 9 * n_pad;
+    bar_wait(0, par);                                  // B1: sx of this cell complete
     // ---- phase A ----------------------------------------------------------------------------
     float e1[TPT][3], e2[TPT][3], nh[TPT][3], inv[TPT], nn[TPT];
     float vol = 0.f;
@@ -185,7 +209,33 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
       atomicAdd(vacc + 2 * (it & 1), int(v >> 24));
       atomicAdd(vacc + 2 * (it & 1) + 1, int(v & 0xffffff));
     }
-    __syncthreads();                                   // barrier 2: sN complete, volume accumulated
+    bar_arrive(1);
+    // membrane part of phase B needs this thread's registers only: it overlaps the wait for B2
+    // (Skalak, readings R5/R7): Q = 2 A0 (W1 R + W2 det^2 adj G)
+    float e11[TPT], e12[TPT], e22[TPT], q11[TPT], q12[TPT], q22[TPT];
+#pragma unroll
+    for (int j = 0; j < TPT; ++j) {
+      const float *a1 = e1[j], *a2 = e2[j];
+      e11[j] = a1[0] * a1[0] + a1[1] * a1[1] + a1[2] * a1[2];
+      e12[j] = a1[0] * a2[0] + a1[1] * a2[1] + a1[2] * a2[2];
+      e22[j] = a2[0] * a2[0] + a2[1] * a2[1] + a2[2] * a2[2];
+      const float R11 = tk[j][0], R12 = tk[j][1], R22 = tk[j][2], J = tk[j][3], tA = tk[j][4], tC = tk[j][5];
+      const float th = fmaf(R12, e12[j], -0.5f);
+      const float I1p1 = fmaf(R11, e11[j], fmaf(R22, e22[j], th + th));      // I1 + 1
+      const float I2 = fmaf(J, nn[j], -1.f);
+      const float W1 = tA * I1p1, W2 = fmaf(tC, I2, -tA * J);
+      q11[j] = fmaf(W2, e22[j], W1 * R11);
+      q22[j] = fmaf(W2, e11[j], W1 * R22);
+      q12[j] = fmaf(-W2, e12[j], W1 * R12);
+    }
+    bar_wait(1, par);                                  // B2: sN complete, volume accumulated
+    if (tid == 0) {
+      // every thread is past phase C of the previous cell: its ring slot and the other volume
+      // accumulator are free
+      vacc[2 * ((it + 1) & 1)] = vacc[2 * ((it + 1) & 1) + 1] = 0;
+      const int64_t nxt = cell + int64_t(NSTAGE - 1) * gridDim.x;
+      if (nxt < p.cells) prefetch(nxt, (it + NSTAGE - 1) % NSTAGE);
+    }
     const int2 vd = *reinterpret_cast<const int2 *>(vacc + 2 * (it & 1));
     const float vc = float(((double(vd.x) * 16777216.0 + double(vd.y)) * p.fx_inv - p.V0x6) * p.kv_coef);
     // ---- phase B ----------------------------------------------------------------------------
@@ -198,13 +248,10 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
       NB[j][1] = lds4(sN, lo16(tw[j][2]));
       NB[j][2] = lds4(sN, hi16(tw[j][2]));
     }
-    float hw[TPT][3], e11[TPT], e12[TPT], e22[TPT];
+    float hw[TPT][3];
 #pragma unroll
     for (int j = 0; j < TPT; ++j) {
       const float *a1 = e1[j], *a2 = e2[j], *nA = nh[j];
-      e11[j] = a1[0] * a1[0] + a1[1] * a1[1] + a1[2] * a1[2];
-      e12[j] = a1[0] * a2[0] + a1[1] * a2[1] + a1[2] * a2[2];
-      e22[j] = a2[0] * a2[0] + a2[1] * a2[1] + a2[2] * a2[2];
       // hinges seen from this triangle (reading R8): side s runs from corner s to s+1
       float w0 = 0.f, w1 = 0.f, w2 = 0.f;
       {
@@ -240,21 +287,14 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
 #pragma unroll
     for (int j = 0; j < TPT; ++j) {
       const float *a1 = e1[j], *a2 = e2[j], *nA = nh[j];
-      // membrane (Skalak, readings R5/R7): Q = 2 A0 (W1 R + W2 det^2 adj G)
-      const float R11 = tk[j][0], R12 = tk[j][1], R22 = tk[j][2], J = tk[j][3], tA = tk[j][4], tC = tk[j][5];
-      const float th = fmaf(R12, e12[j], -0.5f);
-      const float I1p1 = fmaf(R11, e11[j], fmaf(R22, e22[j], th + th));      // I1 + 1
-      const float I2 = fmaf(J, nn[j], -1.f);
-      const float W1 = tA * I1p1, W2 = fmaf(tC, I2, -tA * J);
-      const float q11 = fmaf(W2, e22[j], W1 * R11), q22 = fmaf(W2, e11[j], W1 * R22), q12 = fmaf(-W2, e12[j], W1 * R12);
       // corner weights along the unit normal: volume term (reading R9) + hinge terms / |N|
       const float vn = vc * (nn[j] * inv[j]);
       const float u0 = fmaf(inv[j], hw[j][0], vn), u1 = fmaf(inv[j], hw[j][1], vn), u2 = fmaf(inv[j], hw[j][2], vn);
       const float us = u0 + u1 + u2;
 #pragma unroll
       for (int k = 0; k < 3; ++k) {
-        cf[j][3 + k] = fmaf(u1, nA[k], fmaf(q11, a1[k], q12 * a2[k]));
-        cf[j][6 + k] = fmaf(u2, nA[k], fmaf(q12, a1[k], q22 * a2[k]));
+        cf[j][3 + k] = fmaf(u1, nA[k], fmaf(q11[j], a1[k], q12[j] * a2[k]));
+        cf[j][6 + k] = fmaf(u2, nA[k], fmaf(q12[j], a1[k], q22[j] * a2[k]));
         cf[j][k] = fmaf(us, nA[k], -cf[j][3 + k]) - cf[j][6 + k];
       }
     }
@@ -265,7 +305,12 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
         sts4(sC, hi16(tw[j][3]), cf[j][3], cf[j][4], cf[j][5], 0.f);
         sts4(sC, lo16(tw[j][4]), cf[j][6], cf[j][7], cf[j][8], 0.f);
       }
-    __syncthreads();                                   // barrier 3: corner forces complete
+    bar_arrive(2);
+    if (cell + gridDim.x < p.cells) {                  // sx was last read in phase A (before B2)
+      phase0(it + 1);
+      bar_arrive(0);
+    }
+    bar_wait(2, par);                                  // B3: corner forces complete
     // ---- phase C ----------------------------------------------------------------------------
     if (vact) {
       float4 f[MAXV];
@@ -293,8 +338,7 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
       gout[n_pad] = fmaf(coef2, sg[4 * n_pad + v2], ay - sg[7 * n_pad + v2]);
       gout[2 * n_pad] = fmaf(coef2, sg[5 * n_pad + v2], az - sg[8 * n_pad + v2]);
     }
-    // no barrier: the next phase 0 writes sx (last read in phase A) and reads another ring slot;
-    // sN / sC are rewritten only after barriers 1 / 2 of the next cell
+    // sN / sC are rewritten only after B1 / B2 of the next cell, which every warp reaches after this
   }
 }
 
@@ -303,7 +347,7 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
 namespace {
 
 size_t sched_smem_bytes(const SchedDev &s, int n_pad) {
-  return size_t(s.n_vslots + s.n_tslots + s.n_cslots) * 16 + size_t(NSTAGE) * 9 * n_pad * 4 + 4 * 4 + NSTAGE * 8;
+  return size_t(s.n_vslots + s.n_tslots + s.n_cslots) * 16 + size_t(NSTAGE) * 9 * n_pad * 4 + 4 * 4 + (NSTAGE + 3) * 8;
 }
 
 template <int TPT, int MAXV, int MAXT, int MINB>
