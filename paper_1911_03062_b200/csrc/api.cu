@@ -654,6 +654,14 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
     if ((rc = timed_launch(c, NPFEM_KIND_PROLOGUE, int(t), "prologue", [&] {
            return launch_prologue(c->types[t], c->views[t], c->precision, c->stream); })))
       return rc;
+  // Fused-update mode (fp32, scheduled local step + tensor-core global step, no diagnostics): the
+  // global step only writes its product u = -H~^-1 r; the NEXT local step (or the epilogue) applies
+  // d <- (1 - gamma) d + u while it streams d anyway, so the GEMM epilogue has no loads to wait for.
+  std::vector<char> fused(nb, 0);
+  for (size_t t = 0; t < nb; ++t)
+    fused[t] = c->precision == NPFEM_F32 && !c->diagnostics && c->opt_global_math == 0 &&
+               (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]) &&
+               global_tcgen05_supported(c->types[t]);
   for (int k = 0; k < n_iterations; ++k) {
     if (c->diagnostics && (rc = diag(k))) return rc;
     for (size_t t = 0; t < nb; ++t) {
@@ -662,15 +670,16 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
       const bool fast = f32 && !sched && c->opt_local_impl != 1 && local_smem_supported(c->types[t]);
       const double d_scale = (sched || fast) ? 1.0 - c->types[t].gamma : 1.0;
       if ((rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "local step", [&] {
-             if (sched) return launch_local_sched(c->types[t], c->views[t], c->n_sm, c->stream);
+             if (sched) return launch_local_sched(c->types[t], c->views[t], c->n_sm, fused[t] && k > 0, d_scale, c->stream);
              if (fast) return launch_local_smem(c->types[t], c->views[t], c->n_sm, c->stream);
              return launch_local_generic(c->types[t], c->views[t], c->buckets[t].scratch, c->precision, c->n_sm,
                                          c->stream); })))
         return rc;
       if ((rc = timed_launch(c, NPFEM_KIND_GLOBAL, int(t), "global step", [&] {
              if (c->precision == NPFEM_F32 && c->opt_global_math == 0) {
-               const int n = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, d_scale, c->stream);
-               if (n >= 0) return n;
+               const int n = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, d_scale,
+                                                   fused[t] ? c->views[t].field[F_U] : nullptr, c->stream);
+               if (n >= 0 || fused[t]) return n;
              }
              return launch_global_simt(c->types[t], c->views[t], c->precision, d_scale, c->stream); })))
         return rc;
@@ -679,7 +688,8 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   if (c->diagnostics && (rc = diag(n_iterations))) return rc;
   for (size_t t = 0; t < nb; ++t)
     if ((rc = timed_launch(c, NPFEM_KIND_EPILOGUE, int(t), "epilogue", [&] {
-           return launch_epilogue(c->types[t], c->views[t], c->precision, c->stream); })))
+           return launch_epilogue(c->types[t], c->views[t], c->precision, fused[t] != 0, 1.0 - c->types[t].gamma,
+                                  c->stream); })))
       return rc;
   return NPFEM_OK;
 }

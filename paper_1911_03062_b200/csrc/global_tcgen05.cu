@@ -25,8 +25,8 @@ namespace {
 constexpr int BM = 128;          // rows per tile (TMEM lanes)
 constexpr int BK = 32;           // fp32 per K chunk = 128 bytes = one swizzle row
 constexpr int UMMA_K = 8;        // K per tcgen05.mma for tf32 (32 bytes)
-constexpr int STAGES = 3;
-constexpr int MAX_NPASS = 336;   // accumulator columns per pass (<= 512, multiple of 16)
+constexpr int STAGES = 4;
+constexpr int MAX_NPASS = 256;   // accumulator columns per pass: two accumulators fit the 512 TMEM columns
 constexpr int A_BYTES = BM * BK * 4;
 constexpr int B_BYTES = MAX_NPASS * BK * 4;
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
@@ -93,22 +93,30 @@ __device__ __forceinline__ void umma_commit(uint64_t *bar) {
 }
 
 struct GemmParams {
-  float *D;            // [rows][n_pad], updated in place
+  float *D;            // [rows][n_pad], updated in place (U == nullptr)
+  float *U;            // [rows][n_pad] or nullptr: write the raw product -G W here instead of updating D
   int64_t rows;
   int n_pad;
-  int n_pass;          // accumulator columns per pass (multiple of 16, <= MAX_NPASS)
+  int n_pass;          // accumulator columns per pass = N of the MMA (multiple of 16, <= MAX_NPASS)
   int passes;          // ceil(n_pad / n_pass)
-  int n1, n2;          // columns of the two MMA instructions of a pass (n1 <= 256, n2 may be 0)
   int k_chunks;        // ceil(n_pad / BK)
   int64_t m_tiles;
   float d_scale;       // d <- d_scale * d + acc
 };
 
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+        "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr));
+}
+
 __global__ void __launch_bounds__(192, 1)
-global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_constant__ CUtensorMap map_w1,
-                      const __grid_constant__ CUtensorMap map_w2, const GemmParams p) {
+global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_constant__ CUtensorMap map_w,
+                      const GemmParams p) {
   extern __shared__ unsigned char smem_raw[];
-  __shared__ uint64_t full_bar[STAGES], empty_bar[STAGES], tmem_full_bar, tmem_empty_bar;
+  __shared__ uint64_t full_bar[STAGES], empty_bar[STAGES], tmem_full_bar[2], tmem_empty_bar[2];
   __shared__ uint32_t tmem_base_sh;
   unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -119,11 +127,13 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
       mbar_init(&full_bar[s], 1);
       mbar_init(&empty_bar[s], 1);
     }
-    mbar_init(&tmem_full_bar, 1);
-    mbar_init(&tmem_empty_bar, 128);
+    for (int a = 0; a < 2; ++a) {
+      mbar_init(&tmem_full_bar[a], 1);
+      mbar_init(&tmem_empty_bar[a], 128);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 1) {   // TMEM: 512 columns (the whole SM's, one CTA per SM)
+  if (warp == 1) {   // TMEM: all 512 columns (one CTA per SM) = two accumulators of <= 256 columns
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&tmem_base_sh)));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
@@ -137,7 +147,7 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
-      const uint32_t tx = A_BYTES + uint32_t(p.n1 + p.n2) * BK * 4;
+      const uint32_t tx = A_BYTES + uint32_t(p.n_pass) * BK * 4;
       for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
         const int row0 = int((item / p.passes) * BM), col0 = int(item % p.passes) * p.n_pass;
         for (int kc = 0; kc < p.k_chunks; ++kc) {
@@ -145,8 +155,7 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
           unsigned char *sa = smem + stage * STAGE_BYTES, *sb = sa + A_BYTES;
           mbar_expect_tx(&full_bar[stage], tx);
           tma_load_2d(sa, &map_g, kc * BK, row0, &full_bar[stage]);
-          tma_load_2d(sb, &map_w1, kc * BK, col0, &full_bar[stage]);
-          if (p.n2) tma_load_2d(sb + p.n1 * BK * 4, &map_w2, kc * BK, col0 + p.n1, &full_bar[stage]);
+          tma_load_2d(sb, &map_w, kc * BK, col0, &full_bar[stage]);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
@@ -155,65 +164,85 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
     // ===== MMA issuer =====
     if (lane == 0) {
       int stage = 0;
-      uint32_t phase = 0, acc_phase = 0;
-      const uint32_t idesc1 = make_idesc(BM, p.n1), idesc2 = make_idesc(BM, p.n2 ? p.n2 : 16);
-      for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
-        mbar_wait(&tmem_empty_bar, acc_phase ^ 1);          // epilogue has drained the accumulator
+      uint32_t phase = 0, li = 0;
+      const uint32_t idesc = make_idesc(BM, p.n_pass);
+      for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x, ++li) {
+        const uint32_t acc = li & 1u, acc_phase = (li >> 1) & 1u;
+        mbar_wait(&tmem_empty_bar[acc], acc_phase ^ 1);     // epilogue has drained this accumulator
         asm volatile("tcgen05.fence::after_thread_sync;");
+        const uint32_t tacc = tmem_base + acc * MAX_NPASS;
         for (int kc = 0; kc < p.k_chunks; ++kc) {
           mbar_wait(&full_bar[stage], phase);
           asm volatile("tcgen05.fence::after_thread_sync;");
           const uint32_t sa = smem_u32(smem + stage * STAGE_BYTES), sb = sa + A_BYTES;
 #pragma unroll
-          for (int k = 0; k < BK / UMMA_K; ++k) {
-            const uint64_t a_desc = make_smem_desc(sa + k * UMMA_K * 4);
-            umma_tf32(tmem_base, a_desc, make_smem_desc(sb + k * UMMA_K * 4), idesc1, (kc | k) != 0);
-            if (p.n2)
-              umma_tf32(tmem_base + p.n1, a_desc, make_smem_desc(sb + p.n1 * BK * 4 + k * UMMA_K * 4), idesc2,
-                        (kc | k) != 0);
-          }
+          for (int k = 0; k < BK / UMMA_K; ++k)
+            umma_tf32(tacc, make_smem_desc(sa + k * UMMA_K * 4), make_smem_desc(sb + k * UMMA_K * 4), idesc,
+                      (kc | k) != 0);
           umma_commit(&empty_bar[stage]);                   // frees the smem slot when the MMAs retire
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
-        umma_commit(&tmem_full_bar);                        // accumulator complete
-        acc_phase ^= 1;
+        umma_commit(&tmem_full_bar[acc]);                   // accumulator complete
       }
     }
   } else {
-    // ===== epilogue: warps 2..5 own TMEM lanes 32*(warp%4) .. +31 =====
+    // ===== epilogue: warps 2..5 own TMEM lanes 32*(warp%4) .. +31; overlaps the next item's MMAs =====
     const int lane_base = (warp & 3) * 32;
-    uint32_t acc_phase = 0;
-    for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+    uint32_t li = 0;
+    for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x, ++li) {
+      const uint32_t acc = li & 1u, acc_phase = (li >> 1) & 1u;
       const int64_t row = (item / p.passes) * BM + lane_base + lane;
       const int col0 = int(item % p.passes) * p.n_pass;
-      mbar_wait(&tmem_full_bar, acc_phase);
+      mbar_wait(&tmem_full_bar[acc], acc_phase);
       asm volatile("tcgen05.fence::after_thread_sync;");
-      float *drow = p.D + row * p.n_pad;
-      for (int c = 0; c < p.n_pass; c += 16) {
-        uint32_t r[16];
-        const uint32_t taddr = tmem_base + (uint32_t(lane_base) << 16) + uint32_t(c);
-        asm volatile(
-            "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-            : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-              "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-            : "r"(taddr));
-        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        if (row < p.rows && col0 + c < p.n_pad) {
+      const uint32_t tacc = tmem_base + acc * MAX_NPASS + (uint32_t(lane_base) << 16);
+      const bool row_ok = row < p.rows;
+      if (p.U) {
+        // raw product out: no loads, stores only (the consumer applies d <- d_scale d + u)
+        float *urow = p.U + row * p.n_pad + col0;
+        for (int c = 0; c < p.n_pass; c += 32) {
+          uint32_t r0[16], r1[16];
+          tmem_ld16(tacc + uint32_t(c), r0);
+          tmem_ld16(tacc + uint32_t(c) + 16u, r1);          // n_pass is a multiple of 16: may read an unused column block
+          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+          if (row_ok && col0 + c < p.n_pad) {
 #pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            float4 *ptr = reinterpret_cast<float4 *>(drow + col0 + c + 4 * q);
-            float4 v = *ptr;
-            v.x = p.d_scale * v.x + __uint_as_float(r[4 * q]);
-            v.y = p.d_scale * v.y + __uint_as_float(r[4 * q + 1]);
-            v.z = p.d_scale * v.z + __uint_as_float(r[4 * q + 2]);
-            v.w = p.d_scale * v.w + __uint_as_float(r[4 * q + 3]);
-            *ptr = v;
+            for (int q = 0; q < 4; ++q)
+              *reinterpret_cast<float4 *>(urow + c + 4 * q) =
+                  make_float4(__uint_as_float(r0[4 * q]), __uint_as_float(r0[4 * q + 1]), __uint_as_float(r0[4 * q + 2]),
+                              __uint_as_float(r0[4 * q + 3]));
+          }
+          if (row_ok && c + 16 < p.n_pass && col0 + c + 16 < p.n_pad) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+              *reinterpret_cast<float4 *>(urow + c + 16 + 4 * q) =
+                  make_float4(__uint_as_float(r1[4 * q]), __uint_as_float(r1[4 * q + 1]), __uint_as_float(r1[4 * q + 2]),
+                              __uint_as_float(r1[4 * q + 3]));
+          }
+        }
+      } else {
+        float *drow = p.D + row * p.n_pad + col0;
+        for (int c = 0; c < p.n_pass; c += 16) {
+          uint32_t r[16];
+          tmem_ld16(tacc + uint32_t(c), r);
+          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+          if (row_ok && col0 + c < p.n_pad) {
+            float4 v[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) v[q] = *reinterpret_cast<const float4 *>(drow + c + 4 * q);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              v[q].x = p.d_scale * v[q].x + __uint_as_float(r[4 * q]);
+              v[q].y = p.d_scale * v[q].y + __uint_as_float(r[4 * q + 1]);
+              v[q].z = p.d_scale * v[q].z + __uint_as_float(r[4 * q + 2]);
+              v[q].w = p.d_scale * v[q].w + __uint_as_float(r[4 * q + 3]);
+              *reinterpret_cast<float4 *>(drow + c + 4 * q) = v[q];
+            }
           }
         }
       }
       asm volatile("tcgen05.fence::before_thread_sync;");
-      mbar_arrive(&tmem_empty_bar);
-      acc_phase ^= 1;
+      mbar_arrive(&tmem_empty_bar[acc]);
     }
   }
   __syncthreads();
@@ -254,27 +283,36 @@ bool make_map(CUtensorMap *map, const void *base, uint64_t rows, uint64_t cols, 
 
 }  // namespace
 
-// returns #launches, or -1 if the configuration is unsupported (caller falls back to the SIMT GEMM)
-int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, double d_scale, cudaStream_t s) {
-  if (bv.cells == 0) return 0;
-  GemmParams p{};
-  p.D = static_cast<float *>(bv.field[F_D]);
-  p.rows = bv.cells * 3;
+// shape of the tensor-core path for a type: false when unsupported (caller uses the SIMT GEMM)
+static bool gemm_shape(const TypeDev &td, GemmParams &p) {
   p.n_pad = td.n_pad;
   p.passes = (td.n_pad + MAX_NPASS - 1) / MAX_NPASS;
   p.n_pass = ((td.n_pad + p.passes - 1) / p.passes + 15) / 16 * 16;
-  if (p.n_pass > MAX_NPASS) return -1;
-  p.n1 = p.n_pass > 256 ? 256 : p.n_pass;
-  p.n2 = p.n_pass - p.n1;
+  if (p.n_pass > MAX_NPASS || p.n_pass < 16 || td.Hinv == nullptr) return false;
   p.k_chunks = (td.n_pad + BK - 1) / BK;
+  return true;
+}
+
+bool global_tcgen05_supported(const TypeDev &td) {
+  GemmParams p{};
+  return gemm_shape(td, p) && get_encode() != nullptr;
+}
+
+// d <- d_scale d - g Hinv (u_out == nullptr) or u_out <- -g Hinv.  Returns #launches, or -1 if the
+// configuration is unsupported (caller falls back to the SIMT GEMM).
+int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, double d_scale, void *u_out,
+                          cudaStream_t s) {
+  if (bv.cells == 0) return 0;
+  GemmParams p{};
+  if (!gemm_shape(td, p)) return -1;
+  p.D = static_cast<float *>(bv.field[F_D]);
+  p.U = static_cast<float *>(u_out);
+  p.rows = bv.cells * 3;
   p.m_tiles = (p.rows + BM - 1) / BM;
   p.d_scale = float(d_scale);
-  CUtensorMap map_g, map_w1, map_w2;
+  CUtensorMap map_g, map_w;
   if (!make_map(&map_g, bv.field[F_G], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), BM)) return -1;
-  if (!make_map(&map_w1, td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n1))) return -1;
-  if (!make_map(&map_w2, td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad),
-                uint32_t(p.n2 ? p.n2 : 16)))
-    return -1;
+  if (!make_map(&map_w, td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n_pass))) return -1;
   static bool attr = false;
   if (!attr) {
     if (cudaFuncSetAttribute(global_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES) != cudaSuccess)
@@ -283,9 +321,9 @@ int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, dou
   }
   const int64_t items = p.m_tiles * p.passes;
   // the passes of one M tile are adjacent items: they run on neighbouring CTAs at about the same
-  // time, so the second read of the G tile is an L2 hit
+  // time, so the repeated reads of the G tile are L2 hits
   const unsigned grid = unsigned(items < n_sm ? items : n_sm);
-  global_tcgen05_kernel<<<grid, 192, SMEM_BYTES, s>>>(map_g, map_w1, map_w2, p);
+  global_tcgen05_kernel<<<grid, 192, SMEM_BYTES, s>>>(map_g, map_w, p);
   return 1;
 }
 

@@ -13,7 +13,7 @@
 namespace npfem {
 
 // Number of state fields kept per bucket, each [cells][3][n_pad] of the compute type.
-enum Field { F_X = 0, F_V, F_F, F_B, F_D, F_G, F_COUNT };
+enum Field { F_X = 0, F_V, F_F, F_B, F_D, F_G, F_U, F_COUNT };   // F_U: raw product of the last global step
 
 // Device tables of the scheduled fp32 local step (local_schedule.hpp / local_sched.cu).
 struct SchedDev {
@@ -97,7 +97,9 @@ int launch_set_forces(const BucketView *views_dev, const PackArgs &a, int precis
 int launch_get_state(const BucketView *views_dev, const PackArgs &a, int precision, cudaStream_t s);
 
 int launch_prologue(const TypeDev &td, const BucketView &bv, int precision, cudaStream_t s);
-int launch_epilogue(const TypeDev &td, const BucketView &bv, int precision, cudaStream_t s);
+// pending: d <- d_scale d + u still has to be applied (fused-update mode, see npfem_step)
+int launch_epilogue(const TypeDev &td, const BucketView &bv, int precision, bool pending, double d_scale,
+                    cudaStream_t s);
 
 // local step: g = M~ d/h^2 - b + grad E(x_n + d)
 size_t local_generic_scratch_bytes(const TypeDev &td, int precision, int n_sm);
@@ -109,7 +111,10 @@ int launch_objective(const TypeDev &td, const BucketView &bv, const int64_t *cel
 // global step: d <- d - g Hinv   ([3 cells x n_pad] . [n_pad x n_pad])
 int launch_global_simt(const TypeDev &td, const BucketView &bv, int precision, double d_scale, cudaStream_t s);
 // fp32 contexts, TF32 tensor cores (tcgen05); returns -1 when the shape is unsupported
-int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, double d_scale, cudaStream_t s);
+bool global_tcgen05_supported(const TypeDev &td);
+// u_out == nullptr: d <- d_scale d - g Hinv;  else u_out <- -g Hinv (the next local step / the epilogue applies it)
+int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, double d_scale, void *u_out,
+                          cudaStream_t s);
 
 // fp32 fast local step; writes the reduced gradient (global step must then use d_scale = 1 - gamma)
 bool local_smem_supported(const TypeDev &td);
@@ -118,7 +123,9 @@ int launch_local_smem(const TypeDev &td, const BucketView &bv, int n_sm, cudaStr
 // fp32 scheduled local step (register-resident topology, conflict-free shared-memory slots); same
 // reduced-gradient convention as launch_local_smem
 bool local_sched_supported(const TypeDev &td);
-int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
+// apply_u: first d <- d_scale d + u (pending update of the previous global step), stored back to d
+int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, bool apply_u, double d_scale,
+                       cudaStream_t s);
 
 int launch_monotone_flags(const double *history, int n_entries, int64_t cells, int32_t *flags, cudaStream_t s);
 

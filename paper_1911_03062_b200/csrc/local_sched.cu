@@ -41,8 +41,11 @@ struct SchedParams {
   const float *vtx_coef;       // [vstride]
   double fx_scale, fx_inv;     // fixed-point scale of the 6 V accumulator and its inverse
   double V0x6, kv_coef;        // 6 V0;  k_v / (36 V0):  vc = kv_coef (6V - 6V0) = k_v (V - V0)/V0 / 6
-  const float *x, *d, *b;      // [cells][3][n_pad]
+  const float *x, *b, *u;      // [cells][3][n_pad]
+  float *d;                    // read; written back when apply_u
   float *g;
+  int apply_u;                 // first d <- d_scale d + u (pending update of the last global step)
+  float d_scale;
   int64_t cells;
 };
 
@@ -78,8 +81,8 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
   unsigned char *sx = smem;
   unsigned char *sN = sx + p.sx_bytes;
   unsigned char *sC = sN + p.sN_bytes;
-  float *stage = reinterpret_cast<float *>(sC + p.sC_bytes);            // [NSTAGE][3 fields][3][n_pad]
-  int *vacc = reinterpret_cast<int *>(stage + NSTAGE * 9 * n_pad);   // [2 cells][hi, lo] base-2^24 digits of 6V
+  float *stage = reinterpret_cast<float *>(sC + p.sC_bytes);            // [NSTAGE][4 fields x, d, b, u][3][n_pad]
+  int *vacc = reinterpret_cast<int *>(stage + NSTAGE * 12 * n_pad);   // [2 cells][hi, lo] base-2^24 digits of 6V
   uint64_t *mbar = reinterpret_cast<uint64_t *>(vacc + 4);   // [NSTAGE] TMA ring
   uint64_t *bars = mbar + NSTAGE;                              // [3] split block barriers B1, B2, B3
 
@@ -109,13 +112,14 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
   auto prefetch = [&](int64_t cell, int st) {   // one thread: arm the barrier, start 3 bulk copies
     const size_t base = size_t(cell) * 3 * n_pad;
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar + st)),
-                 "r"(3 * field_bytes) : "memory");
-    const float *src[3] = {p.x + base, p.d + base, p.b + base};
+                 "r"((p.apply_u ? 4u : 3u) * field_bytes) : "memory");
+    const float *src[4] = {p.x + base, p.d + base, p.b + base, p.u + base};
 #pragma unroll
-    for (int f = 0; f < 3; ++f)
-      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                   ::"r"(smem_u32(stage + (st * 9 + f * 3) * n_pad)), "l"(src[f]), "r"(field_bytes),
-                     "r"(smem_u32(mbar + st)) : "memory");
+    for (int f = 0; f < 4; ++f)
+      if (f < 3 || p.apply_u)
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(smem_u32(stage + (st * 12 + f * 3) * n_pad)), "l"(src[f]), "r"(field_bytes),
+                       "r"(smem_u32(mbar + st)) : "memory");
   };
 
   if (tid == 0) {
@@ -151,10 +155,26 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
           : "=r"(done) : "r"(smem_u32(bars + which)), "r"(parity) : "memory");
     } while (!done);
   };
-  // phase 0 of the cell in ring slot `st`: sx[slot(v)] = (x_n + d, 0)
-  auto phase0 = [&](int it0) {
+  // phase 0 of this CTA's it0-th cell (ring slot it0 % NSTAGE): apply the pending update
+  // d <- d_scale d + u (kept in the ring slot for phase C, written back to global d), then
+  // sx[slot(v)] = (x_n + d, 0)
+  auto phase0_vertex = [&](float *sg, float *dglob, int v, uint32_t slot_off) {
+    float dv[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) dv[k] = sg[(3 + k) * n_pad + v];
+    if (p.apply_u) {
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        dv[k] = fmaf(p.d_scale, dv[k], sg[(9 + k) * n_pad + v]);
+        sg[(3 + k) * n_pad + v] = dv[k];
+        dglob[k * n_pad + v] = dv[k];
+      }
+    }
+    sts4(sx, slot_off, sg[v] + dv[0], sg[n_pad + v] + dv[1], sg[2 * n_pad + v] + dv[2], 0.f);
+  };
+  auto phase0 = [&](int it0, int64_t cell0) {
     const int st = it0 % NSTAGE;
-    const float *sg = stage + st * 9 * n_pad;
+    float *sg = stage + st * 12 * n_pad;
     const uint32_t parity = uint32_t(it0 / NSTAGE) & 1u;
     uint32_t done;
     do {
@@ -162,12 +182,9 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
           "{\n.reg .pred q;\nmbarrier.try_wait.parity.shared::cta.b64 q, [%1], %2;\nselp.u32 %0, 1, 0, q;\n}\n"
           : "=r"(done) : "r"(smem_u32(mbar + st)), "r"(parity) : "memory");
     } while (!done);
-    if (vact)
-      sts4(sx, lo16(vw[0]), sg[tid] + sg[3 * n_pad + tid], sg[n_pad + tid] + sg[4 * n_pad + tid],
-           sg[2 * n_pad + tid] + sg[5 * n_pad + tid], 0.f);
-    if (vact2)
-      sts4(sx, p.vtx_words[v2] & 0xffffu, sg[v2] + sg[3 * n_pad + v2], sg[n_pad + v2] + sg[4 * n_pad + v2],
-           sg[2 * n_pad + v2] + sg[5 * n_pad + v2], 0.f);
+    float *dglob = p.d + size_t(cell0) * 3 * n_pad;
+    if (vact) phase0_vertex(sg, dglob, tid, lo16(vw[0]));
+    if (vact2) phase0_vertex(sg, dglob, v2, p.vtx_words[v2] & 0xffffu);
   };
 
   // Software pipeline over the cells of this CTA (B1/B2/B3 = split barriers, parity it & 1):
@@ -175,13 +192,13 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
   //   arrive B1 | wait B3 | phase C
   // so a warp that is early at a barrier runs ahead into work that does not depend on it.
   if (int64_t(blockIdx.x) < p.cells) {
-    phase0(0);
+    phase0(0, blockIdx.x);
     bar_arrive(0);
   }
   int it = 0;
   for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x, ++it) {
     const uint32_t par = uint32_t(it) & 1u;
-    const float *sg = stage + (it % NSTAGE) * 9 * n_pad;
+    const float *sg = stage + (it % NSTAGE) * 12 * n_pad;
     bar_wait(0, par);                                  // B1: sx of this cell complete
     // ---- phase A ----------------------------------------------------------------------------
     float e1[TPT][3], e2[TPT][3], nh[TPT][3], inv[TPT], nn[TPT];
@@ -307,7 +324,7 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
       }
     bar_arrive(2);
     if (cell + gridDim.x < p.cells) {                  // sx was last read in phase A (before B2)
-      phase0(it + 1);
+      phase0(it + 1, cell + gridDim.x);
       bar_arrive(0);
     }
     bar_wait(2, par);                                  // B3: corner forces complete
@@ -347,7 +364,7 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
 namespace {
 
 size_t sched_smem_bytes(const SchedDev &s, int n_pad) {
-  return size_t(s.n_vslots + s.n_tslots + s.n_cslots) * 16 + size_t(NSTAGE) * 9 * n_pad * 4 + 4 * 4 + (NSTAGE + 3) * 8;
+  return size_t(s.n_vslots + s.n_tslots + s.n_cslots) * 16 + size_t(NSTAGE) * 12 * n_pad * 4 + 4 * 4 + (NSTAGE + 3) * 8;
 }
 
 template <int TPT, int MAXV, int MAXT, int MINB>
@@ -379,7 +396,8 @@ bool local_sched_supported(const TypeDev &td) {
   return (s.tpt == 2 && s.threads <= 640) || (s.tpt == 1 && s.threads <= 320);
 }
 
-int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t stream) {
+int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, bool apply_u, double d_scale,
+                       cudaStream_t stream) {
   if (bv.cells == 0) return 0;
   if (!local_sched_supported(td)) return -1;
   const SchedDev &s = td.sched;
@@ -395,7 +413,10 @@ int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, cudaSt
   p.V0x6 = 6.0 * td.V0;
   p.kv_coef = td.kv_over_V0 / 36.0;
   p.x = static_cast<const float *>(bv.field[F_X]);
-  p.d = static_cast<const float *>(bv.field[F_D]);
+  p.d = static_cast<float *>(bv.field[F_D]);
+  p.u = static_cast<const float *>(bv.field[F_U]);
+  p.apply_u = apply_u ? 1 : 0;
+  p.d_scale = float(d_scale);
   p.b = static_cast<const float *>(bv.field[F_B]);
   p.g = static_cast<float *>(bv.field[F_G]);
   p.cells = bv.cells;

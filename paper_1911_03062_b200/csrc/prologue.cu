@@ -118,13 +118,15 @@ prologue_kernel(BucketView bv, const T *__restrict__ mass, double kappa, double 
 
 template <typename T>
 __global__ void __launch_bounds__(256)
-epilogue_kernel(BucketView bv, T inv_h) {
+epilogue_kernel(BucketView bv, T inv_h, bool pending, T d_scale) {
   T *x = static_cast<T *>(bv.field[F_X]);
   T *v = static_cast<T *>(bv.field[F_V]);
   const T *d = static_cast<const T *>(bv.field[F_D]);
+  const T *u = static_cast<const T *>(bv.field[F_U]);
   const size_t total = size_t(bv.cells) * 3 * bv.n_pad;
   for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < total; i += size_t(gridDim.x) * blockDim.x) {
-    const T di = d[i];
+    // pending: the last global step left its product in u (d <- d_scale d + u not applied yet)
+    const T di = pending ? d_scale * d[i] + u[i] : d[i];
     x[i] += di;
     v[i] = di * inv_h;
   }
@@ -142,14 +144,15 @@ int launch_prologue(const TypeDev &td, const BucketView &bv, int precision, cuda
   return 1;
 }
 
-int launch_epilogue(const TypeDev &td, const BucketView &bv, int precision, cudaStream_t s) {
+int launch_epilogue(const TypeDev &td, const BucketView &bv, int precision, bool pending, double d_scale,
+                    cudaStream_t s) {
   if (bv.cells == 0) return 0;
   const size_t total = size_t(bv.cells) * 3 * bv.n_pad;
   const unsigned grid = unsigned((total + 255) / 256 < 148 * 16 ? (total + 255) / 256 : 148 * 16);
   if (precision == NPFEM_F32)
-    epilogue_kernel<float><<<grid, 256, 0, s>>>(bv, float(1.0 / td.h));
+    epilogue_kernel<float><<<grid, 256, 0, s>>>(bv, float(1.0 / td.h), pending, float(d_scale));
   else
-    epilogue_kernel<double><<<grid, 256, 0, s>>>(bv, 1.0 / td.h);
+    epilogue_kernel<double><<<grid, 256, 0, s>>>(bv, 1.0 / td.h, pending, d_scale);
   return 1;
 }
 
