@@ -40,6 +40,9 @@ def parse_args():
     ap.add_argument("--iterations", type=int, default=None, help="solver iterations per step")
     ap.add_argument("--precision", default="fp32", choices=["fp32", "fp64"])
     ap.add_argument("--global-math", default="tf32", choices=["tf32", "fp32"])
+    ap.add_argument("--update-mode", type=int, default=0, choices=[0, 1, 2],
+                    help="0 auto, 1 GEMM epilogue updates d in place, 2 product-out applied by the next local step")
+    ap.add_argument("--local-impl", type=int, default=0, choices=[0, 1, 2, 3])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -182,6 +185,8 @@ def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: 
 
     solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision=args.precision, device=local_rank)
     solver.set_option(binding.OPT_GLOBAL_STEP_MATH, 0 if args.global_math == "tf32" else 1)
+    solver.set_option(binding.OPT_UPDATE_MODE, args.update_mode)
+    solver.set_option(binding.OPT_LOCAL_STEP_IMPL, args.local_impl)
     solver.set_state(torch.from_numpy(pop.packed(pop.positions)).to(dev))
     forces_host = torch.from_numpy(pop.packed(pop.forces(0), dtype=np_io)).pin_memory()
     forces_dev = forces_host.to(dev)

@@ -68,6 +68,8 @@ extern "C" {
                                          3 = scheduled kernel (register-resident topology, conflict-free slots) */
 
 #define NPFEM_OPT_KERNEL_TIMING    4  /* 1: bracket every kernel of npfem_step with CUDA events */
+#define NPFEM_OPT_UPDATE_MODE      5  /* fp32 tensor-core global step: 0 = auto (= 1), 1 = the GEMM epilogue updates d in place,
+                                         2 = the GEMM writes its product, the next local step applies it */
 
 /* kernel kinds reported by npfem_get_kernel_times */
 #define NPFEM_KIND_PROLOGUE 0

@@ -13,7 +13,7 @@ import numpy as np
 
 NPFEM_F32, NPFEM_F64 = 32, 64
 NPFEM_DEVICE, NPFEM_HOST = 0, 1
-OPT_DIAGNOSTICS, OPT_GLOBAL_STEP_MATH, OPT_LOCAL_STEP_IMPL, OPT_KERNEL_TIMING = 1, 2, 3, 4
+OPT_DIAGNOSTICS, OPT_GLOBAL_STEP_MATH, OPT_LOCAL_STEP_IMPL, OPT_KERNEL_TIMING, OPT_UPDATE_MODE = 1, 2, 3, 4, 5
 KIND_NAMES = ("prologue", "local", "global", "epilogue")
 _ERR_NAMES = {-1: "NPFEM_EINVAL", -2: "NPFEM_EMESH", -3: "NPFEM_ECUDA", -4: "NPFEM_ENOMEM", -5: "NPFEM_ESTATE"}
 

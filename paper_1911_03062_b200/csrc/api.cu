@@ -42,7 +42,7 @@ struct npfem_ctx {
   bool diagnostics = false;
   double *history_dev = nullptr;
   int history_cap = 0, history_entries = 0;
-  int64_t opt_global_math = 0, opt_local_impl = 0;
+  int64_t opt_global_math = 0, opt_local_impl = 0, opt_update_mode = 0;
   int64_t launches = 0;
   // kernel timing (NPFEM_OPT_KERNEL_TIMING)
   bool timing = false;
@@ -539,6 +539,10 @@ int npfem_set_option(npfem_ctx *c, int32_t option, int64_t value) {
       c->opt_local_impl = value;
       return NPFEM_OK;
     case NPFEM_OPT_KERNEL_TIMING: c->timing = value != 0; return NPFEM_OK;
+    case NPFEM_OPT_UPDATE_MODE:
+      if (value < 0 || value > 2) return fail(c, NPFEM_EINVAL, "update mode must be 0, 1 or 2");
+      c->opt_update_mode = value;
+      return NPFEM_OK;
     default: return fail(c, NPFEM_EINVAL, "unknown option");
   }
 }
@@ -654,12 +658,14 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
     if ((rc = timed_launch(c, NPFEM_KIND_PROLOGUE, int(t), "prologue", [&] {
            return launch_prologue(c->types[t], c->views[t], c->precision, c->stream); })))
       return rc;
-  // Fused-update mode (fp32, scheduled local step + tensor-core global step, no diagnostics): the
-  // global step only writes its product u = -H~^-1 r; the NEXT local step (or the epilogue) applies
-  // d <- (1 - gamma) d + u while it streams d anyway, so the GEMM epilogue has no loads to wait for.
+  // Product-out mode (NPFEM_OPT_UPDATE_MODE = 2; fp32, scheduled local step + tensor-core global step,
+  // no diagnostics): the global step only writes its product u = -H~^-1 r; the NEXT local step (or
+  // the epilogue) applies d <- (1 - gamma) d + u while it streams d anyway.  Measured slower than
+  // the default (the GEMM epilogue updates d in place from register-prefetched rows): 2.21 vs
+  // 2.15 ms per RBC-642 iteration at 90,000 cells, so auto (0) means mode 1.
   std::vector<char> fused(nb, 0);
   for (size_t t = 0; t < nb; ++t)
-    fused[t] = c->precision == NPFEM_F32 && !c->diagnostics && c->opt_global_math == 0 &&
+    fused[t] = c->precision == NPFEM_F32 && !c->diagnostics && c->opt_global_math == 0 && c->opt_update_mode == 2 &&
                (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]) &&
                global_tcgen05_supported(c->types[t]);
   for (int k = 0; k < n_iterations; ++k) {

@@ -193,11 +193,11 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
       const uint32_t acc = li & 1u, acc_phase = (li >> 1) & 1u;
       const int64_t row = (item / p.passes) * BM + lane_base + lane;
       const int col0 = int(item % p.passes) * p.n_pass;
-      mbar_wait(&tmem_full_bar[acc], acc_phase);
-      asm volatile("tcgen05.fence::after_thread_sync;");
       const uint32_t tacc = tmem_base + acc * MAX_NPASS + (uint32_t(lane_base) << 16);
       const bool row_ok = row < p.rows;
       if (p.U) {
+        mbar_wait(&tmem_full_bar[acc], acc_phase);
+        asm volatile("tcgen05.fence::after_thread_sync;");
         // raw product out: no loads, stores only (the consumer applies d <- d_scale d + u)
         float *urow = p.U + row * p.n_pad + col0;
         for (int c = 0; c < p.n_pass; c += 32) {
@@ -221,24 +221,49 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
           }
         }
       } else {
+        // in-place update d <- d_scale d + acc.  The d row streams through two register buffers of 64
+        // columns: the first is requested BEFORE the accumulator is awaited and each next one while the
+        // current one is processed, so the DRAM latency of d hides behind the MMAs / the TMEM reads.
         float *drow = p.D + row * p.n_pad + col0;
-        for (int c = 0; c < p.n_pass; c += 16) {
-          uint32_t r[16];
-          tmem_ld16(tacc + uint32_t(c), r);
-          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-          if (row_ok && col0 + c < p.n_pad) {
-            float4 v[4];
+        auto load_sc = [&](float4 (&buf)[16], int sc) {
 #pragma unroll
-            for (int q = 0; q < 4; ++q) v[q] = *reinterpret_cast<const float4 *>(drow + c + 4 * q);
+          for (int q = 0; q < 16; ++q) {
+            const int col = sc * 64 + q * 4;
+            buf[q] = (row_ok && col < p.n_pass && col0 + col < p.n_pad)
+                         ? __ldcs(reinterpret_cast<const float4 *>(drow + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
+          }
+        };
+        auto proc_sc = [&](float4 (&buf)[16], int sc) {
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-              v[q].x = p.d_scale * v[q].x + __uint_as_float(r[4 * q]);
-              v[q].y = p.d_scale * v[q].y + __uint_as_float(r[4 * q + 1]);
-              v[q].z = p.d_scale * v[q].z + __uint_as_float(r[4 * q + 2]);
-              v[q].w = p.d_scale * v[q].w + __uint_as_float(r[4 * q + 3]);
-              *reinterpret_cast<float4 *>(drow + c + 4 * q) = v[q];
+          for (int i = 0; i < 4; ++i) {
+            const int c = sc * 64 + i * 16;
+            if (c < p.n_pass) {                              // warp-uniform
+              uint32_t r[16];
+              tmem_ld16(tacc + uint32_t(c), r);
+              asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+              if (row_ok && col0 + c < p.n_pad) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                  float4 v = buf[4 * i + q];
+                  v.x = fmaf(p.d_scale, v.x, __uint_as_float(r[4 * q]));
+                  v.y = fmaf(p.d_scale, v.y, __uint_as_float(r[4 * q + 1]));
+                  v.z = fmaf(p.d_scale, v.z, __uint_as_float(r[4 * q + 2]));
+                  v.w = fmaf(p.d_scale, v.w, __uint_as_float(r[4 * q + 3]));
+                  *reinterpret_cast<float4 *>(drow + c + 4 * q) = v;
+                }
+              }
             }
           }
+        };
+        float4 b0[16], b1[16];
+        load_sc(b0, 0);
+        mbar_wait(&tmem_full_bar[acc], acc_phase);
+        asm volatile("tcgen05.fence::after_thread_sync;");
+        for (int sc = 0; sc * 64 < p.n_pass; sc += 2) {
+          load_sc(b1, sc + 1);
+          proc_sc(b0, sc);
+          load_sc(b0, sc + 2);
+          proc_sc(b1, sc + 1);
         }
       }
       asm volatile("tcgen05.fence::before_thread_sync;");

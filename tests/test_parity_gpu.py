@@ -178,14 +178,15 @@ def test_tf32_tensor_core_global_step_vs_fp32_ffma():
         assert rel_l2(d_tf32, d_ref) < 5e-3
 
 
-@pytest.mark.parametrize("impl", [1, 2, 3])
-def test_fp32_local_step_implementations(impl):
+@pytest.mark.parametrize("impl,update_mode", [(1, 0), (2, 0), (3, 1), (3, 2)])
+def test_fp32_local_step_implementations(impl, update_mode):
     """Every fp32 local-step kernel (1 generic, 2 shared-memory tables, 3 scheduled: register-resident
     topology + colour-assigned conflict-free slots) against the oracle; RBC-642 exercises the second
-    vertex pass of the scheduled kernel (642 vertices on 640 threads)."""
+    vertex pass of the scheduled kernel (642 vertices on 640 threads).  update_mode 1: the tensor-core GEMM
+    epilogue updates d in place; 2: it writes its product and the next local step / the epilogue applies it."""
     from paper_1911_03062_b200 import binding
     pop = make_config(3, n_cells=300)         # 273 RBC + 27 PLT: more cells than one wave of CTAs for PLT
-    gpu, solver = run_gpu(pop, "fp32", n_steps=3, n_iterations=5, options=[(binding.OPT_LOCAL_STEP_IMPL, impl)])
+    gpu, solver = run_gpu(pop, "fp32", n_steps=3, n_iterations=5, options=[(binding.OPT_LOCAL_STEP_IMPL, impl), (binding.OPT_UPDATE_MODE, update_mode)])
     solver.close()
     ref = run_oracle(pop, 3, 5)
     for r in compare(pop, gpu, ref):
