@@ -116,6 +116,129 @@ prologue_kernel(BucketView bv, const T *__restrict__ mass, double kappa, double 
   }
 }
 
+// fp32 fast path: ONE WARP per cell, the lane's vertices (x, v) stay in registers between the moment
+// pass and the update pass, so every field is read and written once.  All 16 moments (mass, m x,
+// m v, sum x x (m v), sum m x x^T about the local origin) are accumulated in fp64 in a single pass
+// and shifted to the mass centre by the parallel-axis relations; the update itself runs in fp32.
+template <int VPT>
+__global__ void __launch_bounds__(128)
+prologue_warp_kernel(BucketView bv, const float *__restrict__ mass, float kappa, float h) {
+  const int n = bv.n, n_pad = bv.n_pad, lane = threadIdx.x & 31;
+  const int64_t warp0 = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) >> 5;
+  const int64_t n_warps = (int64_t(gridDim.x) * blockDim.x) >> 5;
+  float m[VPT];
+#pragma unroll
+  for (int q = 0; q < VPT; ++q) m[q] = lane + 32 * q < n ? mass[lane + 32 * q] : 0.f;
+  const float inv_h = 1.f / h;
+  for (int64_t cell = warp0; cell < bv.cells; cell += n_warps) {
+    const size_t base = size_t(cell) * 3 * n_pad;
+    float *xg = static_cast<float *>(bv.field[F_X]) + base;
+    float *vg = static_cast<float *>(bv.field[F_V]) + base;
+    const float *fg = static_cast<const float *>(bv.field[F_F]) + base;
+    float *bg = static_cast<float *>(bv.field[F_B]) + base;
+    float *dg = static_cast<float *>(bv.field[F_D]) + base;
+    float x[VPT][3], v[VPT][3];
+#pragma unroll
+    for (int q = 0; q < VPT; ++q) {
+      const int i = lane + 32 * q;
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        x[q][k] = i < n ? __ldcs(xg + k * n_pad + i) : 0.f;
+        v[q][k] = i < n ? __ldcs(vg + k * n_pad + i) : 0.f;
+      }
+    }
+    double s[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) s[k] = 0.0;
+#pragma unroll
+    for (int q = 0; q < VPT; ++q) {
+      const double md = double(m[q]);
+      const double x0 = double(x[q][0]), x1 = double(x[q][1]), x2 = double(x[q][2]);
+      const double p0 = md * double(v[q][0]), p1 = md * double(v[q][1]), p2 = md * double(v[q][2]);
+      s[0] += md;
+      s[1] += md * x0; s[2] += md * x1; s[3] += md * x2;
+      s[4] += p0; s[5] += p1; s[6] += p2;
+      if (kappa > 0.f) {
+        s[7] += x1 * p2 - x2 * p1; s[8] += x2 * p0 - x0 * p2; s[9] += x0 * p1 - x1 * p0;
+        s[10] += md * x0 * x0; s[11] += md * x1 * x1; s[12] += md * x2 * x2;
+        s[13] += md * x0 * x1; s[14] += md * x0 * x2; s[15] += md * x1 * x2;
+      }
+    }
+    const int n_red = kappa > 0.f ? 16 : 7;
+#pragma unroll
+    for (int k = 0; k < 16; ++k)
+      if (k < n_red)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s[k] += __shfl_xor_sync(0xffffffffu, s[k], o);
+    const double M = s[0], inv_M = 1.0 / M;
+    const double xc[3] = {s[1] * inv_M, s[2] * inv_M, s[3] * inv_M};
+    const double vc[3] = {s[4] * inv_M, s[5] * inv_M, s[6] * inv_M};
+    double om[3] = {0.0, 0.0, 0.0};
+    if (kappa > 0.f) {
+      // about the mass centre: L_c = L_0 - x_c x P,  S_c = S_0 - M x_c x_c^T
+      const double L0 = s[7] - (xc[1] * s[6] - xc[2] * s[5]);
+      const double L1 = s[8] - (xc[2] * s[4] - xc[0] * s[6]);
+      const double L2 = s[9] - (xc[0] * s[5] - xc[1] * s[4]);
+      const double Sxx = s[10] - M * xc[0] * xc[0], Syy = s[11] - M * xc[1] * xc[1], Szz = s[12] - M * xc[2] * xc[2];
+      const double a = Syy + Szz, bb = Sxx + Szz, c = Sxx + Syy;
+      const double dxy = -(s[13] - M * xc[0] * xc[1]), dxz = -(s[14] - M * xc[0] * xc[2]), dyz = -(s[15] - M * xc[1] * xc[2]);
+      const double A00 = bb * c - dyz * dyz, A01 = dxz * dyz - dxy * c, A02 = dxy * dyz - dxz * bb;
+      const double A11 = a * c - dxz * dxz, A12 = dxy * dxz - a * dyz, A22 = a * bb - dxy * dxy;
+      const double inv_det = 1.0 / (a * A00 + dxy * A01 + dxz * A02);
+      om[0] = (A00 * L0 + A01 * L1 + A02 * L2) * inv_det;
+      om[1] = (A01 * L0 + A11 * L1 + A12 * L2) * inv_det;
+      om[2] = (A02 * L0 + A12 * L1 + A22 * L2) * inv_det;
+    }
+    // re-centre the local frame when the mass centre drifted (exact binary shift, rare)
+    float shift[3] = {0.f, 0.f, 0.f};
+    const bool recentre = fabs(xc[0]) > 0.5 || fabs(xc[1]) > 0.5 || fabs(xc[2]) > 0.5;
+    if (recentre) {
+      double sh[3];
+#pragma unroll
+      for (int k = 0; k < 3; ++k) { sh[k] = rint(xc[k] * 1024.0) / 1024.0; shift[k] = float(sh[k]); }
+      if (lane < 3) bv.origin[size_t(cell) * 3 + lane] += lane == 0 ? sh[0] : (lane == 1 ? sh[1] : sh[2]);
+    }
+    const float xcf[3] = {float(xc[0]), float(xc[1]), float(xc[2])}, vcf[3] = {float(vc[0]), float(vc[1]), float(vc[2])};
+    const float omf[3] = {float(om[0]), float(om[1]), float(om[2])};
+    // three separate loops so that the F loads are issued back to back (a store between two loads
+    // would serialise them on a full DRAM latency each)
+#pragma unroll
+    for (int q = 0; q < VPT; ++q) {
+      const int i = lane + 32 * q;
+      if (kappa > 0.f) {
+        const float r0 = x[q][0] - xcf[0], r1 = x[q][1] - xcf[1], r2 = x[q][2] - xcf[2];
+        const float w[3] = {omf[1] * r2 - omf[2] * r1, omf[2] * r0 - omf[0] * r2, omf[0] * r1 - omf[1] * r0};
+#pragma unroll
+        for (int k = 0; k < 3; ++k) v[q][k] += kappa * (vcf[k] + w[k] - v[q][k]);
+      }
+      if (recentre && i < n) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) xg[k * n_pad + i] = x[q][k] - shift[k];
+      }
+    }
+    float f[VPT][3];
+#pragma unroll
+    for (int q = 0; q < VPT; ++q) {
+      const int i = lane + 32 * q;
+#pragma unroll
+      for (int k = 0; k < 3; ++k) f[q][k] = i < n ? __ldcs(fg + k * n_pad + i) : 0.f;
+    }
+#pragma unroll
+    for (int q = 0; q < VPT; ++q) {
+      const int i = lane + 32 * q;
+      if (i < n) {
+        const float mh = m[q] * inv_h;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+          vg[k * n_pad + i] = v[q][k];
+          bg[k * n_pad + i] = fmaf(mh, v[q][k], f[q][k]);
+          dg[k * n_pad + i] = h * v[q][k];
+        }
+      }
+    }
+  }
+}
+
 template <typename T>
 __global__ void __launch_bounds__(256)
 epilogue_kernel(BucketView bv, T inv_h, bool pending, T d_scale) {
@@ -137,7 +260,15 @@ epilogue_kernel(BucketView bv, T inv_h, bool pending, T d_scale) {
 int launch_prologue(const TypeDev &td, const BucketView &bv, int precision, cudaStream_t s) {
   if (bv.cells == 0) return 0;
   const unsigned grid = unsigned(bv.cells < 148 * 16 ? bv.cells : 148 * 16);
-  if (precision == NPFEM_F32)
+  if (precision == NPFEM_F32 && td.n <= 32 * 21) {
+    // warp per cell; 4 warps per CTA, enough CTAs to fill the machine several times over
+    const int64_t ctas = (bv.cells + 3) / 4;
+    const unsigned g = unsigned(ctas < 148 * 24 ? ctas : 148 * 24);
+    if (td.n <= 32 * 6)
+      prologue_warp_kernel<6><<<g, 128, 0, s>>>(bv, static_cast<const float *>(td.vtx_mass), float(td.kappa), float(td.h));
+    else
+      prologue_warp_kernel<21><<<g, 128, 0, s>>>(bv, static_cast<const float *>(td.vtx_mass), float(td.kappa), float(td.h));
+  } else if (precision == NPFEM_F32)
     prologue_kernel<float><<<grid, 256, 0, s>>>(bv, static_cast<const float *>(td.vtx_mass), td.kappa, td.h);
   else
     prologue_kernel<double><<<grid, 256, 0, s>>>(bv, static_cast<const double *>(td.vtx_mass), td.kappa, td.h);
