@@ -106,8 +106,11 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
   for (int q = 0; q < 1 + MAXV / 2; ++q) vw[q] = p.vtx_words[q * p.vstride + tid];
   const float coef = p.vtx_coef[tid];
   const bool vact = tid < n;
-  const int v2 = tid + nthreads;       // a few vertices may need a second pass (n slightly above the CTA size):
-  const bool vact2 = v2 < n;           // their constants stay in global memory (L1/L2 hits)
+  // a few vertices may need a second pass (n slightly above the CTA size): the LAST warp takes them
+  // (warp 0 already issues the TMA prefetches: any extra work of ONE warp delays the whole block at
+  // the next barrier), their constants stay in global memory (L1 hits)
+  const int v2 = tid + 32;
+  const bool vact2 = tid >= nthreads - 32 && v2 < n;
 
   auto prefetch = [&](int64_t cell, int st) {   // one thread: arm the barrier, start 3 bulk copies
     const size_t base = size_t(cell) * 3 * n_pad;

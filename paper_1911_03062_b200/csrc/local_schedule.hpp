@@ -31,7 +31,7 @@ namespace npfem {
 
 struct LocalSchedule {
   bool valid = false;
-  int threads = 0;   // CTA size (multiple of 32); vertex v is owned by thread v % threads (pass v / threads)
+  int threads = 0;   // CTA size (multiple of 32); vertex v < threads is owned by thread v, the rest by the last warp
   int vstride = 0;   // row stride of the vertex tables (>= n)
   int tpt = 0;       // triangles per thread
   int ttri = 0;      // threads that own triangles (multiple of 8): triangle t = j*ttri + tid
@@ -190,7 +190,7 @@ inline bool build_local_schedule(const HostTypeData &h, const double *X, int tpt
   if (h.valence_max > 8 || tpt < 1 || tpt > 2) return false;
   const int ttri = ((T + tpt - 1) / tpt + 7) / 8 * 8;
   const int threads = (ttri + 31) / 32 * 32;      // triangle threads decide; a few vertices may take a 2nd pass
-  if (n > 2 * threads) return false;
+  if (n > threads + 32) return false;             // the overflow vertices are one extra pass of the last warp
   const int vstride = std::max(threads, (n + 31) / 32 * 32);
   const int maxv = h.valence_max <= 6 ? 6 : 8;
   const int n_vslots = (n + 7) / 8 * 8, n_tslots = tpt * ttri;
