@@ -25,12 +25,15 @@ namespace {
 constexpr int BM = 128;          // rows per tile (TMEM lanes)
 constexpr int BK = 32;           // fp32 per K chunk = 128 bytes = one swizzle row
 constexpr int UMMA_K = 8;        // K per tcgen05.mma for tf32 (32 bytes)
-constexpr int STAGES = 4;
+constexpr int STAGES = 3;
+constexpr int CL = 2;             // thread-block cluster: CL CTAs work on CL consecutive M tiles and share every W tile
 constexpr int MAX_NPASS = 256;   // accumulator columns per pass: two accumulators fit the 512 TMEM columns
 constexpr int A_BYTES = BM * BK * 4;
 constexpr int B_BYTES = MAX_NPASS * BK * 4;
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024;
+constexpr int EBUF = 4;           // per epilogue warp: ring of [32 rows x 32 cols] fp32 staging tiles (4 KB each)
+constexpr int EPI_BYTES = 4 * EBUF * 4096;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + EPI_BYTES + 1024;
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return uint32_t(__cvta_generic_to_shared(p)); }
 
@@ -60,6 +63,28 @@ __device__ __forceinline__ void tma_load_2d(void *smem_dst, const CUtensorMap *m
   asm volatile(
       "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
       ::"r"(smem_u32(smem_dst)), "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y) : "memory");
+}
+
+// same, delivered to the same shared-memory offset of every CTA in `mask` (their full barriers at the
+// same offset receive the complete_tx)
+__device__ __forceinline__ void tma_load_2d_mc(void *smem_dst, const CUtensorMap *map, int x, int y, uint64_t *bar,
+                                               uint16_t mask) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1, {%3, %4}], [%2], %5;"
+      ::"r"(smem_u32(smem_dst)), "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y), "h"(mask) : "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap *map, int x, int y, const void *smem_src) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
+               ::"l"(map), "r"(smem_u32(smem_src)), "r"(x), "r"(y) : "memory");
 }
 
 // K-major, 128B-swizzled operand tile: 8-row atoms of 1024 bytes (SBO), version 1 (sm_100)
@@ -92,6 +117,12 @@ __device__ __forceinline__ void umma_commit(uint64_t *bar) {
                : "memory");
 }
 
+// arrives on the barrier at this offset in every CTA of `mask` once the MMAs issued so far have retired
+__device__ __forceinline__ void umma_commit_mc(uint64_t *bar, uint16_t mask) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(smem_u32(bar)), "h"(mask) : "memory");
+}
+
 struct GemmParams {
   float *D;            // [rows][n_pad], updated in place (U == nullptr)
   float *U;            // [rows][n_pad] or nullptr: write the raw product -G W here instead of updating D
@@ -114,23 +145,30 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
 
 __global__ void __launch_bounds__(192, 1)
 global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_constant__ CUtensorMap map_w,
-                      const GemmParams p) {
+                      const __grid_constant__ CUtensorMap map_d, const GemmParams p) {
   extern __shared__ unsigned char smem_raw[];
-  __shared__ uint64_t full_bar[STAGES], empty_bar[STAGES], tmem_full_bar[2], tmem_empty_bar[2];
+  __shared__ uint64_t full_bar[STAGES], empty_bar[STAGES], tmem_full_bar[2], tmem_empty_bar[2], epi_full[4 * EBUF];
   __shared__ uint32_t tmem_base_sh;
   unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t n_items = p.m_tiles * p.passes;
+  // work item of a CLUSTER = (group of CL consecutive M tiles, N pass); CTA `rank` takes tile CL*group + rank.
+  // A tile past the end is processed like any other (TMA zero-fills, the epilogue stores nothing) so
+  // that both CTAs keep the multicast protocol in step.
+  const uint32_t rank = cluster_ctarank();
+  const int64_t n_items = ((p.m_tiles + CL - 1) / CL) * p.passes;
+  const int64_t first_item = blockIdx.x / CL, item_step = gridDim.x / CL;
+  constexpr uint16_t MASK = uint16_t((1u << CL) - 1u);
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) {
       mbar_init(&full_bar[s], 1);
-      mbar_init(&empty_bar[s], 1);
+      mbar_init(&empty_bar[s], CL);                         // every CTA of the cluster reads what lands here
     }
     for (int a = 0; a < 2; ++a) {
       mbar_init(&tmem_full_bar[a], 1);
       mbar_init(&tmem_empty_bar[a], 128);
     }
+    for (int b = 0; b < 4 * EBUF; ++b) mbar_init(&epi_full[b], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {   // TMEM: all 512 columns (one CTA per SM) = two accumulators of <= 256 columns
@@ -139,6 +177,7 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
   }
   asm volatile("tcgen05.fence::before_thread_sync;");
   __syncthreads();
+  cluster_sync_all();                                       // the peers' barriers exist before anyone signals them
   asm volatile("tcgen05.fence::after_thread_sync;");
   const uint32_t tmem_base = tmem_base_sh;
 
@@ -148,14 +187,16 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
       int stage = 0;
       uint32_t phase = 0;
       const uint32_t tx = A_BYTES + uint32_t(p.n_pass) * BK * 4;
-      for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
-        const int row0 = int((item / p.passes) * BM), col0 = int(item % p.passes) * p.n_pass;
+      const int w_rows = p.n_pass / CL;                     // this CTA's slice of the W tile (multiple of 8 rows)
+      for (int64_t item = first_item; item < n_items; item += item_step) {
+        const int row0 = int(((item / p.passes) * CL + rank) * BM), col0 = int(item % p.passes) * p.n_pass;
         for (int kc = 0; kc < p.k_chunks; ++kc) {
-          mbar_wait(&empty_bar[stage], phase ^ 1);
+          mbar_wait(&empty_bar[stage], phase ^ 1);          // this slot is free in EVERY CTA of the cluster
           unsigned char *sa = smem + stage * STAGE_BYTES, *sb = sa + A_BYTES;
-          mbar_expect_tx(&full_bar[stage], tx);
+          mbar_expect_tx(&full_bar[stage], tx);             // own G tile + all CL slices of the W tile
           tma_load_2d(sa, &map_g, kc * BK, row0, &full_bar[stage]);
-          tma_load_2d(sb, &map_w, kc * BK, col0, &full_bar[stage]);
+          tma_load_2d_mc(sb + size_t(rank) * w_rows * BK * 4, &map_w, kc * BK, col0 + int(rank) * w_rows,
+                         &full_bar[stage], MASK);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
@@ -166,7 +207,7 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
       int stage = 0;
       uint32_t phase = 0, li = 0;
       const uint32_t idesc = make_idesc(BM, p.n_pass);
-      for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x, ++li) {
+      for (int64_t item = first_item; item < n_items; item += item_step, ++li) {
         const uint32_t acc = li & 1u, acc_phase = (li >> 1) & 1u;
         mbar_wait(&tmem_empty_bar[acc], acc_phase ^ 1);     // epilogue has drained this accumulator
         asm volatile("tcgen05.fence::after_thread_sync;");
@@ -179,7 +220,7 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
           for (int k = 0; k < BK / UMMA_K; ++k)
             umma_tf32(tacc, make_smem_desc(sa + k * UMMA_K * 4), make_smem_desc(sb + k * UMMA_K * 4), idesc,
                       (kc | k) != 0);
-          umma_commit(&empty_bar[stage]);                   // frees the smem slot when the MMAs retire
+          umma_commit_mc(&empty_bar[stage], MASK);          // frees the slot in every CTA when these MMAs retire
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
         umma_commit(&tmem_full_bar[acc]);                   // accumulator complete
@@ -187,90 +228,79 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
     }
   } else {
     // ===== epilogue: warps 2..5 own TMEM lanes 32*(warp%4) .. +31; overlaps the next item's MMAs =====
+    // d <- d_scale d + acc (or u <- acc) in tiles of [32 rows x 32 columns], each warp on its own ring of
+    // EBUF staging tiles: TMA load (128B swizzle) -> every lane updates ITS row in shared memory
+    // (conflict-free thanks to the swizzle) -> TMA store.  All global traffic of the epilogue is
+    // full 128-byte rows moved by the TMA unit; a row-per-lane LDG/STG pattern (32 lines per warp
+    // instruction) held the previous version to a third of the tensor peak.
     const int lane_base = (warp & 3) * 32;
+    unsigned char *ebuf = smem + STAGES * STAGE_BYTES + (warp & 3) * (EBUF * 4096);
+    uint64_t *efull = &epi_full[(warp & 3) * EBUF];
+    const bool rmw = p.U == nullptr;
+    const int n_chunks = (p.n_pass + 31) / 32;
+    uint32_t g = 0;                                         // tiles this warp has processed (ring position)
     uint32_t li = 0;
-    for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x, ++li) {
+    for (int64_t item = first_item; item < n_items; item += item_step, ++li) {
       const uint32_t acc = li & 1u, acc_phase = (li >> 1) & 1u;
-      const int64_t row = (item / p.passes) * BM + lane_base + lane;
+      const int row0w = int(((item / p.passes) * CL + rank) * BM) + lane_base;
       const int col0 = int(item % p.passes) * p.n_pass;
       const uint32_t tacc = tmem_base + acc * MAX_NPASS + (uint32_t(lane_base) << 16);
-      const bool row_ok = row < p.rows;
-      if (p.U) {
-        mbar_wait(&tmem_full_bar[acc], acc_phase);
-        asm volatile("tcgen05.fence::after_thread_sync;");
-        // raw product out: no loads, stores only (the consumer applies d <- d_scale d + u)
-        float *urow = p.U + row * p.n_pad + col0;
-        for (int c = 0; c < p.n_pass; c += 32) {
+      auto issue_load = [&](int c, uint32_t gc) {           // lane 0 only
+        const uint32_t b = gc % EBUF;
+        asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // the store that last read this tile is done
+        mbar_expect_tx(&efull[b], 4096);
+        tma_load_2d(ebuf + b * 4096, &map_d, col0 + 32 * c, row0w, &efull[b]);
+      };
+      if (rmw && lane == 0) {                               // requested before the accumulator is awaited
+        issue_load(0, g);
+        if (n_chunks > 1) issue_load(1, g + 1);
+      }
+      mbar_wait(&tmem_full_bar[acc], acc_phase);
+      asm volatile("tcgen05.fence::after_thread_sync;");
+      for (int c = 0; c < n_chunks; ++c) {
+        const uint32_t gc = g + uint32_t(c), b = gc % EBUF;
+        if (rmw && lane == 0 && c + 2 < n_chunks) issue_load(c + 2, gc + 2);
+        uint32_t r[32];
+        {
           uint32_t r0[16], r1[16];
-          tmem_ld16(tacc + uint32_t(c), r0);
-          tmem_ld16(tacc + uint32_t(c) + 16u, r1);          // n_pass is a multiple of 16: may read an unused column block
+          tmem_ld16(tacc + uint32_t(32 * c), r0);
+          tmem_ld16(tacc + uint32_t(32 * c) + 16u, r1);     // may read an unused column block: clipped by the store
           asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-          if (row_ok && col0 + c < p.n_pad) {
 #pragma unroll
-            for (int q = 0; q < 4; ++q)
-              *reinterpret_cast<float4 *>(urow + c + 4 * q) =
-                  make_float4(__uint_as_float(r0[4 * q]), __uint_as_float(r0[4 * q + 1]), __uint_as_float(r0[4 * q + 2]),
-                              __uint_as_float(r0[4 * q + 3]));
-          }
-          if (row_ok && c + 16 < p.n_pass && col0 + c + 16 < p.n_pad) {
-#pragma unroll
-            for (int q = 0; q < 4; ++q)
-              *reinterpret_cast<float4 *>(urow + c + 16 + 4 * q) =
-                  make_float4(__uint_as_float(r1[4 * q]), __uint_as_float(r1[4 * q + 1]), __uint_as_float(r1[4 * q + 2]),
-                              __uint_as_float(r1[4 * q + 3]));
-          }
+          for (int q = 0; q < 16; ++q) { r[q] = r0[q]; r[16 + q] = r1[q]; }
         }
-      } else {
-        // in-place update d <- d_scale d + acc.  The d row streams through two register buffers of 64
-        // columns: the first is requested BEFORE the accumulator is awaited and each next one while the
-        // current one is processed, so the DRAM latency of d hides behind the MMAs / the TMEM reads.
-        float *drow = p.D + row * p.n_pad + col0;
-        auto load_sc = [&](float4 (&buf)[16], int sc) {
+        if (rmw) {
+          mbar_wait(&efull[b], (gc / EBUF) & 1u);
+        } else {
+          if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 3;" ::: "memory");
+          __syncwarp();
+        }
+        float4 *rowp = reinterpret_cast<float4 *>(ebuf + b * 4096 + lane * 128);
 #pragma unroll
-          for (int q = 0; q < 16; ++q) {
-            const int col = sc * 64 + q * 4;
-            buf[q] = (row_ok && col < p.n_pass && col0 + col < p.n_pad)
-                         ? __ldcs(reinterpret_cast<const float4 *>(drow + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
-          }
-        };
-        auto proc_sc = [&](float4 (&buf)[16], int sc) {
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const int c = sc * 64 + i * 16;
-            if (c < p.n_pass) {                              // warp-uniform
-              uint32_t r[16];
-              tmem_ld16(tacc + uint32_t(c), r);
-              asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-              if (row_ok && col0 + c < p.n_pad) {
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                  float4 v = buf[4 * i + q];
-                  v.x = fmaf(p.d_scale, v.x, __uint_as_float(r[4 * q]));
-                  v.y = fmaf(p.d_scale, v.y, __uint_as_float(r[4 * q + 1]));
-                  v.z = fmaf(p.d_scale, v.z, __uint_as_float(r[4 * q + 2]));
-                  v.w = fmaf(p.d_scale, v.w, __uint_as_float(r[4 * q + 3]));
-                  *reinterpret_cast<float4 *>(drow + c + 4 * q) = v;
-                }
-              }
-            }
-          }
-        };
-        float4 b0[16], b1[16];
-        load_sc(b0, 0);
-        mbar_wait(&tmem_full_bar[acc], acc_phase);
-        asm volatile("tcgen05.fence::after_thread_sync;");
-        for (int sc = 0; sc * 64 < p.n_pass; sc += 2) {
-          load_sc(b1, sc + 1);
-          proc_sc(b0, sc);
-          load_sc(b0, sc + 2);
-          proc_sc(b1, sc + 1);
+        for (int q = 0; q < 8; ++q) {
+          float4 *slot = rowp + (q ^ (lane & 7));           // 128B swizzle: 16-byte chunk q of row r sits at q ^ (r % 8)
+          float4 v = rmw ? *slot : make_float4(0.f, 0.f, 0.f, 0.f);
+          v.x = fmaf(p.d_scale, v.x, __uint_as_float(r[4 * q]));
+          v.y = fmaf(p.d_scale, v.y, __uint_as_float(r[4 * q + 1]));
+          v.z = fmaf(p.d_scale, v.z, __uint_as_float(r[4 * q + 2]));
+          v.w = fmaf(p.d_scale, v.w, __uint_as_float(r[4 * q + 3]));
+          *slot = v;
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) {                                    // rows / columns past the matrix are clipped by the TMA unit
+          tma_store_2d(&map_d, col0 + 32 * c, row0w, ebuf + b * 4096);
+          asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
       }
+      g += uint32_t(n_chunks);
       asm volatile("tcgen05.fence::before_thread_sync;");
       mbar_arrive(&tmem_empty_bar[acc]);
     }
+    if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
   }
   __syncthreads();
+  cluster_sync_all();                                       // no CTA leaves while a peer may still signal it
   if (warp == 1) {
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base));
   }
@@ -313,7 +343,7 @@ static bool gemm_shape(const TypeDev &td, GemmParams &p) {
   p.n_pad = td.n_pad;
   p.passes = (td.n_pad + MAX_NPASS - 1) / MAX_NPASS;
   p.n_pass = ((td.n_pad + p.passes - 1) / p.passes + 15) / 16 * 16;
-  if (p.n_pass > MAX_NPASS || p.n_pass < 16 || td.Hinv == nullptr) return false;
+  if (p.n_pass > MAX_NPASS || p.n_pass < 16 || (p.n_pass / CL) % 8 != 0 || td.Hinv == nullptr) return false;
   p.k_chunks = (td.n_pad + BK - 1) / BK;
   return true;
 }
@@ -335,20 +365,36 @@ int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, dou
   p.rows = bv.cells * 3;
   p.m_tiles = (p.rows + BM - 1) / BM;
   p.d_scale = float(d_scale);
-  CUtensorMap map_g, map_w;
+  CUtensorMap map_g, map_w, map_d;
   if (!make_map(&map_g, bv.field[F_G], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), BM)) return -1;
-  if (!make_map(&map_w, td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n_pass))) return -1;
+  if (!make_map(&map_w, td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n_pass / CL)))
+    return -1;
+  // epilogue tiles: [32 rows][32 columns] of D (in-place update) or of U (product out)
+  if (!make_map(&map_d, u_out ? u_out : bv.field[F_D], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), 32))
+    return -1;
   static bool attr = false;
   if (!attr) {
     if (cudaFuncSetAttribute(global_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES) != cudaSuccess)
       return -1;
     attr = true;
   }
-  const int64_t items = p.m_tiles * p.passes;
-  // the passes of one M tile are adjacent items: they run on neighbouring CTAs at about the same
-  // time, so the repeated reads of the G tile are L2 hits
-  const unsigned grid = unsigned(items < n_sm ? items : n_sm);
-  global_tcgen05_kernel<<<grid, 192, SMEM_BYTES, s>>>(map_g, map_w, p);
+  // the passes of one group of M tiles are adjacent items: they run on neighbouring clusters at about
+  // the same time, so the repeated reads of the G tiles are L2 hits
+  const int64_t items = ((p.m_tiles + CL - 1) / CL) * p.passes;
+  const int64_t clusters = items < n_sm / CL ? items : n_sm / CL;
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(unsigned(clusters * CL));
+  cfg.blockDim = dim3(192);
+  cfg.dynamicSmemBytes = SMEM_BYTES;
+  cfg.stream = s;
+  cudaLaunchAttribute attrs[1];
+  attrs[0].id = cudaLaunchAttributeClusterDimension;
+  attrs[0].val.clusterDim.x = CL;
+  attrs[0].val.clusterDim.y = 1;
+  attrs[0].val.clusterDim.z = 1;
+  cfg.attrs = attrs;
+  cfg.numAttrs = 1;
+  if (cudaLaunchKernelEx(&cfg, global_tcgen05_kernel, map_g, map_w, map_d, p) != cudaSuccess) return -1;
   return 1;
 }
 
