@@ -84,7 +84,7 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
   float *stage = reinterpret_cast<float *>(sC + p.sC_bytes);            // [NSTAGE][4 fields x, d, b, u][3][n_pad]
   int *vacc = reinterpret_cast<int *>(stage + NSTAGE * 12 * n_pad);   // [2 cells][hi, lo] base-2^24 digits of 6V
   uint64_t *mbar = reinterpret_cast<uint64_t *>(vacc + 4);   // [NSTAGE] TMA ring
-  uint64_t *bars = mbar + NSTAGE;                              // [3] split block barriers B1, B2, B3
+  uint64_t *bars = mbar + NSTAGE;                              // [4] split block barriers B1, B2, B3, BV
 
   const int tid = threadIdx.x, lane = tid & 31;
   const uint32_t field_bytes = uint32_t(3 * n_pad) * 4u;
@@ -109,8 +109,12 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
   // a few vertices may need a second pass (n slightly above the CTA size): the LAST warp takes them
   // (warp 0 already issues the TMA prefetches: any extra work of ONE warp delays the whole block at
   // the next barrier), their constants stay in global memory (L1 hits)
+  // phase 0 of the overflow vertices runs in the last warp, their phase C in the one before it, so
+  // no warp carries both extras
   const int v2 = tid + 32;
   const bool vact2 = tid >= nthreads - 32 && v2 < n;
+  const int v2c = tid + 64;
+  const bool vact2c = tid >= nthreads - 64 && tid < nthreads - 32 && v2c < n;
 
   auto prefetch = [&](int64_t cell, int st) {   // one thread: arm the barrier, start 3 bulk copies
     const size_t base = size_t(cell) * 3 * n_pad;
@@ -129,7 +133,7 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
 #pragma unroll
     for (int s = 0; s < NSTAGE; ++s) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(mbar + s)));
 #pragma unroll
-    for (int s = 0; s < 3; ++s)
+    for (int s = 0; s < 4; ++s)
       asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bars + s)), "r"(nthreads >> 5));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     vacc[0] = vacc[1] = vacc[2] = vacc[3] = 0;
@@ -191,7 +195,8 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
   };
 
   // Software pipeline over the cells of this CTA (B1/B2/B3 = split barriers, parity it & 1):
-  //   wait B1 | phase A | arrive B2 | wait B2 | phase B | arrive B3 | phase 0 of the NEXT cell |
+  //   wait B1 | phase A | arrive B2 | volume, arrive BV | membrane | wait B2 | hinges | wait BV |
+  //   corner forces | arrive B3 | phase 0 of the NEXT cell |
   //   arrive B1 | wait B3 | phase C
   // so a warp that is early at a barrier runs ahead into work that does not depend on it.
   if (int64_t(blockIdx.x) < p.cells) {
@@ -222,6 +227,9 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
         if (act[j]) sts4(sN, hi16(tw[j][4]), nh[j][0], nh[j][1], nh[j][2], inv[j]);
       }
     }
+    bar_arrive(1);                                     // B2: this warp's normals are stored
+    // the volume has its own barrier (BV), awaited only where the volume coefficient is used, so the
+    // shuffle chain and the atomics stay off the critical path of B2
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) vol += __shfl_xor_sync(0xffffffffu, vol, o);
     if (lane == 0) {   // exact, order-independent: fixed point, split into a signed high and a 24-bit low digit
@@ -229,7 +237,7 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
       atomicAdd(vacc + 2 * (it & 1), int(v >> 24));
       atomicAdd(vacc + 2 * (it & 1) + 1, int(v & 0xffffff));
     }
-    bar_arrive(1);
+    bar_arrive(3);
     // membrane part of phase B needs this thread's registers only: it overlaps the wait for B2
     // (Skalak, readings R5/R7): Q = 2 A0 (W1 R + W2 det^2 adj G)
     float e11[TPT], e12[TPT], e22[TPT], q11[TPT], q12[TPT], q22[TPT];
@@ -248,7 +256,7 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
       q22[j] = fmaf(W2, e11[j], W1 * R22);
       q12[j] = fmaf(-W2, e12[j], W1 * R12);
     }
-    bar_wait(1, par);                                  // B2: sN complete, volume accumulated
+    bar_wait(1, par);                                  // B2: sN complete
     if (tid == 0) {
       // every thread is past phase C of the previous cell: its ring slot and the other volume
       // accumulator are free
@@ -256,8 +264,6 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
       const int64_t nxt = cell + int64_t(NSTAGE - 1) * gridDim.x;
       if (nxt < p.cells) prefetch(nxt, (it + NSTAGE - 1) % NSTAGE);
     }
-    const int2 vd = *reinterpret_cast<const int2 *>(vacc + 2 * (it & 1));
-    const float vc = float(((double(vd.x) * 16777216.0 + double(vd.y)) * p.fx_inv - p.V0x6) * p.kv_coef);
     // ---- phase B ----------------------------------------------------------------------------
     // all neighbour normals first (independent loads in flight together), then the hinge weights of
     // every triangle, then membrane + corner forces + stores (stores last: they would fence the loads)
@@ -303,6 +309,9 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
       }
       hw[j][0] = w0; hw[j][1] = w1; hw[j][2] = w2;
     }
+    bar_wait(3, par);                                  // BV: volume accumulated
+    const int2 vd = *reinterpret_cast<const int2 *>(vacc + 2 * (it & 1));
+    const float vc = float(((double(vd.x) * 16777216.0 + double(vd.y)) * p.fx_inv - p.V0x6) * p.kv_coef);
     float cf[TPT][9];
 #pragma unroll
     for (int j = 0; j < TPT; ++j) {
@@ -345,18 +354,18 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
       gout[n_pad] = fmaf(coef, sg[4 * n_pad + tid], ay - sg[7 * n_pad + tid]);
       gout[2 * n_pad] = fmaf(coef, sg[5 * n_pad + tid], az - sg[8 * n_pad + tid]);
     }
-    if (vact2) {
+    if (vact2c) {
       float ax = 0.f, ay = 0.f, az = 0.f;
       for (int q = 0; q < MAXV; ++q) {
-        const uint32_t w = p.vtx_words[(1 + (q >> 1)) * p.vstride + v2];
+        const uint32_t w = p.vtx_words[(1 + (q >> 1)) * p.vstride + v2c];
         const float4 f = lds4(sC, (q & 1) ? (w >> 16) : (w & 0xffffu));
         ax += f.x; ay += f.y; az += f.z;
       }
-      const float coef2 = p.vtx_coef[v2];
-      float *gout = p.g + size_t(cell) * 3 * n_pad + v2;
-      gout[0] = fmaf(coef2, sg[3 * n_pad + v2], ax - sg[6 * n_pad + v2]);
-      gout[n_pad] = fmaf(coef2, sg[4 * n_pad + v2], ay - sg[7 * n_pad + v2]);
-      gout[2 * n_pad] = fmaf(coef2, sg[5 * n_pad + v2], az - sg[8 * n_pad + v2]);
+      const float coef2 = p.vtx_coef[v2c];
+      float *gout = p.g + size_t(cell) * 3 * n_pad + v2c;
+      gout[0] = fmaf(coef2, sg[3 * n_pad + v2c], ax - sg[6 * n_pad + v2c]);
+      gout[n_pad] = fmaf(coef2, sg[4 * n_pad + v2c], ay - sg[7 * n_pad + v2c]);
+      gout[2 * n_pad] = fmaf(coef2, sg[5 * n_pad + v2c], az - sg[8 * n_pad + v2c]);
     }
     // sN / sC are rewritten only after B1 / B2 of the next cell, which every warp reaches after this
   }
@@ -367,7 +376,7 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
 namespace {
 
 size_t sched_smem_bytes(const SchedDev &s, int n_pad) {
-  return size_t(s.n_vslots + s.n_tslots + s.n_cslots) * 16 + size_t(NSTAGE) * 12 * n_pad * 4 + 4 * 4 + (NSTAGE + 3) * 8;
+  return size_t(s.n_vslots + s.n_tslots + s.n_cslots) * 16 + size_t(NSTAGE) * 12 * n_pad * 4 + 4 * 4 + (NSTAGE + 4) * 8;
 }
 
 template <int TPT, int MAXV, int MAXT, int MINB>

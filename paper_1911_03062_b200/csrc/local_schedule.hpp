@@ -190,7 +190,8 @@ inline bool build_local_schedule(const HostTypeData &h, const double *X, int tpt
   if (h.valence_max > 8 || tpt < 1 || tpt > 2) return false;
   const int ttri = ((T + tpt - 1) / tpt + 7) / 8 * 8;
   const int threads = (ttri + 31) / 32 * 32;      // triangle threads decide; a few vertices may take a 2nd pass
-  if (n > threads + 32) return false;             // the overflow vertices are one extra pass of the last warp
+  // up to 32 overflow vertices: phase 0 in the last warp, phase C in the one before it
+  if (n > threads + 32 || (n > threads && threads < 64)) return false;
   const int vstride = std::max(threads, (n + 31) / 32 * 32);
   const int maxv = h.valence_max <= 6 ? 6 : 8;
   const int n_vslots = (n + 7) / 8 * 8, n_tslots = tpt * ttri;
