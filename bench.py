@@ -171,6 +171,23 @@ def run_reference(args, pop, n_iterations: int, config_desc: dict):
     }
 
 
+# ---- multi-rank plumbing (one process per GPU, replicas only: DESIGN.md section 8) ---------------
+def max_over_ranks(value_ms: float, world: int, device: str) -> float:
+    """Device time of the slowest rank (all_reduce MAX); identity for one rank."""
+    if world <= 1:
+        return float(value_ms)
+    import torch
+    t = torch.tensor([value_ms], device=device, dtype=torch.float64)
+    torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_throughput(cells_per_rank: int, n_iterations: int, steps: int, world: int, max_ms: float) -> float:
+    """Whole-job cells*iterations/s: every rank advances its own replica (weak scaling), the clock is
+    the slowest rank's."""
+    return world * cells_per_rank * n_iterations * steps / (max_ms * 1e-3)
+
+
 # ---- the B200 arm ------------------------------------------------------------------------------
 def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: int):
     import torch
@@ -215,12 +232,9 @@ def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: 
     launches = solver.launch_count - launches0
     ktimes = solver.get_kernel_times(reset=True)
     solver.set_option(binding.OPT_KERNEL_TIMING, 0)
-    if world > 1:
-        t = torch.tensor([elapsed_ms], device=dev, dtype=torch.float64)
-        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-        elapsed_ms = float(t.item())
+    elapsed_ms = max_over_ranks(elapsed_ms, world, dev)
     cell_iters = pop.n_cells * n_iterations * args.steps
-    value = world * cell_iters / (elapsed_ms * 1e-3)
+    value = aggregate_throughput(pop.n_cells, n_iterations, args.steps, world, elapsed_ms)
 
     # ---- per-kernel rooflines from the live CUDA-event times ---------------------------------
     kernels, total_kernel_ms = [], sum(ms for v in ktimes.values() for ms, _ in v)
@@ -278,11 +292,8 @@ def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: 
         e1.record()
         barrier()
         e2e_ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-            torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-            e2e_ms = float(t.item())
-        result["e2e"] = {"value": world * cell_iters / (e2e_ms * 1e-3), "unit": UNIT,
+        e2e_ms = max_over_ranks(e2e_ms, world, dev)
+        result["e2e"] = {"value": aggregate_throughput(pop.n_cells, n_iterations, args.steps, world, e2e_ms), "unit": UNIT,
                          "h2d_bytes_per_step": int(forces_host.numel() * forces_host.element_size()),
                          "d2h_bytes_per_step": int(2 * count * pos_host.element_size()),
                          "ms_per_step": e2e_ms / args.steps}

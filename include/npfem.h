@@ -175,6 +175,24 @@ int npfem_get_kernel_times(npfem_ctx *ctx, double *ms, int64_t *launches, int32_
 /* Number of kernels the library has launched on this context so far. */
 int64_t npfem_launch_count(const npfem_ctx *ctx);
 
+/*
+ * Host-only diagnostic (no CUDA device needed): builds the create-time shared-memory schedule of the
+ * fp32 scheduled local step for one cell type (slots of vertex positions / triangle normals / corner
+ * forces assigned by graph colouring so that the kernel's gathers avoid bank conflicts) and checks
+ * it.  stats (HOST, n_stats >= 10 doubles):
+ *   [0] 1 if the type fits the scheduled kernel, else 0 (the rest is then 0)
+ *   [1] CTA threads  [2] triangles per thread
+ *   [3] predicted wavefronts per vertex-gather instruction   (ideal 4.0)
+ *   [4] predicted wavefronts per normal-gather instruction   (ideal 4.0)
+ *   [5] worst wavefronts of a corner-force STORE instruction quarter (exactly 1.0 expected)
+ *   [6] worst wavefronts of a corner-force GATHER instruction quarter (exactly 1.0 expected)
+ *   [7] 1 if every vertex / triangle / corner slot is unique and every table entry decodes to the
+ *       mesh's own connectivity, else 0
+ *   [8] shared-memory bytes of the kernel's per-cell arrays  [9] host milliseconds to build
+ * Returns NPFEM_OK, NPFEM_EINVAL or NPFEM_EMESH (message via npfem_last_error(NULL)).
+ */
+int npfem_local_schedule_stats(const npfem_cell_type *type, double dt, double *stats, int32_t n_stats);
+
 /* Message of the last failure on `ctx` (ctx == NULL: of the last failed npfem_create). */
 const char *npfem_last_error(const npfem_ctx *ctx);
 

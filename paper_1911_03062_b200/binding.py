@@ -21,6 +21,7 @@ EXPORTED_SYMBOLS = (
     "npfem_create", "npfem_workspace_bytes", "npfem_bind_workspace", "npfem_set_option",
     "npfem_set_state", "npfem_set_forces", "npfem_step", "npfem_get_state", "npfem_get_objective",
     "npfem_get_kernel_times", "npfem_launch_count", "npfem_last_error", "npfem_version", "npfem_destroy",
+    "npfem_local_schedule_stats",
 )
 
 
@@ -90,6 +91,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.npfem_version.restype = C.c_char_p
     lib.npfem_destroy.argtypes = [vp]
     lib.npfem_destroy.restype = None
+    lib.npfem_local_schedule_stats.argtypes = [C.POINTER(_CellType), C.c_double, C.POINTER(C.c_double), i32]
+    lib.npfem_local_schedule_stats.restype = C.c_int
     _LIB = lib
     return lib
 
@@ -97,6 +100,26 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
 def _material_struct(m) -> _Material:
     return _Material(m.skalak_B, m.skalak_C, m.skalak_D, m.k_bending, m.k_volume, m.rayleigh_alpha,
                      m.rayleigh_beta, m.kappa_damping, m.density)
+
+
+SCHEDULE_STAT_NAMES = ("valid", "threads", "triangles_per_thread", "wavefronts_vertex_gather",
+                       "wavefronts_normal_gather", "worst_corner_store", "worst_corner_gather", "tables_consistent",
+                       "smem_bytes", "build_ms")
+
+
+def local_schedule_stats(cell_type, dt: float) -> dict:
+    """npfem_local_schedule_stats (host-only, no GPU needed): the create-time shared-memory schedule
+    of the scheduled fp32 local step for one cell type, checked by the library itself."""
+    lib = load_library()
+    rest = np.ascontiguousarray(cell_type.rest_positions, dtype=np.float64)
+    tri = np.ascontiguousarray(cell_type.triangles, dtype=np.int32)
+    ct = _CellType(rest.shape[0], tri.shape[0], rest.ctypes.data_as(C.POINTER(C.c_double)),
+                   tri.ctypes.data_as(C.POINTER(C.c_int32)), _material_struct(cell_type.material))
+    out = (C.c_double * len(SCHEDULE_STAT_NAMES))()
+    rc = lib.npfem_local_schedule_stats(C.byref(ct), float(dt), out, len(SCHEDULE_STAT_NAMES))
+    if rc != 0:
+        raise NpfemError(rc, lib.npfem_last_error(None).decode())
+    return dict(zip(SCHEDULE_STAT_NAMES, [float(v) for v in out]))
 
 
 class Solver:

@@ -2,6 +2,7 @@
 // Every arithmetic step of the path runs in the CUDA kernels of this directory; there is no
 // CPU fallback.
 #include <algorithm>
+#include <chrono>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -734,6 +735,102 @@ int npfem_get_objective(npfem_ctx *c, double *history, int32_t max_entries, int3
       NPFEM_CUDA(c, cudaMemcpyAsync(monotone, flags, size_t(c->n_cells) * sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
   }
   if (where == NPFEM_HOST) NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  return NPFEM_OK;
+}
+
+int npfem_local_schedule_stats(const npfem_cell_type *type, double dt, double *stats, int32_t n_stats) {
+  if (!type || !stats || n_stats < 10 || !(dt > 0)) return fail(nullptr, NPFEM_EINVAL, "type/stats missing, n_stats < 10 or dt <= 0");
+  std::fill(stats, stats + n_stats, 0.0);
+  HostTypeData h;
+  std::string err;
+  const int rc = build_host_type(*type, dt, h, err);
+  if (rc != NPFEM_OK) return fail(nullptr, rc, err);
+  LocalSchedule sc;
+  const auto t0 = std::chrono::steady_clock::now();
+  if (!build_local_schedule(h, type->rest_positions, h.T <= 320 ? 1 : 2, sc)) return NPFEM_OK;
+  stats[9] = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  stats[0] = 1;
+  stats[1] = sc.threads;
+  stats[2] = sc.tpt;
+  stats[3] = sc.wf_vertex;
+  stats[4] = sc.wf_normal;
+  stats[8] = double(sc.n_vslots + sc.n_tslots + sc.n_cslots) * 16.0;
+  // ---- decode the tables and check them against the mesh ------------------------------------
+  auto lo = [](uint32_t w) { return int(w & 0xffffu) / 16; };
+  auto hi = [](uint32_t w) { return int(w >> 16) / 16; };
+  bool ok = true;
+  std::vector<int> vslot(size_t(h.n)), tslot(size_t(h.T)), seen_v(size_t(sc.n_vslots), 0), seen_t(size_t(sc.n_tslots), 0),
+      seen_c(size_t(sc.n_cslots), 0);
+  for (int v = 0; v < h.n; ++v) {
+    vslot[v] = lo(sc.vtx_words[v]);
+    ok &= vslot[v] < sc.n_vslots && !seen_v[vslot[v]]++;
+  }
+  auto W = [&](int t, int q) { return sc.tri_words[(size_t(t / sc.ttri) * 5 + q) * sc.threads + t % sc.ttri]; };
+  for (int t = 0; t < h.T; ++t) {
+    tslot[t] = hi(W(t, 4));
+    ok &= tslot[t] < sc.n_tslots && !seen_t[tslot[t]]++;
+  }
+  std::vector<std::vector<int>> corner_slots(size_t(h.n));     // per vertex: slots its triangles write
+  double worst_store = 0, worst_gather = 0;
+  for (int t = 0; t < h.T; ++t) {
+    const int vs[3] = {lo(W(t, 0)), hi(W(t, 0)), lo(W(t, 1))}, ns[3] = {hi(W(t, 1)), lo(W(t, 2)), hi(W(t, 2))};
+    const int cs[3] = {lo(W(t, 3)), hi(W(t, 3)), lo(W(t, 4))};
+    // the three decoded vertices must be a cyclic rotation of the triangle, neighbours rotate along
+    int r = -1;
+    for (int k = 0; k < 3; ++k)
+      if (vs[0] == vslot[h.tri[4 * t + k]]) r = k;
+    ok &= r >= 0;
+    for (int k = 0; k < 3 && r >= 0; ++k) {
+      ok &= vs[k] == vslot[h.tri[4 * t + (k + r) % 3]];
+      ok &= ns[k] == tslot[h.tri_nbr[4 * t + (k + r) % 3]];
+      ok &= cs[k] < sc.n_cslots - 8 && !seen_c[cs[k]]++;
+      if (cs[k] < sc.n_cslots) corner_slots[h.tri[4 * t + (k + r) % 3]].push_back(cs[k]);
+    }
+  }
+  // stores: quarter warps of 8 consecutive triangle threads, per pass and corner
+  for (int t0q = 0; t0q < sc.tpt * sc.ttri; t0q += 8)
+    for (int k = 0; k < 3; ++k) {
+      int mult[8] = {0, 0, 0, 0, 0, 0, 0, 0}, w = 0;
+      for (int t = t0q; t < std::min(t0q + 8, h.T); ++t) {
+        const int slot = k == 0 ? lo(W(t, 3)) : (k == 1 ? hi(W(t, 3)) : lo(W(t, 4)));
+        w = std::max(w, ++mult[slot % 8]);
+      }
+      worst_store = std::max(worst_store, double(w));
+    }
+  // gathers: quarter warps of 8 consecutive vertices, per read position; every vertex must read
+  // exactly its own corner slots (in any order) and zero slots otherwise
+  const int vwords = 1 + sc.maxv / 2;
+  for (int v0 = 0; v0 < h.n; v0 += 8)
+    for (int k = 0; k < sc.maxv; ++k) {
+      std::vector<int> slots;
+      for (int v = v0; v < std::min(v0 + 8, h.n); ++v) {
+        const uint32_t w = sc.vtx_words[size_t(1 + k / 2) * sc.vstride + v];
+        slots.push_back((k & 1) ? hi(w) : lo(w));
+      }
+      int mult[8] = {0, 0, 0, 0, 0, 0, 0, 0}, w = 0;
+      for (size_t i = 0; i < slots.size(); ++i) {
+        bool dup = false;
+        for (size_t j = 0; j < i; ++j) dup |= slots[j] == slots[i];
+        if (!dup) w = std::max(w, ++mult[slots[i] % 8]);
+      }
+      worst_gather = std::max(worst_gather, double(w));
+    }
+  for (int v = 0; v < h.n; ++v) {
+    std::vector<int> reads;
+    for (int k = 0; k < sc.maxv; ++k) {
+      const uint32_t w = sc.vtx_words[size_t(1 + k / 2) * sc.vstride + v];
+      const int slot = (k & 1) ? hi(w) : lo(w);
+      if (slot < sc.n_cslots - 8) reads.push_back(slot);
+      else ok &= slot < sc.n_cslots;
+    }
+    std::sort(reads.begin(), reads.end());
+    std::sort(corner_slots[v].begin(), corner_slots[v].end());
+    ok &= reads == corner_slots[v];
+  }
+  (void)vwords;
+  stats[5] = worst_store;
+  stats[6] = worst_gather;
+  stats[7] = ok ? 1 : 0;
   return NPFEM_OK;
 }
 

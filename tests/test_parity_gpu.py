@@ -193,3 +193,27 @@ def test_fp32_local_step_implementations(impl, update_mode):
         print(impl, r)
         assert r["pos"] <= TOL_POS["fp32"] and r["worst_cell_pos"] <= TOL_POS["fp32"], r
         assert r["disp"] <= TOL_DISP["fp32"] and r["vel"] <= TOL_DISP["fp32"], r
+
+
+@pytest.mark.parametrize("precision,impl", [("fp64", 0), ("fp32", 1), ("fp32", 3)])
+def test_irregular_mesh_valence_up_to_8(precision, impl):
+    """A mesh that is not an icosphere (flipped edges, valences 4..8): generic kernels and the
+    8-read variant of the scheduled kernel against the oracle."""
+    from paper_1911_03062_b200 import binding
+    from workloads.meshes import irregular_cell_type
+    ct = irregular_cell_type(2, 40, seed=3)
+    val = np.bincount(ct.triangles.ravel())
+    assert val.max() > 6
+    rng = np.random.default_rng(11)
+    n_cells = 37
+    pos = ct.rest_positions[None] + rng.uniform(0, 80, (n_cells, 1, 3))
+    pop = Population(name="irr", types=[ct], type_of_cell=np.zeros(n_cells, np.int32), positions=[pos],
+                     velocities=[0.01 * rng.standard_normal(pos.shape)], dt=0.1, n_steps=3, n_iterations=6,
+                     box=(80.0,) * 3, force_sigma=1.0, shear_gamma=0.0, redraw_noise_each_step=False,
+                     _force_seed=np.random.SeedSequence(12), _shear_height=[pos[..., 2]])
+    gpu, solver = run_gpu(pop, precision, options=[(binding.OPT_LOCAL_STEP_IMPL, impl)])
+    solver.close()
+    ref = run_oracle(pop)
+    for r in compare(pop, gpu, ref):
+        print(precision, impl, r)
+        assert r["pos"] <= TOL_POS[precision] and r["disp"] <= TOL_DISP[precision] and r["vel"] <= TOL_DISP[precision], r

@@ -177,3 +177,40 @@ def icosahedron_cell_type(circumradius: float = 3.0, material: Material | None =
         triangles=np.ascontiguousarray(f),
         material=material or rbc_material(),
     )
+
+
+def irregular_cell_type(level: int = 2, n_flips: int = 40, seed: int = 3, material: Material | None = None) -> CellType:
+    """A closed mesh that is NOT an icosphere: interior edges of the platelet icosphere are flipped at
+    random (valences spread over 4..8), so code that silently relies on valence <= 6 or on the
+    subdivision ordering fails on it.  Edge-case input for the parity tests."""
+    base = platelet_cell_type(level, material)
+    rng = np.random.default_rng(seed)
+    tri = [tuple(int(v) for v in t) for t in base.triangles]
+    attempts = 0
+    while n_flips > 0 and attempts < 100000:
+        attempts += 1
+        t = int(rng.integers(len(tri)))
+        a, b, c = tri[t]
+        other = next((i for i, u in enumerate(tri) if i != t and a in u and b in u), None)
+        if other is None:
+            continue
+        d = next(v for v in tri[other] if v not in (a, b))
+        val = np.bincount(np.array(tri).ravel(), minlength=base.n_vertices)
+        if val[a] <= 4 or val[b] <= 4 or val[c] >= 8 or val[d] >= 8:
+            continue
+        if any(c in u and d in u for u in tri):
+            continue
+        # the flipped pair must stay convex enough to keep positive areas and outward orientation
+        p = base.rest_positions
+        n1 = np.cross(p[d] - p[a], p[c] - p[a])
+        n2 = np.cross(p[b] - p[d], p[c] - p[d])
+        if np.dot(n1, p[a] + p[d] + p[c]) <= 0 or np.dot(n2, p[d] + p[b] + p[c]) <= 0:
+            continue
+        if min(np.linalg.norm(n1), np.linalg.norm(n2)) < 0.2 * max(np.linalg.norm(n1), np.linalg.norm(n2)):
+            continue
+        if np.dot(n1, n2) < 0.9 * np.linalg.norm(n1) * np.linalg.norm(n2):      # keep the surface smooth
+            continue
+        tri[t], tri[other] = (a, d, c), (d, b, c)
+        n_flips -= 1
+    return CellType(name=f"IRR-{base.n_vertices}", rest_positions=base.rest_positions,
+                    triangles=np.array(tri, dtype=np.int32), material=base.material)
