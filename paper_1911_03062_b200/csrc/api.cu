@@ -314,6 +314,7 @@ int ensure_ready(npfem_ctx *c) {
       sd.valid = true;
       sd.threads = sc.threads; sd.vstride = sc.vstride; sd.tpt = sc.tpt; sd.ttri = sc.ttri; sd.maxv = sc.maxv;
       sd.n_vslots = sc.n_vslots; sd.n_tslots = sc.n_tslots; sd.n_cslots = sc.n_cslots;
+      sd.vol_lane_bound = sc.vol_lane_bound;
       sd.tri_words = reinterpret_cast<const uint32_t *>(c->ws + L.type_off[14][t]);
       sd.tri_consts = reinterpret_cast<const float *>(c->ws + L.type_off[15][t]);
       sd.vtx_words = reinterpret_cast<const uint32_t *>(c->ws + L.type_off[16][t]);

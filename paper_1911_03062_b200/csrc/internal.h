@@ -23,6 +23,7 @@ struct SchedDev {
   const float *tri_consts = nullptr;
   const uint32_t *vtx_words = nullptr;
   const float *vtx_coef = nullptr;
+  double vol_lane_bound = 0;   // max over threads of sum_j |x0| 2A_t of the rest shape (6V partial per lane)
 };
 
 // Device view of one cell type (pointers into the workspace; element type = compute type).

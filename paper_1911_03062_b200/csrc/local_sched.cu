@@ -39,8 +39,9 @@ struct SchedParams {
   const float *tri_consts;     // [TPT][12][threads]
   const uint32_t *vtx_words;   // [1 + MAXV/2][vstride]
   const float *vtx_coef;       // [vstride]
-  double fx_scale, fx_inv;     // fixed-point scale of the 6 V accumulator and its inverse
-  double V0x6, kv_coef;        // 6 V0;  k_v / (36 V0):  vc = kv_coef (6V - 6V0) = k_v (V - V0)/V0 / 6
+  float fx_scale;              // per-lane 6V partials are reduced as integers in units of 1 / fx_scale
+  long long fx_rest;           // round(6 V0 fx_scale)
+  float vc_scale;              // k_v / (36 V0) / fx_scale:  vc = vc_scale (6V - 6V0)_fixed = k_v (V - V0)/V0 / 6
   const float *x, *b, *u;      // [cells][3][n_pad]
   float *d;                    // read; written back when apply_u
   float *g;
@@ -82,7 +83,7 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
   unsigned char *sN = sx + p.sx_bytes;
   unsigned char *sC = sN + p.sN_bytes;
   float *stage = reinterpret_cast<float *>(sC + p.sC_bytes);            // [NSTAGE][4 fields x, d, b, u][3][n_pad]
-  int *vacc = reinterpret_cast<int *>(stage + NSTAGE * 12 * n_pad);   // [2 cells][hi, lo] base-2^24 digits of 6V
+  int *vacc = reinterpret_cast<int *>(stage + NSTAGE * 12 * n_pad);   // [2 cells][hi, lo] base-2^12 digits of 6V (fixed point)
   uint64_t *mbar = reinterpret_cast<uint64_t *>(vacc + 4);   // [NSTAGE] TMA ring
   uint64_t *bars = mbar + NSTAGE;                              // [4] split block barriers B1, B2, B3, BV
 
@@ -230,12 +231,16 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
     bar_arrive(1);                                     // B2: this warp's normals are stored
     // the volume has its own barrier (BV), awaited only where the volume coefficient is used, so the
     // shuffle chain and the atomics stay off the critical path of B2
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) vol += __shfl_xor_sync(0xffffffffu, vol, o);
-    if (lane == 0) {   // exact, order-independent: fixed point, split into a signed high and a 24-bit low digit
-      const long long v = __double2ll_rn(double(vol) * p.fx_scale);
-      atomicAdd(vacc + 2 * (it & 1), int(v >> 24));
-      atomicAdd(vacc + 2 * (it & 1) + 1, int(v & 0xffffff));
+    // fixed point from here on: one REDUX instead of a shuffle tree, integer shared atomics, and the
+    // result is exact, order independent and deterministic.  fx_scale leaves a factor 16 of headroom
+    // over the largest per-lane partial of the rest shape; the rounding (<= 0.5 / fx_scale per lane)
+    // is of the size of the fp32 rounding of the partial itself.
+    {
+      const int wsum = __reduce_add_sync(0xffffffffu, __float2int_rn(vol * p.fx_scale));
+      if (lane == 0) {
+        atomicAdd(vacc + 2 * (it & 1), wsum >> 12);          // signed high digit
+        atomicAdd(vacc + 2 * (it & 1) + 1, wsum & 0xfff);    // 12-bit low digit
+      }
     }
     bar_arrive(3);
     // membrane part of phase B needs this thread's registers only: it overlaps the wait for B2
@@ -311,7 +316,7 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
     }
     bar_wait(3, par);                                  // BV: volume accumulated
     const int2 vd = *reinterpret_cast<const int2 *>(vacc + 2 * (it & 1));
-    const float vc = float(((double(vd.x) * 16777216.0 + double(vd.y)) * p.fx_inv - p.V0x6) * p.kv_coef);
+    const float vc = p.vc_scale * float(int((static_cast<long long>(vd.x) << 12) + vd.y - p.fx_rest));
     float cf[TPT][9];
 #pragma unroll
     for (int j = 0; j < TPT; ++j) {
@@ -417,13 +422,14 @@ int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, bool a
   p.n = td.n; p.T = td.T; p.n_pad = td.n_pad; p.ttri = s.ttri; p.threads = s.threads; p.vstride = s.vstride;
   p.sx_bytes = s.n_vslots * 16; p.sN_bytes = s.n_tslots * 16; p.sC_bytes = s.n_cslots * 16;
   p.tri_words = s.tri_words; p.tri_consts = s.tri_consts; p.vtx_words = s.vtx_words; p.vtx_coef = s.vtx_coef;
-  // 6V accumulates in fixed point (two 32-bit digits, base 2^24) with room for 64 x the rest volume
+  // 6V is reduced in fixed point: 32 lane partials must fit an int32 REDUX with 16 x headroom over the
+  // largest per-lane partial of the rest shape (s.vol_lane_bound, create time)
   int k = 0;
-  std::frexp(384.0 * td.V0, &k);                    // 384 V0 < 2^k
-  p.fx_scale = std::ldexp(1.0, 52 - k);
-  p.fx_inv = std::ldexp(1.0, k - 52);
-  p.V0x6 = 6.0 * td.V0;
-  p.kv_coef = td.kv_over_V0 / 36.0;
+  std::frexp(16.0 * 32.0 * s.vol_lane_bound, &k);   // 512 bound < 2^k
+  const double scale = std::ldexp(1.0, 31 - k);
+  p.fx_scale = float(scale);
+  p.fx_rest = std::llrint(6.0 * td.V0 * scale);
+  p.vc_scale = float(td.kv_over_V0 / 36.0 / scale);
   p.x = static_cast<const float *>(bv.field[F_X]);
   p.d = static_cast<float *>(bv.field[F_D]);
   p.u = static_cast<const float *>(bv.field[F_U]);

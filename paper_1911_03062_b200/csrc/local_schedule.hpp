@@ -42,6 +42,7 @@ struct LocalSchedule {
   std::vector<uint32_t> vtx_words;   // [1 + maxv/2][vstride] own slot, corner-force slots
   std::vector<float> vtx_coef;       // [vstride]
   double wf_vertex = 0, wf_normal = 0;   // predicted wavefronts per gather instruction (ideal 4)
+  double vol_lane_bound = 0;             // max over threads of sum_j |x_0 - centroid| 2 A_t (rest shape)
 };
 
 namespace sched_detail {
@@ -322,6 +323,23 @@ inline bool build_local_schedule(const HostTypeData &h, const double *X, int tpt
       K(6 + s) = float(m.k_bending * h.hinge_rest[6 * t + 2 * so + 0]);
       K(9 + s) = float(m.k_bending * h.hinge_rest[6 * t + 2 * so + 1]);
     }
+  }
+  {   // bound of a thread's partial of 6V = sum_t x_0 . (e_1 x e_2) in cell-local (centroid) coordinates
+    double cen[3] = {0, 0, 0}, rmax = 0, bound = 0;
+    for (int v = 0; v < n; ++v)
+      for (int q = 0; q < 3; ++q) cen[q] += X[3 * v + q] / n;
+    for (int v = 0; v < n; ++v) {
+      double r2 = 0;
+      for (int q = 0; q < 3; ++q) r2 += (X[3 * v + q] - cen[q]) * (X[3 * v + q] - cen[q]);
+      rmax = std::max(rmax, std::sqrt(r2));
+    }
+    for (int tid = 0; tid < ttri; ++tid) {
+      double sum = 0;
+      for (int j = 0; j < tpt; ++j)
+        if (j * ttri + tid < T) sum += rmax * 2.0 * h.tri_rest[4 * (j * ttri + tid) + 3];
+      bound = std::max(bound, sum);
+    }
+    out.vol_lane_bound = bound;
   }
   // vertex reads: real corner slots, then zero slots of a bank group the read group does not use
   std::vector<std::array<int, 8>> reads(static_cast<size_t>(n));
