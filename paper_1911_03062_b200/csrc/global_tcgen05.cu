@@ -25,15 +25,14 @@ namespace {
 constexpr int BM = 128;          // rows per tile (TMEM lanes)
 constexpr int BK = 32;           // fp32 per K chunk = 128 bytes = one swizzle row
 constexpr int UMMA_K = 8;        // K per tcgen05.mma for tf32 (32 bytes)
-constexpr int STAGES = 3;
+constexpr int MAX_STAGES = 4;      // ring depth is chosen per launch: as many stages as fit next to the epilogue tiles
 constexpr int CL = 2;             // thread-block cluster: CL CTAs work on CL consecutive M tiles and share every W tile
 constexpr int MAX_NPASS = 256;   // accumulator columns per pass: two accumulators fit the 512 TMEM columns
 constexpr int A_BYTES = BM * BK * 4;
 constexpr int B_BYTES = MAX_NPASS * BK * 4;
-constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-constexpr int EBUF = 4;           // per epilogue warp: ring of [32 rows x 32 cols] fp32 staging tiles (4 KB each)
+constexpr int EBUF = 3;           // per epilogue warp: ring of [32 rows x 32 cols] fp32 staging tiles (4 KB each)
 constexpr int EPI_BYTES = 4 * EBUF * 4096;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + EPI_BYTES + 1024;
+constexpr int SMEM_LIMIT = 227 * 1024;
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return uint32_t(__cvta_generic_to_shared(p)); }
 
@@ -133,6 +132,8 @@ struct GemmParams {
   int k_chunks;        // ceil(n_pad / BK)
   int64_t m_tiles;
   float d_scale;       // d <- d_scale * d + acc
+  int stages;          // depth of the operand ring (<= MAX_STAGES)
+  int stage_bytes;     // A tile + W tile of n_pass rows, multiple of 1024
 };
 
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
@@ -147,7 +148,7 @@ __global__ void __launch_bounds__(192, 1)
 global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_constant__ CUtensorMap map_w,
                       const __grid_constant__ CUtensorMap map_d, const GemmParams p) {
   extern __shared__ unsigned char smem_raw[];
-  __shared__ uint64_t full_bar[STAGES], empty_bar[STAGES], tmem_full_bar[2], tmem_empty_bar[2], epi_full[4 * EBUF];
+  __shared__ uint64_t full_bar[MAX_STAGES], empty_bar[MAX_STAGES], tmem_full_bar[2], tmem_empty_bar[2], epi_full[4 * EBUF];
   __shared__ uint32_t tmem_base_sh;
   unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -160,7 +161,7 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
   constexpr uint16_t MASK = uint16_t((1u << CL) - 1u);
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < STAGES; ++s) {
+    for (int s = 0; s < p.stages; ++s) {
       mbar_init(&full_bar[s], 1);
       mbar_init(&empty_bar[s], CL);                         // every CTA of the cluster reads what lands here
     }
@@ -192,12 +193,12 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
         const int row0 = int(((item / p.passes) * CL + rank) * BM), col0 = int(item % p.passes) * p.n_pass;
         for (int kc = 0; kc < p.k_chunks; ++kc) {
           mbar_wait(&empty_bar[stage], phase ^ 1);          // this slot is free in EVERY CTA of the cluster
-          unsigned char *sa = smem + stage * STAGE_BYTES, *sb = sa + A_BYTES;
+          unsigned char *sa = smem + stage * p.stage_bytes, *sb = sa + A_BYTES;
           mbar_expect_tx(&full_bar[stage], tx);             // own G tile + all CL slices of the W tile
           tma_load_2d(sa, &map_g, kc * BK, row0, &full_bar[stage]);
           tma_load_2d_mc(sb + size_t(rank) * w_rows * BK * 4, &map_w, kc * BK, col0 + int(rank) * w_rows,
                          &full_bar[stage], MASK);
-          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          if (++stage == p.stages) { stage = 0; phase ^= 1; }
         }
       }
     }
@@ -215,13 +216,13 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
         for (int kc = 0; kc < p.k_chunks; ++kc) {
           mbar_wait(&full_bar[stage], phase);
           asm volatile("tcgen05.fence::after_thread_sync;");
-          const uint32_t sa = smem_u32(smem + stage * STAGE_BYTES), sb = sa + A_BYTES;
+          const uint32_t sa = smem_u32(smem + stage * p.stage_bytes), sb = sa + A_BYTES;
 #pragma unroll
           for (int k = 0; k < BK / UMMA_K; ++k)
             umma_tf32(tacc, make_smem_desc(sa + k * UMMA_K * 4), make_smem_desc(sb + k * UMMA_K * 4), idesc,
                       (kc | k) != 0);
           umma_commit_mc(&empty_bar[stage], MASK);          // frees the slot in every CTA when these MMAs retire
-          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          if (++stage == p.stages) { stage = 0; phase ^= 1; }
         }
         umma_commit(&tmem_full_bar[acc]);                   // accumulator complete
       }
@@ -234,7 +235,7 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
     // full 128-byte rows moved by the TMA unit; a row-per-lane LDG/STG pattern (32 lines per warp
     // instruction) held the previous version to a third of the tensor peak.
     const int lane_base = (warp & 3) * 32;
-    unsigned char *ebuf = smem + STAGES * STAGE_BYTES + (warp & 3) * (EBUF * 4096);
+    unsigned char *ebuf = smem + p.stages * p.stage_bytes + (warp & 3) * (EBUF * 4096);
     uint64_t *efull = &epi_full[(warp & 3) * EBUF];
     const bool rmw = p.U == nullptr;
     const int n_chunks = (p.n_pass + 31) / 32;
@@ -251,15 +252,12 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
         mbar_expect_tx(&efull[b], 4096);
         tma_load_2d(ebuf + b * 4096, &map_d, col0 + 32 * c, row0w, &efull[b]);
       };
-      if (rmw && lane == 0) {                               // requested before the accumulator is awaited
-        issue_load(0, g);
-        if (n_chunks > 1) issue_load(1, g + 1);
-      }
+      if (rmw && lane == 0) issue_load(0, g);               // requested before the accumulator is awaited
       mbar_wait(&tmem_full_bar[acc], acc_phase);
       asm volatile("tcgen05.fence::after_thread_sync;");
       for (int c = 0; c < n_chunks; ++c) {
         const uint32_t gc = g + uint32_t(c), b = gc % EBUF;
-        if (rmw && lane == 0 && c + 2 < n_chunks) issue_load(c + 2, gc + 2);
+        if (rmw && lane == 0 && c + 1 < n_chunks) issue_load(c + 1, gc + 1);   // tile gc-2's store may still run
         uint32_t r[32];
         {
           uint32_t r0[16], r1[16];
@@ -272,7 +270,7 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
         if (rmw) {
           mbar_wait(&efull[b], (gc / EBUF) & 1u);
         } else {
-          if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 3;" ::: "memory");
+          if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 2;" ::: "memory");
           __syncwarp();
         }
         float4 *rowp = reinterpret_cast<float4 *>(ebuf + b * 4096 + lane * 128);
@@ -372,11 +370,16 @@ int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, dou
   // epilogue tiles: [32 rows][32 columns] of D (in-place update) or of U (product out)
   if (!make_map(&map_d, u_out ? u_out : bv.field[F_D], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), 32))
     return -1;
-  static bool attr = false;
-  if (!attr) {
-    if (cudaFuncSetAttribute(global_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES) != cudaSuccess)
+  p.stage_bytes = A_BYTES + (p.n_pass * BK * 4 + 1023) / 1024 * 1024;
+  p.stages = (SMEM_LIMIT - 1024 - EPI_BYTES) / p.stage_bytes;
+  if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;
+  if (p.stages < 2) return -1;
+  const int smem_bytes = p.stages * p.stage_bytes + EPI_BYTES + 1024;
+  static int smem_set = 0;
+  if (smem_bytes > smem_set) {
+    if (cudaFuncSetAttribute(global_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes) != cudaSuccess)
       return -1;
-    attr = true;
+    smem_set = smem_bytes;
   }
   // the passes of one group of M tiles are adjacent items: they run on neighbouring clusters at about
   // the same time, so the repeated reads of the G tiles are L2 hits
@@ -385,7 +388,7 @@ int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, dou
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(unsigned(clusters * CL));
   cfg.blockDim = dim3(192);
-  cfg.dynamicSmemBytes = SMEM_BYTES;
+  cfg.dynamicSmemBytes = size_t(smem_bytes);
   cfg.stream = s;
   cudaLaunchAttribute attrs[1];
   attrs[0].id = cudaLaunchAttributeClusterDimension;
