@@ -49,6 +49,14 @@ def parse_args():
     return ap.parse_args()
 
 
+def load_ncu_capture():
+    """Per-launch DRAM bytes and warp instructions of the two hot kernels from the committed ncu
+    `--set full` capture (profiles/r1_ncu_capture.json, written by hand from the .ncu-rep: bench.py
+    cannot run ncu).  Only valid for the workload it was captured on."""
+    path = os.path.join(ROOT, "profiles", "r1_ncu_capture.json")
+    return json.load(open(path)) if os.path.exists(path) else {}
+
+
 def load_peaks():
     """Measured roofline denominators (driver-written), else the profiling guide's fallback."""
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -56,7 +64,7 @@ def load_peaks():
         p = json.load(open(path))
         return {"hbm_gbs": float(p["hbm_gbs"]), "bf16_tflops": float(p["bf16_tflops"]),
                 "bf16_tflops_sustained": float(p.get("bf16_tflops_sustained", p["bf16_tflops"])),
-                "source": "measured"}
+                "sm_max_mhz": float(p.get("sm_max_mhz", 1965.0)), "source": "measured"}
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
 
 
@@ -259,10 +267,26 @@ def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: 
             kernels.append(row)
     dominant = max(kernels, key=lambda r: r["share_of_kernel_time"]) if kernels else None
     roofline = None
+    capture = load_ncu_capture()
+    same_workload = capture.get("cells") == pop.n_cells and capture.get("precision") == args.precision
     if dominant:
+        cap = capture.get("kernels", {}).get(dominant["kernel"]) if same_workload else None
         roofline = {"kernel": dominant["kernel"], "bound": "hbm", "achieved": dominant["hbm_gbs"],
-                    "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": dominant["hbm_frac"], "traffic": None,
-                    "peak_source": peaks["source"] + " (MEASURED_PEAKS.json hbm_gbs)"}
+                    "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": dominant["hbm_frac"],
+                    "traffic": cap["dram_bytes"] if cap else None,
+                    "peak_source": peaks["source"] + " (MEASURED_PEAKS.json hbm_gbs)",
+                    "note": "north_star names HBM for the local step; the kernel is bound by instruction issue and "
+                            "shared-memory wavefronts (DESIGN.md 7.1), see `alu`"}
+        if cap and cap.get("warp_instructions"):
+            # plain-ALU roofline: 148 SMs x 4 schedulers x 1 warp instruction / cycle at the max SM clock
+            sm_mhz = peaks.get("sm_max_mhz", 1965.0)
+            alu_peak = 148 * 4 * sm_mhz * 1e6
+            ach = cap["warp_instructions"] / (dominant["avg_ms"] * 1e-3)
+            roofline["alu"] = {"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "warp-instructions/s",
+                               "frac": ach / alu_peak, "smem_wavefronts_per_launch": cap.get("smem_wavefronts")}
+    for row in kernels:
+        cap = capture.get("kernels", {}).get(row["kernel"]) if same_workload else None
+        row["traffic"] = cap["dram_bytes"] if cap else None
 
     result = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
