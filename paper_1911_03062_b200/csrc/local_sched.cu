@@ -75,10 +75,12 @@ __device__ __forceinline__ void sts4(unsigned char *base, uint32_t off, float x,
   *reinterpret_cast<float4 *>(base + off) = make_float4(x, y, z, w);
 }
 
-template <int TPT, int MAXV, int MAXT, int MINB>
+// NPAD: compile-time row pitch of the state fields (0 = run-time p.n_pad): with it every access to the
+// staging ring is base register + immediate instead of a per-access address computation
+template <int TPT, int MAXV, int MAXT, int MINB, int NPAD>
 __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedParams p) {
   extern __shared__ __align__(16) unsigned char smem[];
-  const int n = p.n, n_pad = p.n_pad, nthreads = p.threads;
+  const int n = p.n, n_pad = NPAD ? NPAD : p.n_pad, nthreads = p.threads;
   unsigned char *sx = smem;
   unsigned char *sN = sx + p.sx_bytes;
   unsigned char *sC = sN + p.sN_bytes;
@@ -384,9 +386,9 @@ size_t sched_smem_bytes(const SchedDev &s, int n_pad) {
   return size_t(s.n_vslots + s.n_tslots + s.n_cslots) * 16 + size_t(NSTAGE) * 12 * n_pad * 4 + 4 * 4 + (NSTAGE + 4) * 8;
 }
 
-template <int TPT, int MAXV, int MAXT, int MINB>
+template <int TPT, int MAXV, int MAXT, int MINB, int NPAD>
 int launch_variant(const SchedParams &p, size_t smem, int n_sm, int64_t cells, cudaStream_t s) {
-  auto kernel = local_sched_kernel<TPT, MAXV, MAXT, MINB>;
+  auto kernel = local_sched_kernel<TPT, MAXV, MAXT, MINB, NPAD>;
   static int per_sm = 0;          // per template instance; the smem size of a type never changes
   static size_t smem_set = 0;
   if (smem > smem_set) {
@@ -439,12 +441,15 @@ int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, bool a
   p.g = static_cast<float *>(bv.field[F_G]);
   p.cells = bv.cells;
   const size_t smem = sched_smem_bytes(s, td.n_pad);
+  // the BASELINE cell types get their row pitch at compile time, everything else the generic variants
   if (s.tpt == 2) {
-    if (s.maxv == 6) return launch_variant<2, 6, 640, 1>(p, smem, n_sm, bv.cells, stream);
-    return launch_variant<2, 8, 640, 1>(p, smem, n_sm, bv.cells, stream);
+    if (s.maxv == 6 && td.n_pad == 656) return launch_variant<2, 6, 640, 1, 656>(p, smem, n_sm, bv.cells, stream);
+    if (s.maxv == 6) return launch_variant<2, 6, 640, 1, 0>(p, smem, n_sm, bv.cells, stream);
+    return launch_variant<2, 8, 640, 1, 0>(p, smem, n_sm, bv.cells, stream);
   }
-  if (s.maxv == 6) return launch_variant<1, 6, 320, 2>(p, smem, n_sm, bv.cells, stream);
-  return launch_variant<1, 8, 320, 2>(p, smem, n_sm, bv.cells, stream);
+  if (s.maxv == 6 && td.n_pad == 176) return launch_variant<1, 6, 320, 2, 176>(p, smem, n_sm, bv.cells, stream);
+  if (s.maxv == 6) return launch_variant<1, 6, 320, 2, 0>(p, smem, n_sm, bv.cells, stream);
+  return launch_variant<1, 8, 320, 2, 0>(p, smem, n_sm, bv.cells, stream);
 }
 
 }  // namespace npfem
