@@ -17,7 +17,8 @@ oracle is the algorithm step by step in the paper's order; the only library
 primitive used as a step is LAPACK's Cholesky factor/solve (scipy.linalg).
 
 Pins: tests/test_oracle_pins.py (P1-P13 of SURVEY.md section 8(c)).
-PARITY UNPINNED for: the unused Skalak constant D (R6), the platelet stiffness
+PARITY UNPINNED for: the line-search constants of `step_line_search` (Armijo c1, halving factor 1/2:
+conventional choices, the paper has no line search), the unused Skalak constant D (R6), the platelet stiffness
 factor (R13), and fidelity to the authors' actual npFEM energies - parity with
 the published npFEM is not claimed.
 
@@ -358,6 +359,54 @@ def step(x_n: np.ndarray, v_n: np.ndarray, f_ext: np.ndarray, td: TypeData,
         g = gradient_g(d, x_n, b, td)
         history["objective"].append(objective(d, x_n, b, td))
         history["grad_norm"].append(np.sqrt(np.sum(g * g, axis=(-2, -1))))
+    x_next = x_n + d
+    v_next = d / h
+    return (x_next, v_next, history) if record else (x_next, v_next)
+
+
+def step_line_search(x_n: np.ndarray, v_n: np.ndarray, f_ext: np.ndarray, td: TypeData, n_iterations: int,
+                     max_halvings: int = 8, c1: float = 1e-4, grad_tol: float = 0.0, record: bool = False):
+    """`step` with a per-cell Armijo backtracking line search and a gradient-norm stopping test
+    (the paper's text has neither - reading R2 - but claims "unconditional
+    stability for arbitrary time steps", which the plain iteration does not have).
+
+    Per cell and iteration k:  grad = grad g(d);  if ||grad||_2 <= grad_tol ||b||_2 the cell is
+    frozen (d unchanged).  Otherwise p = -H~^-1 grad, slope = <grad, p> (< 0 because H~ is SPD),
+    alpha = 1, and alpha is halved while  g(d + alpha p) > g(d) + c1 alpha slope,  at most
+    `max_halvings` times (the last alpha is taken even if the test still fails).  d <- d + alpha p.
+    Returns (x_next, v_next[, history]); history["alpha"] is [n_iterations] arrays of step lengths.
+    """
+    h = td.h
+    v = pbd_damping(x_n, v_n, td.mass, td.kappa)
+    b = td.mass[:, None] * v / h + f_ext
+    d = h * v
+    lead = d.shape[:-2]
+    b_norm = np.sqrt(np.sum(b * b, axis=(-2, -1)))
+    history = {"objective": [], "alpha": [], "grad_norm": []}
+    for _ in range(n_iterations):
+        grad = gradient_g(d, x_n, b, td)
+        g_norm = np.sqrt(np.sum(grad * grad, axis=(-2, -1)))
+        frozen = g_norm <= grad_tol * b_norm
+        p = -solve_H_tilde(grad, td)
+        slope = np.sum(grad * p, axis=(-2, -1))
+        g0 = objective(d, x_n, b, td)
+        alpha = np.ones(lead)
+        done = np.array(frozen, copy=True)
+        for halving in range(max_halvings + 1):
+            trial = objective(d + alpha[..., None, None] * p, x_n, b, td)
+            ok = trial <= g0 + c1 * alpha * slope
+            done = done | ok
+            if halving == max_halvings or np.all(done):
+                break
+            alpha = np.where(done, alpha, 0.5 * alpha)
+        alpha = np.where(frozen, 0.0, alpha)
+        d = d + alpha[..., None, None] * p
+        if record:
+            history["objective"].append(g0)
+            history["alpha"].append(alpha)
+            history["grad_norm"].append(g_norm)
+    if record:
+        history["objective"].append(objective(d, x_n, b, td))
     x_next = x_n + d
     v_next = d / h
     return (x_next, v_next, history) if record else (x_next, v_next)

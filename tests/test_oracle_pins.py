@@ -387,3 +387,67 @@ def test_mesh_counts():
         assert np.sum(valence == 5) == 12 and np.all((valence == 5) | (valence == 6))
         # outward orientation: positive enclosed volume
         assert orc.enclosed_volume(v, f.astype(np.int64)) > 0
+
+
+# ---- Armijo line search + gradient-norm stopping test (oracle.step_line_search) ----
+def _violent_case():
+    """RBC-162, h = 30 us, N(0, 3000 pN) forces: the plain iteration of Eq. (4) blows up (SURVEY.md
+    section 4: 'unconditional stability ... only holds with a line search')."""
+    import warnings
+    from workloads.meshes import rbc_cell_type
+    ct = rbc_cell_type(2)
+    td = orc.make_type(ct, 30.0)
+    rng = np.random.default_rng(0)
+    x = np.repeat(ct.rest_positions[None], 2, axis=0)
+    f = 3000.0 * rng.standard_normal(x.shape)
+    warnings.filterwarnings("ignore")
+    return td, x, np.zeros_like(x), f
+
+
+def test_ls_accepts_full_steps_where_the_plain_iteration_descends(rbc162):
+    ct, td = rbc162
+    rng = np.random.default_rng(3)
+    x = np.repeat(ct.rest_positions[None], 3, axis=0)
+    f = rng.standard_normal(x.shape)
+    xa, va = orc.step(x, 0 * x, f, td, 8)
+    xb, vb, hist = orc.step_line_search(x, 0 * x, f, td, 8, record=True)
+    assert all(np.all(a == 1.0) for a in hist["alpha"])
+    assert np.array_equal(xa, xb) and np.array_equal(va, vb)
+
+
+def test_ls_keeps_the_objective_monotone_where_the_plain_iteration_blows_up():
+    td, x, v, f = _violent_case()
+    try:
+        xa, _, hist_plain = orc.step(x, v, f, td, 15, record=True)
+        obj = np.array(hist_plain["objective"])
+        plain_ok = np.all(np.isfinite(xa)) and np.all(np.diff(obj, axis=0) <= 0)
+    except ValueError:                      # LAPACK refuses the NaNs of the diverged iterate
+        plain_ok = False
+    assert not plain_ok
+    xb, vb, hist = orc.step_line_search(x, v, f, td, 15, max_halvings=8, c1=1e-4, record=True)
+    obj = np.array(hist["objective"])       # [16, cells]
+    assert np.all(np.isfinite(xb)) and np.all(np.diff(obj, axis=0) <= 0)
+    alpha = np.array(hist["alpha"])
+    assert alpha.min() < 1.0                                          # the search really backtracked
+    assert np.all(np.isin(alpha, 0.5 ** np.arange(0, 9)))             # powers of 1/2 only
+    # Armijo at every accepted step that did not exhaust the halvings: g_new <= g_old + c1 alpha slope, slope < 0
+    assert np.all(obj[1:][alpha > 0.5 ** 8] < obj[:-1][alpha > 0.5 ** 8])
+
+
+def test_ls_gradient_tolerance_freezes_converged_cells(rbc162):
+    ct, td = rbc162
+    rng = np.random.default_rng(4)
+    x = np.repeat(ct.rest_positions[None], 2, axis=0)
+    v = 1e-3 * rng.standard_normal(x.shape)
+    f = rng.standard_normal(x.shape)
+    # huge tolerance: every cell is "converged" at once -> d stays at its start h v (damped)
+    xa, va, hist = orc.step_line_search(x, v, f, td, 5, grad_tol=1e9, record=True)
+    vd = orc.pbd_damping(x, v, td.mass, td.kappa)
+    assert np.all(np.array(hist["alpha"]) == 0.0)
+    assert np.allclose(xa, x + td.h * vd, rtol=0, atol=1e-15) and np.allclose(va, vd, rtol=0, atol=1e-15)
+    # tight tolerance: cells stop once the gradient is small, and the result equals the full run to that level
+    xb, _, hist_b = orc.step_line_search(x, v, f, td, 60, grad_tol=1e-6, record=True)
+    xc, _ = orc.step(x, v, f, td, 60)
+    alpha = np.array(hist_b["alpha"])
+    assert np.all(alpha[-1] == 0.0) and np.all(alpha[0] == 1.0)       # they did stop, after working
+    assert np.linalg.norm(xb - xc) <= 1e-5 * np.linalg.norm(xc - x)
