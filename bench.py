@@ -43,6 +43,7 @@ def parse_args():
     ap.add_argument("--update-mode", type=int, default=0, choices=[0, 1, 2],
                     help="0 auto, 1 GEMM epilogue updates d in place, 2 product-out applied by the next local step")
     ap.add_argument("--local-impl", type=int, default=0, choices=[0, 1, 2, 3])
+    ap.add_argument("--line-search", type=int, default=0, help="Armijo backtracking with this many halvings (0 = off)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -212,6 +213,8 @@ def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: 
     solver.set_option(binding.OPT_GLOBAL_STEP_MATH, 0 if args.global_math == "tf32" else 1)
     solver.set_option(binding.OPT_UPDATE_MODE, args.update_mode)
     solver.set_option(binding.OPT_LOCAL_STEP_IMPL, args.local_impl)
+    if args.line_search:
+        solver.set_line_search(args.line_search)
     solver.set_state(torch.from_numpy(pop.packed(pop.positions)).to(dev))
     forces_host = torch.from_numpy(pop.packed(pop.forces(0), dtype=np_io)).pin_memory()
     forces_dev = forces_host.to(dev)
@@ -370,6 +373,7 @@ def config_description(args, pop, n_cells: int, n_iterations: int) -> dict:
     return {"workload": f"BASELINE.json configs[{args.config - 1}]: {CONFIG_NAMES[args.config]}",
             "cells": int(n_cells), "cell_types_vertices": mix, "iterations_per_step": int(n_iterations),
             "dt_us": pop.dt, "precision": args.precision, "global_step_math": args.global_math,
+            "line_search_halvings": int(args.line_search),
             "l2": "no flush needed: the state touched per iteration (>= 2.9 GB at 100k cells) exceeds the 126 MB L2"}
 
 

@@ -76,7 +76,8 @@ extern "C" {
 #define NPFEM_KIND_LOCAL    1
 #define NPFEM_KIND_GLOBAL   2
 #define NPFEM_KIND_EPILOGUE 3
-#define NPFEM_KIND_COUNT    4
+#define NPFEM_KIND_LINE_SEARCH 4   /* objective evaluations + accept / backtrack kernels */
+#define NPFEM_KIND_COUNT    5
 
 #define NPFEM_MAX_ITERATIONS 256
 
@@ -163,6 +164,20 @@ int npfem_get_state(npfem_ctx *ctx, const int64_t *cell_ids, int64_t n_ids,
  */
 int npfem_get_objective(npfem_ctx *ctx, double *history, int32_t max_entries,
                         int32_t *n_entries, int32_t *monotone, int32_t where);
+
+/*
+ * Per-cell Armijo backtracking line search + gradient-norm stopping test for the following steps
+ * (the paper's text has none, reading R2, but claims unconditional stability,
+ * PAPER.md:37, :264).  max_halvings = 0 switches it off (default: plain Eq. (4), step length 1).
+ * Per cell and iteration: frozen if ||grad g||_2 <= grad_tol ||b||_2; otherwise alpha = 1 and alpha is
+ * halved while g(d + alpha p) > g(d) + armijo_c1 alpha <grad g, p>, at most max_halvings (<= 30) times,
+ * p = -H~^-1 grad g; d <- d + alpha p.  With it on, the local step runs the generic kernel (full
+ * gradient) and every iteration costs max_halvings + 2 extra objective evaluations.
+ */
+int npfem_set_line_search(npfem_ctx *ctx, int32_t max_halvings, double armijo_c1, double grad_tol);
+
+/* Step lengths alpha of the LAST iteration of the last step, HOST array [n_cells] in cell-id order. */
+int npfem_get_step_lengths(npfem_ctx *ctx, double *alpha);
 
 /*
  * Device time per kernel kind since the last reset (needs NPFEM_OPT_KERNEL_TIMING = 1): CUDA

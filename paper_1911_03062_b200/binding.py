@@ -14,14 +14,14 @@ import numpy as np
 NPFEM_F32, NPFEM_F64 = 32, 64
 NPFEM_DEVICE, NPFEM_HOST = 0, 1
 OPT_DIAGNOSTICS, OPT_GLOBAL_STEP_MATH, OPT_LOCAL_STEP_IMPL, OPT_KERNEL_TIMING, OPT_UPDATE_MODE = 1, 2, 3, 4, 5
-KIND_NAMES = ("prologue", "local", "global", "epilogue")
+KIND_NAMES = ("prologue", "local", "global", "epilogue", "line_search")
 _ERR_NAMES = {-1: "NPFEM_EINVAL", -2: "NPFEM_EMESH", -3: "NPFEM_ECUDA", -4: "NPFEM_ENOMEM", -5: "NPFEM_ESTATE"}
 
 EXPORTED_SYMBOLS = (
     "npfem_create", "npfem_workspace_bytes", "npfem_bind_workspace", "npfem_set_option",
     "npfem_set_state", "npfem_set_forces", "npfem_step", "npfem_get_state", "npfem_get_objective",
     "npfem_get_kernel_times", "npfem_launch_count", "npfem_last_error", "npfem_version", "npfem_destroy",
-    "npfem_local_schedule_stats",
+    "npfem_local_schedule_stats", "npfem_set_line_search", "npfem_get_step_lengths",
 )
 
 
@@ -91,6 +91,10 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.npfem_version.restype = C.c_char_p
     lib.npfem_destroy.argtypes = [vp]
     lib.npfem_destroy.restype = None
+    lib.npfem_set_line_search.argtypes = [vp, i32, C.c_double, C.c_double]
+    lib.npfem_set_line_search.restype = C.c_int
+    lib.npfem_get_step_lengths.argtypes = [vp, vp]
+    lib.npfem_get_step_lengths.restype = C.c_int
     lib.npfem_local_schedule_stats.argtypes = [C.POINTER(_CellType), C.c_double, C.POINTER(C.c_double), i32]
     lib.npfem_local_schedule_stats.restype = C.c_int
     _LIB = lib
@@ -251,6 +255,16 @@ class Solver:
         self._check(self._lib.npfem_get_objective(self._ctx, C.c_void_p(hist.ctypes.data), 257, C.byref(n_entries),
                                                   C.c_void_p(mono.ctypes.data), NPFEM_HOST))
         return hist[:n_entries.value, :self.n_cells].copy(), mono[:self.n_cells].copy()
+
+    def set_line_search(self, max_halvings: int, armijo_c1: float = 1e-4, grad_tol: float = 0.0) -> None:
+        """Armijo backtracking + gradient-norm stopping test for the following steps (0 = off)."""
+        self._check(self._lib.npfem_set_line_search(self._ctx, int(max_halvings), float(armijo_c1), float(grad_tol)))
+
+    def get_step_lengths(self) -> np.ndarray:
+        """alpha of the last iteration of the last step, [n_cells] in cell-id order."""
+        out = np.zeros(self.n_cells, dtype=np.float64)
+        self._check(self._lib.npfem_get_step_lengths(self._ctx, C.c_void_p(out.ctypes.data)))
+        return out
 
     def get_kernel_times(self, reset: bool = True):
         """{kind: [(ms, launches) per cell type]} accumulated since the last reset (OPT_KERNEL_TIMING)."""

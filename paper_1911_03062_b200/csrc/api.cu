@@ -44,6 +44,11 @@ struct npfem_ctx {
   double *history_dev = nullptr;
   int history_cap = 0, history_entries = 0;
   int64_t opt_global_math = 0, opt_local_impl = 0, opt_update_mode = 0;
+  // line search (npfem_set_line_search)
+  int ls_max_halvings = 0;
+  double ls_c1 = 1e-4, ls_tol = 0.0;
+  std::vector<LineSearchDev> ls;          // per bucket, allocated on first use
+  bool ls_ran = false;
   int64_t launches = 0;
   // kernel timing (NPFEM_OPT_KERNEL_TIMING)
   bool timing = false;
@@ -649,7 +654,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   auto diag = [&](int row) -> int {
     for (size_t t = 0; t < nb; ++t) {
       const int r = check_launch(c, launch_objective(c->types[t], c->views[t], c->cell_id_dev[t],
-                                                     c->history_dev + size_t(row) * c->n_cells, c->precision, c->stream),
+                                                     c->history_dev + size_t(row) * c->n_cells, nullptr, c->precision, c->stream),
                                  "objective");
       if (r) return r;
     }
@@ -665,15 +670,35 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   // the epilogue) applies d <- (1 - gamma) d + u while it streams d anyway.  Measured slower than
   // the default (the GEMM epilogue updates d in place from register-prefetched rows): 2.21 vs
   // 2.15 ms per RBC-642 iteration at 90,000 cells, so auto (0) means mode 1.
+  const bool ls_on = c->ls_max_halvings > 0;
+  if (ls_on) {
+    if (c->ls.size() != nb) c->ls.assign(nb, LineSearchDev());
+    for (size_t t = 0; t < nb; ++t) {
+      LineSearchDev &l = c->ls[t];
+      const size_t cells = size_t(c->buckets[t].cells);
+      if (l.obj0 || cells == 0) continue;
+      void *pd = nullptr, *pi = nullptr;
+      if (cudaMalloc(&pd, 4 * cells * sizeof(double)) != cudaSuccess || cudaMalloc(&pi, cells * sizeof(int)) != cudaSuccess) {
+        cudaGetLastError();
+        cudaFree(pd);
+        return fail(c, NPFEM_ENOMEM, "cannot allocate the line-search state");
+      }
+      l.obj0 = static_cast<double *>(pd);
+      l.obj1 = l.obj0 + cells;
+      l.slope = l.obj1 + cells;
+      l.alpha = l.slope + cells;
+      l.done = static_cast<int *>(pi);
+    }
+  }
   std::vector<char> fused(nb, 0);
   for (size_t t = 0; t < nb; ++t)
-    fused[t] = c->precision == NPFEM_F32 && !c->diagnostics && c->opt_global_math == 0 && c->opt_update_mode == 2 &&
+    fused[t] = !ls_on && c->precision == NPFEM_F32 && !c->diagnostics && c->opt_global_math == 0 && c->opt_update_mode == 2 &&
                (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]) &&
                global_tcgen05_supported(c->types[t]);
   for (int k = 0; k < n_iterations; ++k) {
     if (c->diagnostics && (rc = diag(k))) return rc;
     for (size_t t = 0; t < nb; ++t) {
-      const bool f32 = c->precision == NPFEM_F32;
+      const bool f32 = c->precision == NPFEM_F32 && !ls_on;   // the line search needs the FULL gradient: generic kernel
       const bool sched = f32 && (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]);
       const bool fast = f32 && !sched && c->opt_local_impl != 1 && local_smem_supported(c->types[t]);
       const double d_scale = (sched || fast) ? 1.0 - c->types[t].gamma : 1.0;
@@ -683,6 +708,14 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
              return launch_local_generic(c->types[t], c->views[t], c->buckets[t].scratch, c->precision, c->n_sm,
                                          c->stream); })))
         return rc;
+      if (ls_on && c->buckets[t].cells) {
+        // g(d) of every cell and a copy of d before the global step overwrites it
+        const size_t bytes = size_t(c->buckets[t].cells) * 3 * c->types[t].n_pad * esize(c->precision);
+        if ((rc = timed_launch(c, NPFEM_KIND_LINE_SEARCH, int(t), "line search: objective", [&] {
+               return launch_objective(c->types[t], c->views[t], nullptr, c->ls[t].obj0, nullptr, c->precision, c->stream); })))
+          return rc;
+        NPFEM_CUDA(c, cudaMemcpyAsync(c->views[t].field[F_U], c->views[t].field[F_D], bytes, cudaMemcpyDeviceToDevice, c->stream));
+      }
       if ((rc = timed_launch(c, NPFEM_KIND_GLOBAL, int(t), "global step", [&] {
              if (c->precision == NPFEM_F32 && c->opt_global_math == 0) {
                const int n = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, d_scale,
@@ -691,6 +724,17 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
              }
              return launch_global_simt(c->types[t], c->views[t], c->precision, d_scale, c->stream); })))
         return rc;
+      if (ls_on && c->buckets[t].cells) {
+        if ((rc = timed_launch(c, NPFEM_KIND_LINE_SEARCH, int(t), "line search", [&] {
+               int nl = launch_ls_init(c->views[t], c->ls[t], c->ls_tol, c->precision, c->stream);
+               for (int l = 0; l <= c->ls_max_halvings; ++l) {
+                 nl += launch_objective(c->types[t], c->views[t], nullptr, c->ls[t].obj1, c->ls[t].done, c->precision, c->stream);
+                 nl += launch_ls_accept(c->views[t], c->ls[t], c->ls_c1, l == c->ls_max_halvings, c->precision, c->stream);
+               }
+               return nl; })))
+          return rc;
+        c->ls_ran = true;
+      }
     }
   }
   if (c->diagnostics && (rc = diag(n_iterations))) return rc;
@@ -699,6 +743,32 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
            return launch_epilogue(c->types[t], c->views[t], c->precision, fused[t] != 0, 1.0 - c->types[t].gamma,
                                   c->stream); })))
       return rc;
+  return NPFEM_OK;
+}
+
+int npfem_set_line_search(npfem_ctx *c, int32_t max_halvings, double armijo_c1, double grad_tol) {
+  if (!c) return NPFEM_EINVAL;
+  if (max_halvings < 0 || max_halvings > 30 || !(armijo_c1 >= 0) || !(armijo_c1 < 1) || !(grad_tol >= 0))
+    return fail(c, NPFEM_EINVAL, "line search: 0 <= max_halvings <= 30, 0 <= armijo_c1 < 1, grad_tol >= 0");
+  c->ls_max_halvings = max_halvings;
+  c->ls_c1 = armijo_c1;
+  c->ls_tol = grad_tol;
+  return NPFEM_OK;
+}
+
+int npfem_get_step_lengths(npfem_ctx *c, double *alpha) {
+  if (!c || !alpha) return NPFEM_EINVAL;
+  if (c->sticky) return fail(c, NPFEM_ECUDA, "context is in a sticky CUDA error state: " + c->err);
+  if (!c->ls_ran) return fail(c, NPFEM_ESTATE, "no step lengths: enable npfem_set_line_search before npfem_step");
+  std::vector<std::vector<double>> per_bucket(c->buckets.size());
+  for (size_t t = 0; t < c->buckets.size(); ++t) {
+    per_bucket[t].resize(size_t(c->buckets[t].cells));
+    if (c->buckets[t].cells)
+      NPFEM_CUDA(c, cudaMemcpyAsync(per_bucket[t].data(), c->ls[t].alpha, per_bucket[t].size() * sizeof(double),
+                                    cudaMemcpyDeviceToHost, c->stream));
+  }
+  NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  for (int64_t cell = 0; cell < c->n_cells; ++cell) alpha[cell] = per_bucket[c->type_of_cell[cell]][c->slot_of_cell[cell]];
   return NPFEM_OK;
 }
 
@@ -841,6 +911,10 @@ void npfem_destroy(npfem_ctx *c) {
   cudaStreamSynchronize(c->stream);
   if (c->ws_owned && c->ws) cudaFree(c->ws);
   if (c->history_dev) cudaFree(c->history_dev);
+  for (auto &l : c->ls) {
+    if (l.obj0) cudaFree(l.obj0);
+    if (l.done) cudaFree(l.done);
+  }
   for (auto &sp : c->spans) {
     cudaEventDestroy(sp.a);
     cudaEventDestroy(sp.b);

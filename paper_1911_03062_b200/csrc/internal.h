@@ -106,8 +106,20 @@ int launch_epilogue(const TypeDev &td, const BucketView &bv, int precision, bool
 size_t local_generic_scratch_bytes(const TypeDev &td, int precision, int n_sm);
 int launch_local_generic(const TypeDev &td, const BucketView &bv, void *scratch, int precision, int n_sm,
                          cudaStream_t s);
+// cell_id_dev == nullptr: objective_row is indexed by the bucket slot; skip_dev[slot] != 0 skips a cell
 int launch_objective(const TypeDev &td, const BucketView &bv, const int64_t *cell_id_dev, double *objective_row,
-                     int precision, cudaStream_t s);
+                     const int *skip_dev, int precision, cudaStream_t s);
+
+// Armijo backtracking line search, per-cell state of one bucket
+struct LineSearchDev {
+  double *obj0 = nullptr, *obj1 = nullptr, *slope = nullptr, *alpha = nullptr;   // [cells]
+  int *done = nullptr;                                                            // [cells]
+};
+// after the global step: d holds d_old + p, u holds d_old, g the gradient.  slope = <g, p>, alpha = 1,
+// done = frozen (||g|| <= grad_tol ||b||: alpha = 0, d restored); g is overwritten with p
+int launch_ls_init(const BucketView &bv, const LineSearchDev &ls, double grad_tol, int precision, cudaStream_t s);
+// per cell not done: accept if obj1 <= obj0 + c1 alpha slope (or `last`), else alpha /= 2, d = d_old + alpha p
+int launch_ls_accept(const BucketView &bv, const LineSearchDev &ls, double c1, bool last, int precision, cudaStream_t s);
 
 // global step: d <- d - g Hinv   ([3 cells x n_pad] . [n_pad x n_pad])
 int launch_global_simt(const TypeDev &td, const BucketView &bv, int precision, double d_scale, cudaStream_t s);

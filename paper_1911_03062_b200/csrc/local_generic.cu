@@ -215,10 +215,12 @@ local_generic_kernel(const LocalParams<T> p) {
 template <typename T>
 __global__ void __launch_bounds__(256)
 objective_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_id, double *__restrict__ out_row,
-                 double h) {
+                 const int *__restrict__ skip, double h) {
+  // cell_id == nullptr: out_row is indexed by the bucket slot; skip[slot] != 0: leave that cell alone
   __shared__ double red[8];
   const int n = p.n, n_pad = p.n_pad, nt = p.T_;
   for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x) {
+    if (skip && skip[cell]) continue;
     const size_t base = size_t(cell) * 3 * n_pad;
     auto pos = [&](int v, int k) { return double(p.x[base + k * n_pad + v]) + double(p.d[base + k * n_pad + v]); };
     double acc = 0.0, vol = 0.0;
@@ -289,7 +291,7 @@ objective_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_id, do
     }
     if (threadIdx.x == 0) {
       const double V = two[1] / 6.0, V0 = double(p.V0);
-      out_row[cell_id[cell]] = two[0] + 0.5 * double(p.kv_over_V0) * (V - V0) * (V - V0);
+      out_row[cell_id ? cell_id[cell] : cell] = two[0] + 0.5 * double(p.kv_over_V0) * (V - V0) * (V - V0);
     }
     __syncthreads();
   }
@@ -365,13 +367,13 @@ int launch_local_generic(const TypeDev &td, const BucketView &bv, void *scratch,
 }
 
 int launch_objective(const TypeDev &td, const BucketView &bv, const int64_t *cell_id_dev, double *objective_row,
-                     int precision, cudaStream_t s) {
+                     const int *skip_dev, int precision, cudaStream_t s) {
   if (bv.cells == 0) return 0;
   const unsigned grid = unsigned(bv.cells < 148 * 8 ? bv.cells : 148 * 8);
   if (precision == NPFEM_F32)
-    objective_kernel<float><<<grid, 256, 0, s>>>(make_params<float>(td, bv), cell_id_dev, objective_row, td.h);
+    objective_kernel<float><<<grid, 256, 0, s>>>(make_params<float>(td, bv), cell_id_dev, objective_row, skip_dev, td.h);
   else
-    objective_kernel<double><<<grid, 256, 0, s>>>(make_params<double>(td, bv), cell_id_dev, objective_row, td.h);
+    objective_kernel<double><<<grid, 256, 0, s>>>(make_params<double>(td, bv), cell_id_dev, objective_row, skip_dev, td.h);
   return 1;
 }
 

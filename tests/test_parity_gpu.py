@@ -217,3 +217,78 @@ def test_irregular_mesh_valence_up_to_8(precision, impl):
     for r in compare(pop, gpu, ref):
         print(precision, impl, r)
         assert r["pos"] <= TOL_POS[precision] and r["disp"] <= TOL_DISP[precision] and r["vel"] <= TOL_DISP[precision], r
+
+
+def _ls_population(n_cells, h, force_sigma, seed):
+    """RBC-162 cells at rest shape under N(0, force_sigma) forces: with h = 30 us and 3000 pN the plain
+    iteration of Eq. (4) diverges (tests/test_oracle_pins.py), the line search must not."""
+    from workloads.meshes import rbc_cell_type
+    ct = rbc_cell_type(2)
+    rng = np.random.default_rng(seed)
+    pos = ct.rest_positions[None] + rng.uniform(0, 60, (n_cells, 1, 3))
+    return Population(name="ls", types=[ct], type_of_cell=np.zeros(n_cells, np.int32), positions=[pos],
+                      velocities=[np.zeros_like(pos)], dt=h, n_steps=1, n_iterations=15, box=(60.0,) * 3,
+                      force_sigma=force_sigma, shear_gamma=0.0, redraw_noise_each_step=False,
+                      _force_seed=np.random.SeedSequence(seed + 1), _shear_height=[pos[..., 2]])
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_line_search_violent_case_matches_oracle(precision):
+    """Armijo backtracking on the GPU against oracle.step_line_search, on a case
+    where the plain iteration blows up.  fp64: same step lengths (the decisions are taken in fp64 on
+    both sides); errors within the displacement bounds of DESIGN.md section 5 (1e-8 / 5e-3)."""
+    import torch
+    from oracle import npfem_oracle as orc
+    from paper_1911_03062_b200 import Solver
+    pop = _ls_population(9, 30.0, 3000.0, seed=21)
+    td = orc.make_type(pop.types[0], pop.dt)
+    f = pop.forces(0)[0]
+    xr, vr, hist = orc.step_line_search(pop.positions[0], pop.velocities[0], f, td, 15, max_halvings=8, c1=1e-4, record=True)
+    assert np.array(hist["alpha"]).min() < 1.0                       # the case does backtrack
+    solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision=precision)
+    solver.set_line_search(8, 1e-4, 0.0)
+    solver.set_state(torch.from_numpy(pop.packed(pop.positions)).cuda())
+    solver.set_forces(torch.from_numpy(pop.packed(pop.forces(0))).cuda())
+    solver.step(15)
+    x, v = solver.get_state()
+    alpha = solver.get_step_lengths()
+    solver.close()
+    xg = pop.unpack(x.cpu().numpy())[0]
+    x0 = pop.positions[0]
+    print(precision, "pos", rel_l2(xg, xr), "disp", rel_l2(xg - x0, xr - x0), "alpha gpu", alpha, "oracle", hist["alpha"][-1])
+    assert np.all(np.isfinite(xg))
+    # the cells deform by a good fraction of their size here, so the position-relative error IS the
+    # displacement-relative one: the displacement bound of DESIGN.md section 5 applies to both
+    assert rel_l2(xg, xr) <= TOL_DISP[precision]
+    assert rel_l2(xg - x0, xr - x0) <= TOL_DISP[precision]
+    if precision == "fp64":
+        assert np.array_equal(alpha, hist["alpha"][-1])
+    else:
+        assert np.all(np.isin(alpha, 0.5 ** np.arange(0, 9)))
+
+
+def test_line_search_is_neutral_on_a_tame_case_and_freezes_by_tolerance():
+    import torch
+    from paper_1911_03062_b200 import Solver
+    pop = make_config(3, n_cells=30)
+    ref = run_oracle(pop, 2, 5)                                      # plain oracle: every full step descends here
+    solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision="fp64")
+    solver.set_line_search(6)
+    solver.set_state(torch.from_numpy(pop.packed(pop.positions)).cuda())
+    for s in range(2):
+        solver.set_forces(torch.from_numpy(pop.packed(pop.forces(s))).cuda())
+        solver.step(5)
+    x, _ = solver.get_state()
+    assert np.all(solver.get_step_lengths() == 1.0)
+    xs = pop.unpack(x.cpu().numpy())
+    for t in range(2):
+        assert rel_l2(xs[t], ref[t][0]) <= 1e-10
+    # huge tolerance: nothing moves beyond d0 = h v (v = 0 here): positions stay
+    solver.set_line_search(6, 1e-4, 1e12)
+    x_before, _ = solver.get_state()
+    solver.step(3)
+    assert np.all(solver.get_step_lengths() == 0.0)
+    x_after, v_after = solver.get_state()
+    # d = h v_damped: the cells only coast with their (damped) velocity
+    assert torch.allclose(x_after, x_before + pop.dt * v_after, rtol=0, atol=1e-12)
+    solver.close()
