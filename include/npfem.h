@@ -68,6 +68,8 @@ extern "C" {
                                          3 = scheduled kernel (register-resident topology, conflict-free slots) */
 
 #define NPFEM_OPT_KERNEL_TIMING    4  /* 1: bracket every kernel of npfem_step with CUDA events */
+#define NPFEM_OPT_FORCE_MEDIAN_FILTER 6  /* 1: npfem_set_forces median-filters F_ext over the one-ring of every vertex
+                                            (per component, vertex + neighbours, even counts average) */
 #define NPFEM_OPT_UPDATE_MODE      5  /* fp32 tensor-core global step: 0 = auto (= 1), 1 = the GEMM epilogue updates d in place,
                                          2 = the GEMM writes its product, the next local step applies it */
 
@@ -175,6 +177,12 @@ int npfem_get_objective(npfem_ctx *ctx, double *history, int32_t max_entries,
  * gradient) and every iteration costs max_halvings + 2 extra objective evaluations.
  */
 int npfem_set_line_search(npfem_ctx *ctx, int32_t max_halvings, double armijo_c1, double grad_tol);
+
+/*
+ * Vertex-velocity cap: after every step the magnitude of each vertex velocity v_{n+1} is
+ * clamped to v_max (um/us), its direction kept; positions are not touched.  0 = off (default).
+ */
+int npfem_set_velocity_cap(npfem_ctx *ctx, double v_max);
 
 /* Step lengths alpha of the LAST iteration of the last step, HOST array [n_cells] in cell-id order. */
 int npfem_get_step_lengths(npfem_ctx *ctx, double *alpha);

@@ -307,6 +307,33 @@ def pbd_damping(x: np.ndarray, v: np.ndarray, mass: np.ndarray, kappa: float) ->
     return v + kappa * dv
 
 
+def cap_velocity(v: np.ndarray, v_max: float) -> np.ndarray:
+    """Vertex-velocity cap (the npFEM vertex velocity, "if it exceeds a value of U*_max,
+    is truncated towards this threshold").  Reading R17: the MAGNITUDE of each vertex velocity is
+    clamped to v_max, its direction kept; applied to v_{n+1} as stored."""
+    speed = np.sqrt(np.sum(v * v, axis=-1, keepdims=True))
+    return v * np.minimum(1.0, v_max / np.maximum(speed, np.finfo(np.float64).tiny))
+
+
+def one_ring(tri: np.ndarray, n: int) -> list:
+    """Sorted one-ring neighbour indices of every vertex."""
+    ring = [set() for _ in range(n)]
+    for a, b, c in tri:
+        ring[a].update((b, c)); ring[b].update((a, c)); ring[c].update((a, b))
+    return [np.array(sorted(r), dtype=np.int64) for r in ring]
+
+
+def median_filter_forces(f: np.ndarray, td: TypeData) -> np.ndarray:
+    """Median filter of F_ext "in the one-ring neighbourhood of every Lagrangian point".
+    Reading R18: per vertex and per Cartesian component, the median over the vertex itself and its
+    one-ring neighbours (an even count averages the two central values), SURVEY.md 8(f)-2."""
+    out = np.empty_like(f)
+    for v, ring in enumerate(one_ring(td.tri, td.n)):
+        idx = np.concatenate(([v], ring))
+        out[..., v, :] = np.median(f[..., idx, :], axis=-2)
+    return out
+
+
 def apply_M_tilde(d: np.ndarray, td: TypeData) -> np.ndarray:
     return np.einsum("ij,...jc->...ic", td.M_tilde, d)
 
@@ -337,7 +364,7 @@ def objective(d: np.ndarray, x_n: np.ndarray, b: np.ndarray, td: TypeData) -> np
 
 
 def step(x_n: np.ndarray, v_n: np.ndarray, f_ext: np.ndarray, td: TypeData,
-         n_iterations: int, record: bool = False):
+         n_iterations: int, record: bool = False, v_max: float = 0.0):
     """One time step h: {x_n, v_n} -> {x_{n+1}, v_{n+1}}.
 
     1. PBD damping of v_n (kappa > 0);  2. b = M v/h + F, d^0 = h v (reading R3);
@@ -361,6 +388,8 @@ def step(x_n: np.ndarray, v_n: np.ndarray, f_ext: np.ndarray, td: TypeData,
         history["grad_norm"].append(np.sqrt(np.sum(g * g, axis=(-2, -1))))
     x_next = x_n + d
     v_next = d / h
+    if v_max > 0.0:
+        v_next = cap_velocity(v_next, v_max)
     return (x_next, v_next, history) if record else (x_next, v_next)
 
 
@@ -424,9 +453,13 @@ def eq2_residual(v_damped: np.ndarray, x_next: np.ndarray, v_next: np.ndarray,
 
 
 def run(x0: np.ndarray, v0: np.ndarray, forces_of_step, td: TypeData,
-        n_steps: int, n_iterations: int):
-    """n_steps time steps; `forces_of_step(s)` returns F_ext for step s."""
+        n_steps: int, n_iterations: int, v_max: float = 0.0, median_filter: bool = False):
+    """n_steps time steps; `forces_of_step(s)` returns F_ext for step s (median-filtered over the
+    one-ring first if asked); v_max > 0 caps the vertex velocities."""
     x, v = x0.copy(), v0.copy()
     for s in range(n_steps):
-        x, v = step(x, v, forces_of_step(s), td, n_iterations)
+        f = forces_of_step(s)
+        if median_filter:
+            f = median_filter_forces(f, td)
+        x, v = step(x, v, f, td, n_iterations, v_max=v_max)
     return x, v

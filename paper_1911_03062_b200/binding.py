@@ -14,6 +14,7 @@ import numpy as np
 NPFEM_F32, NPFEM_F64 = 32, 64
 NPFEM_DEVICE, NPFEM_HOST = 0, 1
 OPT_DIAGNOSTICS, OPT_GLOBAL_STEP_MATH, OPT_LOCAL_STEP_IMPL, OPT_KERNEL_TIMING, OPT_UPDATE_MODE = 1, 2, 3, 4, 5
+OPT_FORCE_MEDIAN_FILTER = 6
 KIND_NAMES = ("prologue", "local", "global", "epilogue", "line_search")
 _ERR_NAMES = {-1: "NPFEM_EINVAL", -2: "NPFEM_EMESH", -3: "NPFEM_ECUDA", -4: "NPFEM_ENOMEM", -5: "NPFEM_ESTATE"}
 
@@ -21,7 +22,7 @@ EXPORTED_SYMBOLS = (
     "npfem_create", "npfem_workspace_bytes", "npfem_bind_workspace", "npfem_set_option",
     "npfem_set_state", "npfem_set_forces", "npfem_step", "npfem_get_state", "npfem_get_objective",
     "npfem_get_kernel_times", "npfem_launch_count", "npfem_last_error", "npfem_version", "npfem_destroy",
-    "npfem_local_schedule_stats", "npfem_set_line_search", "npfem_get_step_lengths",
+    "npfem_local_schedule_stats", "npfem_set_line_search", "npfem_get_step_lengths", "npfem_set_velocity_cap",
 )
 
 
@@ -93,6 +94,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.npfem_destroy.restype = None
     lib.npfem_set_line_search.argtypes = [vp, i32, C.c_double, C.c_double]
     lib.npfem_set_line_search.restype = C.c_int
+    lib.npfem_set_velocity_cap.argtypes = [vp, C.c_double]
+    lib.npfem_set_velocity_cap.restype = C.c_int
     lib.npfem_get_step_lengths.argtypes = [vp, vp]
     lib.npfem_get_step_lengths.restype = C.c_int
     lib.npfem_local_schedule_stats.argtypes = [C.POINTER(_CellType), C.c_double, C.POINTER(C.c_double), i32]
@@ -259,6 +262,10 @@ class Solver:
     def set_line_search(self, max_halvings: int, armijo_c1: float = 1e-4, grad_tol: float = 0.0) -> None:
         """Armijo backtracking + gradient-norm stopping test for the following steps (0 = off)."""
         self._check(self._lib.npfem_set_line_search(self._ctx, int(max_halvings), float(armijo_c1), float(grad_tol)))
+
+    def set_velocity_cap(self, v_max: float) -> None:
+        """Clamp |v_{n+1}| of every vertex to v_max after each step (0 = off)."""
+        self._check(self._lib.npfem_set_velocity_cap(self._ctx, float(v_max)))
 
     def get_step_lengths(self) -> np.ndarray:
         """alpha of the last iteration of the last step, [n_cells] in cell-id order."""

@@ -49,6 +49,9 @@ struct npfem_ctx {
   double ls_c1 = 1e-4, ls_tol = 0.0;
   std::vector<LineSearchDev> ls;          // per bucket, allocated on first use
   bool ls_ran = false;
+  // coupling-side options
+  bool median_filter = false;
+  double v_max = 0.0;
   int64_t launches = 0;
   // kernel timing (NPFEM_OPT_KERNEL_TIMING)
   bool timing = false;
@@ -546,6 +549,7 @@ int npfem_set_option(npfem_ctx *c, int32_t option, int64_t value) {
       c->opt_local_impl = value;
       return NPFEM_OK;
     case NPFEM_OPT_KERNEL_TIMING: c->timing = value != 0; return NPFEM_OK;
+    case NPFEM_OPT_FORCE_MEDIAN_FILTER: c->median_filter = value != 0; return NPFEM_OK;
     case NPFEM_OPT_UPDATE_MODE:
       if (value < 0 || value > 2) return fail(c, NPFEM_EINVAL, "update mode must be 0, 1 or 2");
       c->opt_update_mode = value;
@@ -597,6 +601,12 @@ int npfem_set_forces(npfem_ctx *c, const int64_t *cell_ids, int64_t n_ids, const
     a.src_a = c->stage_a;
   }
   if ((rc = check_launch(c, launch_set_forces(c->views_dev, a, c->precision, c->stream), "set_forces"))) return rc;
+  if (c->median_filter)
+    for (size_t t = 0; t < c->buckets.size(); ++t)
+      if (c->buckets[t].cells &&
+          (rc = check_launch(c, launch_median_filter(c->views_dev, a.refs, a.n_refs, int(t), c->types[t], c->precision, c->stream),
+                             "median filter")))
+        return rc;
   if (where == NPFEM_HOST) NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
   return NPFEM_OK;
 }
@@ -741,7 +751,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   for (size_t t = 0; t < nb; ++t)
     if ((rc = timed_launch(c, NPFEM_KIND_EPILOGUE, int(t), "epilogue", [&] {
            return launch_epilogue(c->types[t], c->views[t], c->precision, fused[t] != 0, 1.0 - c->types[t].gamma,
-                                  c->stream); })))
+                                  c->v_max, c->stream); })))
       return rc;
   return NPFEM_OK;
 }
@@ -753,6 +763,13 @@ int npfem_set_line_search(npfem_ctx *c, int32_t max_halvings, double armijo_c1, 
   c->ls_max_halvings = max_halvings;
   c->ls_c1 = armijo_c1;
   c->ls_tol = grad_tol;
+  return NPFEM_OK;
+}
+
+int npfem_set_velocity_cap(npfem_ctx *c, double v_max) {
+  if (!c) return NPFEM_EINVAL;
+  if (!(v_max >= 0)) return fail(c, NPFEM_EINVAL, "velocity cap must be >= 0 (0 = off)");
+  c->v_max = v_max;
   return NPFEM_OK;
 }
 

@@ -100,7 +100,11 @@ int launch_get_state(const BucketView *views_dev, const PackArgs &a, int precisi
 int launch_prologue(const TypeDev &td, const BucketView &bv, int precision, cudaStream_t s);
 // pending: d <- d_scale d + u still has to be applied (fused-update mode, see npfem_step)
 int launch_epilogue(const TypeDev &td, const BucketView &bv, int precision, bool pending, double d_scale,
-                    cudaStream_t s);
+                    double v_max, cudaStream_t s);
+
+// one-ring median filter of the forces of the listed cells that belong to `bucket` (coupling.cu)
+int launch_median_filter(const BucketView *views_dev, const CellRef *refs_dev, int64_t n_refs, int bucket,
+                         const TypeDev &td, int precision, cudaStream_t s);
 
 // local step: g = M~ d/h^2 - b + grad E(x_n + d)
 size_t local_generic_scratch_bytes(const TypeDev &td, int precision, int n_sm);

@@ -241,17 +241,32 @@ prologue_warp_kernel(BucketView bv, const float *__restrict__ mass, float kappa,
 
 template <typename T>
 __global__ void __launch_bounds__(256)
-epilogue_kernel(BucketView bv, T inv_h, bool pending, T d_scale) {
+epilogue_kernel(BucketView bv, T inv_h, bool pending, T d_scale, T v_max) {
   T *x = static_cast<T *>(bv.field[F_X]);
   T *v = static_cast<T *>(bv.field[F_V]);
   const T *d = static_cast<const T *>(bv.field[F_D]);
   const T *u = static_cast<const T *>(bv.field[F_U]);
-  const size_t total = size_t(bv.cells) * 3 * bv.n_pad;
+  const int n_pad = bv.n_pad;
+  const size_t total = size_t(bv.cells) * n_pad;          // one thread per (cell, vertex slot)
   for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < total; i += size_t(gridDim.x) * blockDim.x) {
-    // pending: the last global step left its product in u (d <- d_scale d + u not applied yet)
-    const T di = pending ? d_scale * d[i] + u[i] : d[i];
-    x[i] += di;
-    v[i] = di * inv_h;
+    const size_t base = (i / n_pad) * 3 * size_t(n_pad) + i % n_pad;
+    T vi[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const size_t o = base + size_t(k) * n_pad;
+      // pending: the last global step left its product in u (d <- d_scale d + u not applied yet)
+      const T di = pending ? d_scale * d[o] + u[o] : d[o];
+      x[o] += di;
+      vi[k] = di * inv_h;
+    }
+    if (v_max > T(0)) {   // vertex-velocity cap (reading R17): clamp the magnitude, keep the direction
+      const T speed = sqrt(vi[0] * vi[0] + vi[1] * vi[1] + vi[2] * vi[2]);
+      const T scale = speed > v_max ? v_max / speed : T(1);
+#pragma unroll
+      for (int k = 0; k < 3; ++k) vi[k] *= scale;
+    }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) v[base + size_t(k) * n_pad] = vi[k];
   }
 }
 
@@ -276,14 +291,14 @@ int launch_prologue(const TypeDev &td, const BucketView &bv, int precision, cuda
 }
 
 int launch_epilogue(const TypeDev &td, const BucketView &bv, int precision, bool pending, double d_scale,
-                    cudaStream_t s) {
+                    double v_max, cudaStream_t s) {
   if (bv.cells == 0) return 0;
-  const size_t total = size_t(bv.cells) * 3 * bv.n_pad;
+  const size_t total = size_t(bv.cells) * bv.n_pad;
   const unsigned grid = unsigned((total + 255) / 256 < 148 * 16 ? (total + 255) / 256 : 148 * 16);
   if (precision == NPFEM_F32)
-    epilogue_kernel<float><<<grid, 256, 0, s>>>(bv, float(1.0 / td.h), pending, float(d_scale));
+    epilogue_kernel<float><<<grid, 256, 0, s>>>(bv, float(1.0 / td.h), pending, float(d_scale), float(v_max));
   else
-    epilogue_kernel<double><<<grid, 256, 0, s>>>(bv, 1.0 / td.h, pending, d_scale);
+    epilogue_kernel<double><<<grid, 256, 0, s>>>(bv, 1.0 / td.h, pending, d_scale, v_max);
   return 1;
 }
 

@@ -451,3 +451,48 @@ def test_ls_gradient_tolerance_freezes_converged_cells(rbc162):
     alpha = np.array(hist_b["alpha"])
     assert np.all(alpha[-1] == 0.0) and np.all(alpha[0] == 1.0)       # they did stop, after working
     assert np.linalg.norm(xb - xc) <= 1e-5 * np.linalg.norm(xc - x)
+
+
+# ---- velocity cap and one-ring median filter of F_ext ----
+def test_velocity_cap_closed_form():
+    rng = np.random.default_rng(0)
+    v = rng.standard_normal((4, 50, 3)) * np.array([0.01, 0.1, 1.0, 10.0])[:, None, None]
+    out = orc.cap_velocity(v, 0.5)
+    speed_in, speed_out = np.linalg.norm(v, axis=-1), np.linalg.norm(out, axis=-1)
+    assert np.all(speed_out <= 0.5 * (1 + 1e-15))
+    slow = speed_in <= 0.5
+    assert np.array_equal(out[slow], v[slow])                              # untouched below the threshold
+    assert np.allclose(speed_out[~slow], 0.5, rtol=1e-14)                  # exactly on it above
+    assert np.allclose(np.cross(out, v), 0.0, atol=1e-12)                  # direction kept
+    assert np.array_equal(orc.cap_velocity(np.zeros((2, 3, 3)), 0.5), np.zeros((2, 3, 3)))   # no 0/0
+
+
+def test_median_filter_removes_a_spike_and_keeps_a_constant(ico):
+    ct, td = ico                                  # icosahedron: every vertex has exactly 5 neighbours
+    ring = orc.one_ring(td.tri, td.n)
+    assert all(len(r) == 5 for r in ring) and all(v not in r for v, r in enumerate(ring))
+    f = np.tile(np.array([1.0, -2.0, 3.0]), (td.n, 1))
+    assert np.array_equal(orc.median_filter_forces(f, td), f)              # constant field is a fixed point
+    spike = f.copy()
+    spike[7] = [1e6, 1e6, 1e6]
+    assert np.array_equal(orc.median_filter_forces(spike, td), f)          # one outlier never reaches a median of 6
+    # brute force against the definition on random data (6 values: mean of the two central ones)
+    rng = np.random.default_rng(1)
+    g = rng.standard_normal((3, td.n, 3))
+    out = orc.median_filter_forces(g, td)
+    for c in range(3):
+        for v in range(td.n):
+            for k in range(3):
+                vals = sorted([g[c, v, k]] + [g[c, u, k] for u in ring[v]])
+                assert out[c, v, k] == 0.5 * (vals[2] + vals[3])
+
+
+def test_step_with_cap_only_changes_the_velocity(rbc162):
+    ct, td = rbc162
+    rng = np.random.default_rng(5)
+    x = ct.rest_positions[None]
+    f = 50.0 * rng.standard_normal(x.shape)
+    xa, va = orc.step(x, 0 * x, f, td, 4)
+    xb, vb = orc.step(x, 0 * x, f, td, 4, v_max=1e-4)
+    assert np.array_equal(xa, xb) and np.linalg.norm(va, axis=-1).max() > 1e-4
+    assert np.array_equal(vb, orc.cap_velocity(va, 1e-4))

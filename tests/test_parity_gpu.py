@@ -292,3 +292,39 @@ def test_line_search_is_neutral_on_a_tame_case_and_freezes_by_tolerance():
     # d = h v_damped: the cells only coast with their (damped) velocity
     assert torch.allclose(x_after, x_before + pop.dt * v_after, rtol=0, atol=1e-12)
     solver.close()
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_median_filtered_forces_and_velocity_cap(precision):
+    """one-ring median filter of F_ext in set_forces and the vertex-velocity
+    cap in the epilogue against the oracle; mixed cell types (valence 5 and 6: even and odd
+    median counts), forces redrawn every step, the cap set so that it really bites."""
+    import torch
+    from oracle import npfem_oracle as orc
+    from paper_1911_03062_b200 import Solver, binding
+    pop = make_config(3, n_cells=34)
+    n_steps, n_its, v_max = 3, 5, 2.0e-4
+    solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision=precision)
+    solver.set_option(binding.OPT_FORCE_MEDIAN_FILTER, 1)
+    solver.set_velocity_cap(v_max)
+    solver.set_state(torch.from_numpy(pop.packed(pop.positions)).cuda())
+    for s in range(n_steps):
+        solver.set_forces(torch.from_numpy(pop.packed(pop.forces(s))).cuda())
+        solver.step(n_its)
+    x, v = solver.get_state()
+    solver.close()
+    xs, vs = pop.unpack(x.cpu().numpy()), pop.unpack(v.cpu().numpy())
+    for t, ct in enumerate(pop.types):
+        td = orc.make_type(ct, pop.dt)
+        xr, vr = orc.run(pop.positions[t], pop.velocities[t], lambda s, t=t: pop.forces(s)[t], td, n_steps, n_its,
+                         v_max=v_max, median_filter=True)
+        x_plain, v_plain = orc.run(pop.positions[t], pop.velocities[t], lambda s, t=t: pop.forces(s)[t], td, n_steps, n_its)
+        x0 = pop.positions[t]
+        speed = np.linalg.norm(vr, axis=-1)
+        assert np.isclose(speed.max(), v_max) and np.linalg.norm(v_plain, axis=-1).max() > v_max   # the cap bites
+        assert rel_l2(xr - x0, x_plain - x0) > 0.05                                              # the filter matters
+        print(precision, ct.name, rel_l2(xs[t], xr), rel_l2(xs[t] - x0, xr - x0), rel_l2(vs[t], vr))
+        assert rel_l2(xs[t], xr) <= TOL_POS[precision]
+        assert rel_l2(xs[t] - x0, xr - x0) <= TOL_DISP[precision]
+        assert rel_l2(vs[t], vr) <= TOL_DISP[precision]
+        assert np.linalg.norm(vs[t], axis=-1).max() <= v_max * (1 + 1e-6)
