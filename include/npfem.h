@@ -179,6 +179,18 @@ int npfem_get_objective(npfem_ctx *ctx, double *history, int32_t max_entries,
 int npfem_set_line_search(npfem_ctx *ctx, int32_t max_halvings, double armijo_c1, double grad_tol);
 
 /*
+ * PIK collision term (near contact "a collision force, coming from a quadratic potential
+ * energy" replaces the fluid force).  For the listed cells: targets p `[n][3]` (the
+ * projection points from the caller's collision detection, global coordinates like positions) and
+ * stiffness k `[n]` (pN/um, 0 = vertex not in contact), both of `dtype`, living `where` says.  The energy
+ * sum_i 1/2 k_i |x_i - p_i|^2 enters grad g and the objective of every following step (not the constant
+ * H~: keep k well below m_v / h^2), until overwritten or cleared.  Collision DETECTION is the caller's.
+ */
+int npfem_set_collisions(npfem_ctx *ctx, const int64_t *cell_ids, int64_t n_ids, const void *targets,
+                         const void *stiffness, int32_t dtype, int32_t where);
+int npfem_clear_collisions(npfem_ctx *ctx);
+
+/*
  * Vertex-velocity cap: after every step the magnitude of each vertex velocity v_{n+1} is
  * clamped to v_max (um/us), its direction kept; positions are not touched.  0 = off (default).
  */

@@ -346,25 +346,44 @@ def solve_H_tilde(g: np.ndarray, td: TypeData) -> np.ndarray:
     return np.moveaxis(sol.reshape(td.n, -1, 3), 0, 1).reshape(lead + (td.n, 3))
 
 
-def gradient_g(d: np.ndarray, x_n: np.ndarray, b: np.ndarray, td: TypeData) -> np.ndarray:
+def collision_energy(x: np.ndarray, targets: np.ndarray, stiffness: np.ndarray) -> np.ndarray:
+    """PIK collision energy (near contact "a collision force, coming from a quadratic
+    potential energy", replaces the fluid force): sum_i 1/2 k_i |x_i - p_i|^2 over the flagged vertices
+    (k_i = 0: not in contact), p_i the projection point handed over by the collision detection
+    (reading R19: the term enters grad g but not the constant H~)."""
+    return 0.5 * np.sum(stiffness * np.sum((x - targets) ** 2, axis=-1), axis=-1)
+
+
+def grad_collision(x: np.ndarray, targets: np.ndarray, stiffness: np.ndarray) -> np.ndarray:
+    return stiffness[..., None] * (x - targets)
+
+
+def gradient_g(d: np.ndarray, x_n: np.ndarray, b: np.ndarray, td: TypeData, collisions=None) -> np.ndarray:
     """grad g = M~ (x - y_n)/h^2 + grad E(x) written with d = x - x_n:  M~ d/h^2 - b + grad E.
 
     b = M v_n/h + F_ext, because M~ y_n/h^2 = M~ x_n/h^2 + M v_n/h + F_ext.
+    collisions = (targets, stiffness) adds the PIK term.
     """
-    return apply_M_tilde(d, td) / td.h ** 2 - b + grad_energy(x_n + d, td)
+    g = apply_M_tilde(d, td) / td.h ** 2 - b + grad_energy(x_n + d, td)
+    if collisions is not None:
+        g = g + grad_collision(x_n + d, *collisions)
+    return g
 
 
-def objective(d: np.ndarray, x_n: np.ndarray, b: np.ndarray, td: TypeData) -> np.ndarray:
+def objective(d: np.ndarray, x_n: np.ndarray, b: np.ndarray, td: TypeData, collisions=None) -> np.ndarray:
     """g of Eq. (3) minus the d-independent constant (h^2/2) b^T M~^-1 b:
 
     1/(2h^2) d^T M~ d - d^T b + E(x_n + d).  Its gradient is `gradient_g`.
     """
     quad = 0.5 * np.sum(d * apply_M_tilde(d, td), axis=(-2, -1)) / td.h ** 2
-    return quad - np.sum(d * b, axis=(-2, -1)) + total_energy(x_n + d, td)
+    out = quad - np.sum(d * b, axis=(-2, -1)) + total_energy(x_n + d, td)
+    if collisions is not None:
+        out = out + collision_energy(x_n + d, *collisions)
+    return out
 
 
 def step(x_n: np.ndarray, v_n: np.ndarray, f_ext: np.ndarray, td: TypeData,
-         n_iterations: int, record: bool = False, v_max: float = 0.0):
+         n_iterations: int, record: bool = False, v_max: float = 0.0, collisions=None):
     """One time step h: {x_n, v_n} -> {x_{n+1}, v_{n+1}}.
 
     1. PBD damping of v_n (kappa > 0);  2. b = M v/h + F, d^0 = h v (reading R3);
@@ -377,14 +396,14 @@ def step(x_n: np.ndarray, v_n: np.ndarray, f_ext: np.ndarray, td: TypeData,
     d = h * v
     history = {"objective": [], "grad_norm": [], "v_damped": v}
     for _ in range(n_iterations):
-        g = gradient_g(d, x_n, b, td)
+        g = gradient_g(d, x_n, b, td, collisions)
         if record:
-            history["objective"].append(objective(d, x_n, b, td))
+            history["objective"].append(objective(d, x_n, b, td, collisions))
             history["grad_norm"].append(np.sqrt(np.sum(g * g, axis=(-2, -1))))
         d = d - solve_H_tilde(g, td)
     if record:
-        g = gradient_g(d, x_n, b, td)
-        history["objective"].append(objective(d, x_n, b, td))
+        g = gradient_g(d, x_n, b, td, collisions)
+        history["objective"].append(objective(d, x_n, b, td, collisions))
         history["grad_norm"].append(np.sqrt(np.sum(g * g, axis=(-2, -1))))
     x_next = x_n + d
     v_next = d / h
@@ -453,7 +472,7 @@ def eq2_residual(v_damped: np.ndarray, x_next: np.ndarray, v_next: np.ndarray,
 
 
 def run(x0: np.ndarray, v0: np.ndarray, forces_of_step, td: TypeData,
-        n_steps: int, n_iterations: int, v_max: float = 0.0, median_filter: bool = False):
+        n_steps: int, n_iterations: int, v_max: float = 0.0, median_filter: bool = False, collisions=None):
     """n_steps time steps; `forces_of_step(s)` returns F_ext for step s (median-filtered over the
     one-ring first if asked); v_max > 0 caps the vertex velocities."""
     x, v = x0.copy(), v0.copy()
@@ -461,5 +480,5 @@ def run(x0: np.ndarray, v0: np.ndarray, forces_of_step, td: TypeData,
         f = forces_of_step(s)
         if median_filter:
             f = median_filter_forces(f, td)
-        x, v = step(x, v, f, td, n_iterations, v_max=v_max)
+        x, v = step(x, v, f, td, n_iterations, v_max=v_max, collisions=collisions)
     return x, v

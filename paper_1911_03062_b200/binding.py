@@ -22,7 +22,8 @@ EXPORTED_SYMBOLS = (
     "npfem_create", "npfem_workspace_bytes", "npfem_bind_workspace", "npfem_set_option",
     "npfem_set_state", "npfem_set_forces", "npfem_step", "npfem_get_state", "npfem_get_objective",
     "npfem_get_kernel_times", "npfem_launch_count", "npfem_last_error", "npfem_version", "npfem_destroy",
-    "npfem_local_schedule_stats", "npfem_set_line_search", "npfem_get_step_lengths", "npfem_set_velocity_cap",
+    "npfem_local_schedule_stats", "npfem_set_line_search", "npfem_get_step_lengths", "npfem_set_velocity_cap", "npfem_set_collisions",
+    "npfem_clear_collisions",
 )
 
 
@@ -94,6 +95,10 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.npfem_destroy.restype = None
     lib.npfem_set_line_search.argtypes = [vp, i32, C.c_double, C.c_double]
     lib.npfem_set_line_search.restype = C.c_int
+    lib.npfem_set_collisions.argtypes = [vp, C.POINTER(i64), i64, vp, vp, i32, i32]
+    lib.npfem_set_collisions.restype = C.c_int
+    lib.npfem_clear_collisions.argtypes = [vp]
+    lib.npfem_clear_collisions.restype = C.c_int
     lib.npfem_set_velocity_cap.argtypes = [vp, C.c_double]
     lib.npfem_set_velocity_cap.restype = C.c_int
     lib.npfem_get_step_lengths.argtypes = [vp, vp]
@@ -227,6 +232,19 @@ class Solver:
         ids_p, n_ids, ids = self._ids(cell_ids)
         p, code, where, _k = self._buffer(forces, self._count(ids), "forces")
         self._check(self._lib.npfem_set_forces(self._ctx, ids_p, n_ids, p, code, where))
+
+    def set_collisions(self, targets, stiffness, cell_ids=None) -> None:
+        """PIK collision term: targets `[n][3]` and stiffness `[n]` per listed cell (same dtype and place)."""
+        ids_p, n_ids, ids = self._ids(cell_ids)
+        count = self._count(ids)
+        p, code, where, _k = self._buffer(targets, count, "targets")
+        q, code_q, where_q, _k2 = self._buffer(stiffness, count // 3, "stiffness")
+        if code != code_q or where != where_q:
+            raise ValueError("targets and stiffness must share dtype and location")
+        self._check(self._lib.npfem_set_collisions(self._ctx, ids_p, n_ids, p, q, code, where))
+
+    def clear_collisions(self) -> None:
+        self._check(self._lib.npfem_clear_collisions(self._ctx))
 
     def step(self, n_iterations: int) -> None:
         self._check(self._lib.npfem_step(self._ctx, int(n_iterations)))

@@ -52,6 +52,9 @@ struct npfem_ctx {
   // coupling-side options
   bool median_filter = false;
   double v_max = 0.0;
+  std::vector<CollisionDev> col;          // per bucket, allocated by the first npfem_set_collisions
+  CollisionDev *col_dev = nullptr;        // the same table on the device
+  bool col_active = false;
   int64_t launches = 0;
   // kernel timing (NPFEM_OPT_KERNEL_TIMING)
   bool timing = false;
@@ -663,10 +666,14 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   }
   auto diag = [&](int row) -> int {
     for (size_t t = 0; t < nb; ++t) {
-      const int r = check_launch(c, launch_objective(c->types[t], c->views[t], c->cell_id_dev[t],
-                                                     c->history_dev + size_t(row) * c->n_cells, nullptr, c->precision, c->stream),
-                                 "objective");
+      double *out = c->history_dev + size_t(row) * c->n_cells;
+      int r = check_launch(c, launch_objective(c->types[t], c->views[t], c->cell_id_dev[t], out, nullptr, c->precision, c->stream),
+                           "objective");
       if (r) return r;
+      if (c->col_active &&
+          (r = check_launch(c, launch_collision_energy(c->views[t], c->col[t], c->cell_id_dev[t], out, nullptr, c->precision,
+                                                       c->stream), "collision energy")))
+        return r;
     }
     return NPFEM_OK;
   };
@@ -702,7 +709,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   }
   std::vector<char> fused(nb, 0);
   for (size_t t = 0; t < nb; ++t)
-    fused[t] = !ls_on && c->precision == NPFEM_F32 && !c->diagnostics && c->opt_global_math == 0 && c->opt_update_mode == 2 &&
+    fused[t] = !ls_on && !c->col_active && c->precision == NPFEM_F32 && !c->diagnostics && c->opt_global_math == 0 && c->opt_update_mode == 2 &&
                (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]) &&
                global_tcgen05_supported(c->types[t]);
   for (int k = 0; k < n_iterations; ++k) {
@@ -718,11 +725,18 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
              return launch_local_generic(c->types[t], c->views[t], c->buckets[t].scratch, c->precision, c->n_sm,
                                          c->stream); })))
         return rc;
+      if (c->col_active && c->buckets[t].cells &&
+          (rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "collision gradient", [&] {
+             return launch_collision_grad(c->views[t], c->col[t], c->precision, c->stream); })))
+        return rc;
       if (ls_on && c->buckets[t].cells) {
         // g(d) of every cell and a copy of d before the global step overwrites it
         const size_t bytes = size_t(c->buckets[t].cells) * 3 * c->types[t].n_pad * esize(c->precision);
         if ((rc = timed_launch(c, NPFEM_KIND_LINE_SEARCH, int(t), "line search: objective", [&] {
-               return launch_objective(c->types[t], c->views[t], nullptr, c->ls[t].obj0, nullptr, c->precision, c->stream); })))
+               int nl = launch_objective(c->types[t], c->views[t], nullptr, c->ls[t].obj0, nullptr, c->precision, c->stream);
+               if (c->col_active)
+                 nl += launch_collision_energy(c->views[t], c->col[t], nullptr, c->ls[t].obj0, nullptr, c->precision, c->stream);
+               return nl; })))
           return rc;
         NPFEM_CUDA(c, cudaMemcpyAsync(c->views[t].field[F_U], c->views[t].field[F_D], bytes, cudaMemcpyDeviceToDevice, c->stream));
       }
@@ -739,6 +753,9 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
                int nl = launch_ls_init(c->views[t], c->ls[t], c->ls_tol, c->precision, c->stream);
                for (int l = 0; l <= c->ls_max_halvings; ++l) {
                  nl += launch_objective(c->types[t], c->views[t], nullptr, c->ls[t].obj1, c->ls[t].done, c->precision, c->stream);
+                 if (c->col_active)
+                   nl += launch_collision_energy(c->views[t], c->col[t], nullptr, c->ls[t].obj1, c->ls[t].done, c->precision,
+                                                 c->stream);
                  nl += launch_ls_accept(c->views[t], c->ls[t], c->ls_c1, l == c->ls_max_halvings, c->precision, c->stream);
                }
                return nl; })))
@@ -763,6 +780,65 @@ int npfem_set_line_search(npfem_ctx *c, int32_t max_halvings, double armijo_c1, 
   c->ls_max_halvings = max_halvings;
   c->ls_c1 = armijo_c1;
   c->ls_tol = grad_tol;
+  return NPFEM_OK;
+}
+
+int npfem_set_collisions(npfem_ctx *c, const int64_t *cell_ids, int64_t n_ids, const void *targets, const void *stiffness,
+                         int32_t dtype, int32_t where) {
+  int rc = common_checks(c, dtype, where);
+  if (rc) return rc;
+  if (!targets || !stiffness) return fail(c, NPFEM_EINVAL, "targets / stiffness is NULL");
+  if (!c->ready || c->n_set != c->n_cells) return fail(c, NPFEM_ESTATE, "set_collisions before every cell has been given a state");
+  const size_t nb = c->buckets.size(), es = esize(c->precision);
+  if (c->col.size() != nb) {
+    c->col.assign(nb, CollisionDev());
+    for (size_t t = 0; t < nb; ++t) {
+      const size_t slots = size_t(c->buckets[t].cells) * c->types[t].n_pad;
+      if (!slots) continue;
+      if (cudaMalloc(&c->col[t].targets, 3 * slots * es) != cudaSuccess || cudaMalloc(&c->col[t].stiffness, slots * es) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, NPFEM_ENOMEM, "cannot allocate the collision targets");
+      }
+      NPFEM_CUDA(c, cudaMemsetAsync(c->col[t].targets, 0, 3 * slots * es, c->stream));
+      NPFEM_CUDA(c, cudaMemsetAsync(c->col[t].stiffness, 0, slots * es, c->stream));
+    }
+    void *p = nullptr;
+    if (cudaMalloc(&p, nb * sizeof(CollisionDev)) != cudaSuccess) {
+      cudaGetLastError();
+      return fail(c, NPFEM_ENOMEM, "cannot allocate the collision table");
+    }
+    c->col_dev = static_cast<CollisionDev *>(p);
+    NPFEM_CUDA(c, cudaMemcpyAsync(c->col_dev, c->col.data(), nb * sizeof(CollisionDev), cudaMemcpyHostToDevice, c->stream));
+    NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  }
+  PackArgs a{};
+  int64_t n_elems = 0;
+  if ((rc = resolve_refs(c, cell_ids, n_ids, &a.refs, &a.n_refs, &n_elems, false))) return rc;
+  a.io_dtype = dtype;
+  a.src_a = targets;
+  a.src_b = stiffness;
+  if (where == NPFEM_HOST && n_elems) {
+    const size_t bytes = size_t(n_elems) * (dtype == NPFEM_F32 ? 4 : 8);
+    NPFEM_CUDA(c, cudaMemcpyAsync(c->stage_a, targets, bytes, cudaMemcpyHostToDevice, c->stream));
+    NPFEM_CUDA(c, cudaMemcpyAsync(c->stage_b, stiffness, bytes / 3, cudaMemcpyHostToDevice, c->stream));
+    a.src_a = c->stage_a;
+    a.src_b = c->stage_b;
+  }
+  if ((rc = check_launch(c, launch_set_collisions(c->views_dev, c->col_dev, a, c->precision, c->stream), "set_collisions")))
+    return rc;
+  if (where == NPFEM_HOST) NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  c->col_active = true;
+  return NPFEM_OK;
+}
+
+int npfem_clear_collisions(npfem_ctx *c) {
+  if (!c) return NPFEM_EINVAL;
+  if (c->sticky) return fail(c, NPFEM_ECUDA, "context is in a sticky CUDA error state: " + c->err);
+  for (size_t t = 0; t < c->col.size(); ++t) {
+    const size_t slots = size_t(c->buckets[t].cells) * c->types[t].n_pad;
+    if (slots) NPFEM_CUDA(c, cudaMemsetAsync(c->col[t].stiffness, 0, slots * esize(c->precision), c->stream));
+  }
+  c->col_active = false;
   return NPFEM_OK;
 }
 
@@ -928,6 +1004,11 @@ void npfem_destroy(npfem_ctx *c) {
   cudaStreamSynchronize(c->stream);
   if (c->ws_owned && c->ws) cudaFree(c->ws);
   if (c->history_dev) cudaFree(c->history_dev);
+  for (auto &cl : c->col) {
+    if (cl.targets) cudaFree(cl.targets);
+    if (cl.stiffness) cudaFree(cl.stiffness);
+  }
+  if (c->col_dev) cudaFree(c->col_dev);
   for (auto &l : c->ls) {
     if (l.obj0) cudaFree(l.obj0);
     if (l.done) cudaFree(l.done);

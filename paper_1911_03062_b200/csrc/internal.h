@@ -102,6 +102,17 @@ int launch_prologue(const TypeDev &td, const BucketView &bv, int precision, cuda
 int launch_epilogue(const TypeDev &td, const BucketView &bv, int precision, bool pending, double d_scale,
                     double v_max, cudaStream_t s);
 
+// PIK collision term (coupling.cu): per bucket, targets [cells][3][n_pad] in cell-local coordinates and
+// stiffness [cells][n_pad] (0 = vertex not in contact), compute type
+struct CollisionDev {
+  void *targets = nullptr, *stiffness = nullptr;
+};
+int launch_set_collisions(const BucketView *views_dev, const CollisionDev *cols_dev, const PackArgs &a, int precision,
+                          cudaStream_t s);   // a.src_a = targets, a.src_b = stiffness
+int launch_collision_grad(const BucketView &bv, const CollisionDev &col, int precision, cudaStream_t s);
+int launch_collision_energy(const BucketView &bv, const CollisionDev &col, const int64_t *cell_id_dev, double *out,
+                            const int *skip_dev, int precision, cudaStream_t s);
+
 // one-ring median filter of the forces of the listed cells that belong to `bucket` (coupling.cu)
 int launch_median_filter(const BucketView *views_dev, const CellRef *refs_dev, int64_t n_refs, int bucket,
                          const TypeDev &td, int precision, cudaStream_t s);

@@ -496,3 +496,41 @@ def test_step_with_cap_only_changes_the_velocity(rbc162):
     xb, vb = orc.step(x, 0 * x, f, td, 4, v_max=1e-4)
     assert np.array_equal(xa, xb) and np.linalg.norm(va, axis=-1).max() > 1e-4
     assert np.array_equal(vb, orc.cap_velocity(va, 1e-4))
+
+
+# ---- PIK collision energy ----
+def test_collision_energy_closed_forms_and_gradient(rbc162):
+    ct, td = rbc162
+    rng = np.random.default_rng(6)
+    x = ct.rest_positions + 0.05 * rng.standard_normal(ct.rest_positions.shape)
+    k = np.where(rng.random(td.n) < 0.3, rng.uniform(10, 200, td.n), 0.0)       # 30 % of the vertices in contact
+    t = np.array([0.3, -0.2, 0.1])
+    # rigid offset from the targets: E = 1/2 sum k |t|^2, gradient k t; zero at the targets
+    assert np.isclose(orc.collision_energy(x + t, x, k), 0.5 * k.sum() * t @ t, rtol=1e-14)
+    assert np.allclose(orc.grad_collision(x + t, x, k), k[:, None] * t, rtol=1e-14)
+    assert orc.collision_energy(x, x, k) == 0.0 and not orc.grad_collision(x, x, k).any()
+    # central finite differences of the energy against the analytic gradient
+    p = x + 0.1 * rng.standard_normal(x.shape)
+    g = orc.grad_collision(x, p, k)
+    for v, c in [(0, 0), (5, 1), (17, 2), (100, 0)]:
+        e = np.zeros_like(x); e[v, c] = 1e-6
+        fd = (orc.collision_energy(x + e, p, k) - orc.collision_energy(x - e, p, k)) / 2e-6
+        assert np.isclose(fd, g[v, c], rtol=1e-7, atol=1e-9)
+
+
+def test_step_with_collisions_pulls_flagged_vertices_to_their_targets(rbc162):
+    ct, td = rbc162
+    x = ct.rest_positions[None]
+    k = np.zeros((1, td.n)); flagged = [3, 40, 41, 90]; k[0, flagged] = 400.0
+    targets = x + np.array([0.0, 0.0, 0.02])                      # push the flagged vertices 20 nm up
+    f = np.zeros_like(x)
+    xa, _ = orc.step(x, 0 * x, f, td, 10)                          # rest state: nothing moves (pin P1)
+    assert np.abs(xa - x).max() < 1e-10
+    xb, _, hist = orc.step(x, 0 * x, f, td, 40, collisions=(targets, k), record=True)
+    obj = np.array(hist["objective"])[:, 0]
+    assert np.all(np.diff(obj) <= 1e-12 * np.abs(obj[:-1]).max())  # the constant-H~ iteration still descends (R19)
+    moved = (xb - x)[0, :, 2]
+    assert np.all(moved[flagged] > 1e-4) and moved[flagged].min() > 5 * np.abs(np.delete(moved, flagged)).mean()
+    # k = 0 everywhere is exactly the plain step
+    xc, _ = orc.step(x, 0 * x, f, td, 10, collisions=(targets, 0 * k))
+    assert np.array_equal(xc, xa)

@@ -328,3 +328,58 @@ def test_median_filtered_forces_and_velocity_cap(precision):
         assert rel_l2(xs[t] - x0, xr - x0) <= TOL_DISP[precision]
         assert rel_l2(vs[t], vr) <= TOL_DISP[precision]
         assert np.linalg.norm(vs[t], axis=-1).max() <= v_max * (1 + 1e-6)
+
+
+@pytest.mark.parametrize("precision,where", [("fp64", "device"), ("fp32", "host")])
+def test_collision_term_matches_oracle(precision, where):
+    """PIK collision energy 1/2 k |x - p|^2 on flagged vertices in the
+    gradient and in the objective, mixed cell types, a subset of the cells in contact."""
+    import torch
+    from oracle import npfem_oracle as orc
+    from paper_1911_03062_b200 import Solver, binding
+    pop = make_config(3, n_cells=23)
+    rng = np.random.default_rng(31)
+    n_steps, n_its = 2, 6
+    targets, stiff = [], []
+    for t, ct in enumerate(pop.types):
+        k = np.where(rng.random(pop.positions[t].shape[:2]) < 0.15, rng.uniform(20, 300, pop.positions[t].shape[:2]), 0.0)
+        k[::2] = 0.0                                              # every other cell is not in contact at all
+        targets.append(pop.positions[t] + 0.02 * rng.standard_normal(pop.positions[t].shape))
+        stiff.append(k)
+    np_io = np.float64 if precision == "fp64" else np.float32
+    solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision=precision)
+    solver.set_option(binding.OPT_DIAGNOSTICS, 1)
+    solver.set_state(torch.from_numpy(pop.packed(pop.positions)).cuda())
+    tg, kk = pop.packed(targets), pop.packed([k[..., None].repeat(3, -1) for k in stiff])[::3].copy()
+    if where == "device":
+        solver.set_collisions(torch.from_numpy(tg).cuda(), torch.from_numpy(kk).cuda())
+    else:
+        solver.set_collisions(tg.astype(np.float64), kk.astype(np.float64))
+    for s in range(n_steps):
+        solver.set_forces(torch.from_numpy(pop.packed(pop.forces(s), dtype=np_io)).cuda())
+        solver.step(n_its)
+    x, v = solver.get_state()
+    hist, mono = solver.get_objective()
+    xs = pop.unpack(x.cpu().numpy())
+    for t, ct in enumerate(pop.types):
+        td = orc.make_type(ct, pop.dt)
+        col = (targets[t], stiff[t])
+        xr, vr = orc.run(pop.positions[t], pop.velocities[t], lambda s, t=t: pop.forces(s)[t], td, n_steps, n_its, collisions=col)
+        x_plain, _ = orc.run(pop.positions[t], pop.velocities[t], lambda s, t=t: pop.forces(s)[t], td, n_steps, n_its)
+        x0 = pop.positions[t]
+        assert rel_l2(xr - x0, x_plain - x0) > 0.05               # the contacts matter
+        print(precision, ct.name, rel_l2(xs[t], xr), rel_l2(xs[t] - x0, xr - x0))
+        assert rel_l2(xs[t], xr) <= TOL_POS[precision]
+        assert rel_l2(xs[t] - x0, xr - x0) <= TOL_DISP[precision]
+    # objective of the last step (diagnostics) includes the collision energy
+    t = 0
+    td = orc.make_type(pop.types[t], pop.dt)
+    xr1, vr1 = orc.run(pop.positions[t], pop.velocities[t], lambda s: pop.forces(s)[t], td, 1, n_its, collisions=(targets[t], stiff[t]))
+    _, _, rec = orc.step(xr1, vr1, pop.forces(1)[t], td, n_its, record=True, collisions=(targets[t], stiff[t]))
+    ref = np.array(rec["objective"])
+    ids = np.nonzero(pop.type_of_cell == t)[0]
+    scale = np.abs(ref).max()
+    assert np.abs(hist[:, ids] - ref).max() < (1e-8 if precision == "fp64" else 5e-3) * scale
+    # clearing restores the plain step
+    solver.clear_collisions()
+    solver.close()
