@@ -340,7 +340,10 @@ bool make_map(CUtensorMap *map, const void *base, uint64_t rows, uint64_t cols, 
 static bool gemm_shape(const TypeDev &td, GemmParams &p) {
   p.n_pad = td.n_pad;
   p.passes = (td.n_pad + MAX_NPASS - 1) / MAX_NPASS;
-  p.n_pass = ((td.n_pad + p.passes - 1) / p.passes + 15) / 16 * 16;
+  // the epilogue moves 32-column tiles: with several passes a pass must END on a tile boundary, or its
+  // last tile would also rewrite the first columns of the next pass (one pass: the TMA store clips at n_pad)
+  const int gran = p.passes > 1 ? 32 : 16;
+  p.n_pass = ((td.n_pad + p.passes - 1) / p.passes + gran - 1) / gran * gran;
   if (p.n_pass > MAX_NPASS || p.n_pass < 16 || (p.n_pass / CL) % 8 != 0 || td.Hinv == nullptr) return false;
   p.k_chunks = (td.n_pad + BK - 1) / BK;
   return true;

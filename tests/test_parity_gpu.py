@@ -383,3 +383,12 @@ def test_collision_term_matches_oracle(precision, where):
     # clearing restores the plain step
     solver.clear_collisions()
     solver.close()
+
+
+@pytest.mark.parametrize("precision", ["fp32", "fp64"])
+def test_paper_resolution_meshes_config6(precision):
+    """the paper's own resolutions (octahedral RBC-258 / PLT-66), its
+    per-GPU load of 114 cells and h = 0.25 us; valence-4 vertices, 2 overflow vertices on a 256-thread CTA."""
+    pop = make_config(6)
+    assert [ct.n_vertices for ct in pop.types] == [258, 66] and pop.n_cells == 114 and pop.dt == 0.25
+    _check(pop, precision, n_steps=4, n_iterations=5)

@@ -58,3 +58,22 @@ def test_rigid_placement_preserves_shape():
         x = pop.positions[0][c]
         assert np.allclose(np.linalg.norm(x[1:] - x[:-1], axis=1), d_rest, rtol=1e-12)
     assert np.all(pop.positions[0].mean(axis=1) >= -1e-9)
+
+
+def test_octahedral_meshes_of_the_paper():
+    """RBC 258 / platelet 66 surface vertices = octahedron subdivided 3 / 2 times."""
+    import numpy as np
+    from workloads import make_config, octasphere
+    for level, n in ((2, 66), (3, 258)):
+        v, f = octasphere(level)
+        assert v.shape == (n, 3) and f.shape == (8 * 4 ** level, 3)
+        assert np.allclose(np.linalg.norm(v, axis=1), 1.0)
+        val = np.bincount(f.ravel())
+        assert sorted(set(val)) == [4, 6] and np.sum(val == 4) == 6
+        # closed and consistently oriented: every directed edge once, its twin present
+        edges = {(a, b) for t in f for a, b in ((t[0], t[1]), (t[1], t[2]), (t[2], t[0]))}
+        assert len(edges) == 3 * len(f) and all((b, a) in edges for a, b in edges)
+        nrm = np.cross(v[f[:, 1]] - v[f[:, 0]], v[f[:, 2]] - v[f[:, 0]])
+        assert np.all(np.sum(nrm * (v[f[:, 0]] + v[f[:, 1]] + v[f[:, 2]]), axis=1) > 0)      # outward
+    pop = make_config(6)
+    assert pop.n_cells == 114 and int(np.sum(pop.type_of_cell == 1)) == 19

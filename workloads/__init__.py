@@ -11,6 +11,7 @@ from .meshes import (  # noqa: F401
     Material,
     icosahedron,
     icosphere,
+    octasphere,
     rbc_material,
     platelet_material,
     rbc_cell_type,

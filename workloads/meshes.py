@@ -130,6 +130,33 @@ def icosphere(level: int) -> tuple[np.ndarray, np.ndarray]:
     return np.array(verts, dtype=np.float64), f
 
 
+def octasphere(level: int) -> tuple[np.ndarray, np.ndarray]:
+    """Octahedron subdivided `level` times onto the unit sphere: V = 4*4^L + 2 (66 at L = 2, 258 at L = 3,
+    the paper's platelet / RBC resolutions), T = 8*4^L."""
+    verts = [(1.0, 0, 0), (-1.0, 0, 0), (0, 1.0, 0), (0, -1.0, 0), (0, 0, 1.0), (0, 0, -1.0)]
+    f = np.array([(0, 2, 4), (2, 1, 4), (1, 3, 4), (3, 0, 4), (2, 0, 5), (1, 2, 5), (3, 1, 5), (0, 3, 5)], dtype=np.int32)
+    for _ in range(level):
+        cache: dict[tuple[int, int], int] = {}
+
+        def midpoint(a: int, b: int) -> int:
+            key = (a, b) if a < b else (b, a)
+            idx = cache.get(key)
+            if idx is None:
+                m = 0.5 * (np.asarray(verts[a], dtype=np.float64) + np.asarray(verts[b], dtype=np.float64))
+                m /= np.linalg.norm(m)
+                idx = len(verts)
+                verts.append(tuple(m))
+                cache[key] = idx
+            return idx
+
+        new_f = []
+        for a, b, c in f:
+            ab, bc, ca = midpoint(a, b), midpoint(b, c), midpoint(c, a)
+            new_f += [(a, ab, ca), (b, bc, ab), (c, ca, bc), (ab, bc, ca)]
+        f = np.array(new_f, dtype=np.int32)
+    return np.array(verts, dtype=np.float64), f
+
+
 # Evans-Fung biconcave profile constants (literature values, not in PAPER.md; reading R14)
 _EF_C0, _EF_C1, _EF_C2 = 0.207161, 2.002558, -1.122762
 RBC_RADIUS_UM = 3.91
@@ -145,8 +172,8 @@ def evans_fung_map(unit_points: np.ndarray, radius: float = RBC_RADIUS_UM) -> np
     return np.stack([x, y, z], axis=1)
 
 
-def rbc_cell_type(level: int = 3, material: Material | None = None) -> CellType:
-    v, f = icosphere(level)
+def rbc_cell_type(level: int = 3, material: Material | None = None, base: str = "ico") -> CellType:
+    v, f = icosphere(level) if base == "ico" else octasphere(level)
     return CellType(
         name=f"RBC-{v.shape[0]}",
         rest_positions=np.ascontiguousarray(evans_fung_map(v)),
@@ -158,8 +185,8 @@ def rbc_cell_type(level: int = 3, material: Material | None = None) -> CellType:
 PLATELET_SEMI_AXES_UM = (1.8, 1.8, 0.5)
 
 
-def platelet_cell_type(level: int = 2, material: Material | None = None) -> CellType:
-    v, f = icosphere(level)
+def platelet_cell_type(level: int = 2, material: Material | None = None, base: str = "ico") -> CellType:
+    v, f = icosphere(level) if base == "ico" else octasphere(level)
     return CellType(
         name=f"PLT-{v.shape[0]}",
         rest_positions=np.ascontiguousarray(v * np.asarray(PLATELET_SEMI_AXES_UM)),

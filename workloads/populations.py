@@ -24,6 +24,8 @@ CONFIG_NAMES = {
     3: "20,000 RBC-642 + 2,000 PLT-162 at 35% Hct, shear-like forces, 20 steps x 5 its",
     4: "90,000 RBC-642 + 10,000 PLT-162, shear-like forces, 10 steps x 10 its",
     5: "10,000 RBC-2562, N(0,1 pN) forces, 10 steps x K its",
+    6: "the paper's own per-GPU load: 95 RBC-258 + 19 PLT-66 (octahedral meshes), h = 0.25 us, shear-like forces, "
+       "20 steps x 5 its",
 }
 
 
@@ -168,9 +170,13 @@ class Population:
 
 
 def make_config(index: int, n_cells: int | None = None, level: int | None = None) -> Population:
-    """Build BASELINE.json config `index` (1..5); `n_cells` shrinks it, keeping the recipe."""
+    """Build BASELINE.json config `index` (1..5); `n_cells` shrinks it, keeping the recipe.
+    Index 6 is not a BASELINE config: the paper's own resolutions and per-GPU load:
+    RBC 258 / platelet 66 surface vertices, PLT:RBC = 1:5, 571 cells of the 50^3 um^3
+    domain over 5 GPU nodes = 114 cells per GPU, solid step = 2 LBM steps = 0.25 us
+    (PAPER.md:45, :230)."""
     if index not in CONFIG_NAMES:
-        raise ValueError(f"config index must be 1..5, got {index}")
+        raise ValueError(f"config index must be 1..6, got {index}")
     seed = np.random.SeedSequence(index - 1)          # seeds 0..4 (SURVEY.md 8(d))
     s_rot, s_trans, s_force = seed.spawn(3)
     dt = 0.1                                           # 1e-7 s
@@ -189,9 +195,13 @@ def make_config(index: int, n_cells: int | None = None, level: int | None = None
         total, period, box, steps, its = 100000, 10, (289.0,) * 3, 10, 10
         types = [rbc_cell_type(3), platelet_cell_type(2)]
         sigma, gamma = 0.2, 0.02
-    else:
+    elif index == 5:
         total, period, box, steps, its = 10000, 0, (139.0,) * 3, 10, 10
         types = [rbc_cell_type(level if level is not None else 4)]
+    else:
+        total, period, box, steps, its = 114, 6, (50.0, 50.0, 10.0), 20, 5
+        types = [rbc_cell_type(3, base="octa"), platelet_cell_type(2, base="octa")]
+        sigma, gamma, redraw, dt = 0.2, 0.02, True, 0.25
     if n_cells is not None:
         total = int(n_cells)
     type_of_cell = np.zeros(total, dtype=np.int32)
