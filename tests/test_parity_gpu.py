@@ -392,3 +392,49 @@ def test_paper_resolution_meshes_config6(precision):
     pop = make_config(6)
     assert [ct.n_vertices for ct in pop.types] == [258, 66] and pop.n_cells == 114 and pop.dt == 0.25
     _check(pop, precision, n_steps=4, n_iterations=5)
+
+
+def _sampled_full_size(config, precision, n_steps, n_iterations, samples_per_type=6):
+    """BASELINE.json full size in the launch configuration bench.py times; the oracle recomputes a seeded
+    sample of cells one by one (cells are independent: PAPER.md:61, :63), first and last slot included."""
+    import torch
+    from oracle import npfem_oracle as orc
+    from paper_1911_03062_b200 import Solver
+    pop = make_config(config)
+    solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision=precision)
+    solver.set_state(torch.from_numpy(pop.packed(pop.positions)).cuda())
+    np_io = np.float32 if precision == "fp32" else np.float64
+    for s in range(n_steps):
+        solver.set_forces(torch.from_numpy(pop.packed(pop.forces(s), dtype=np_io)).cuda())
+        solver.step(n_iterations)
+    rng = np.random.default_rng(100 + config)
+    rows = []
+    for t, ct in enumerate(pop.types):
+        ids = pop.cells_of_type(t)
+        if ids.size == 0:
+            continue
+        slots = np.unique(np.concatenate(([0, ids.size - 1], rng.integers(0, ids.size, samples_per_type))))
+        x, v = solver.get_state(cell_ids=ids[slots])
+        xg = x.cpu().numpy().reshape(slots.size, ct.n_vertices, 3)
+        vg = v.cpu().numpy().reshape(slots.size, ct.n_vertices, 3)
+        td = orc.make_type(ct, pop.dt)
+        x0 = pop.positions[t][slots]
+        xr, vr = orc.run(x0, pop.velocities[t][slots], lambda s, t=t: pop.forces(s)[t][slots], td, n_steps, n_iterations)
+        rows.append((ct.name, rel_l2(xg, xr), rel_l2(xg - x0, xr - x0), rel_l2(vg, vr)))
+    solver.close()
+    return rows
+
+
+def test_full_size_config4_100k_cells_sampled():
+    """BASELINE configs[3] at its full 100,000 cells, fp32, default kernels (what bench.py times)."""
+    for name, pos, disp, vel in _sampled_full_size(4, "fp32", n_steps=2, n_iterations=10):
+        print(name, pos, disp, vel)
+        assert pos <= TOL_POS["fp32"] and disp <= TOL_DISP["fp32"] and vel <= TOL_DISP["fp32"]
+
+
+@pytest.mark.parametrize("precision", ["fp32", "fp64"])
+def test_full_size_config5_10k_level4_cells_sampled(precision):
+    """BASELINE configs[4] at its full 10,000 RBC-2562 cells (generic local step, 11-pass GEMM)."""
+    for name, pos, disp, vel in _sampled_full_size(5, precision, n_steps=1, n_iterations=5, samples_per_type=3):
+        print(name, pos, disp, vel)
+        assert pos <= TOL_POS[precision] and disp <= TOL_DISP[precision] and vel <= TOL_DISP[precision]
