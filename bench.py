@@ -42,7 +42,7 @@ def parse_args():
     ap.add_argument("--global-math", default="tf32", choices=["tf32", "fp32"])
     ap.add_argument("--update-mode", type=int, default=0, choices=[0, 1, 2],
                     help="0 auto, 1 GEMM epilogue updates d in place, 2 product-out applied by the next local step")
-    ap.add_argument("--local-impl", type=int, default=0, choices=[0, 1, 2, 3])
+    ap.add_argument("--local-impl", type=int, default=0, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--line-search", type=int, default=0, help="Armijo backtracking with this many halvings (0 = off)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

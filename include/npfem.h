@@ -65,7 +65,8 @@ extern "C" {
 #define NPFEM_OPT_DIAGNOSTICS      1  /* 1: record the objective before every iteration (row a5) */
 #define NPFEM_OPT_GLOBAL_STEP_MATH 2  /* fp32 contexts: 0 = TF32 tensor cores (default), 1 = FP32 FFMA */
 #define NPFEM_OPT_LOCAL_STEP_IMPL  3  /* 0 = auto, 1 = generic kernel, 2 = shared-memory persistent kernel,
-                                         3 = scheduled kernel (register-resident topology, conflict-free slots) */
+                                         3 = scheduled kernel (register-resident topology, conflict-free slots),
+                                         4 = large-mesh kernel (chunked corner forces, e.g. 2562-vertex cells) */
 
 #define NPFEM_OPT_KERNEL_TIMING    4  /* 1: bracket every kernel of npfem_step with CUDA events */
 #define NPFEM_OPT_FORCE_MEDIAN_FILTER 6  /* 1: npfem_set_forces median-filters F_ext over the one-ring of every vertex

@@ -548,7 +548,7 @@ int npfem_set_option(npfem_ctx *c, int32_t option, int64_t value) {
       c->opt_global_math = value;
       return NPFEM_OK;
     case NPFEM_OPT_LOCAL_STEP_IMPL:
-      if (value < 0 || value > 3) return fail(c, NPFEM_EINVAL, "local-step impl must be 0, 1, 2 or 3");
+      if (value < 0 || value > 4) return fail(c, NPFEM_EINVAL, "local-step impl must be 0 ... 4");
       c->opt_local_impl = value;
       return NPFEM_OK;
     case NPFEM_OPT_KERNEL_TIMING: c->timing = value != 0; return NPFEM_OK;
@@ -717,11 +717,13 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
     for (size_t t = 0; t < nb; ++t) {
       const bool f32 = c->precision == NPFEM_F32 && !ls_on;   // the line search needs the FULL gradient: generic kernel
       const bool sched = f32 && (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]);
-      const bool fast = f32 && !sched && c->opt_local_impl != 1 && local_smem_supported(c->types[t]);
-      const double d_scale = (sched || fast) ? 1.0 - c->types[t].gamma : 1.0;
+      const bool fast = f32 && !sched && (c->opt_local_impl == 0 || c->opt_local_impl == 2) && local_smem_supported(c->types[t]);
+      const bool big = f32 && !sched && !fast && (c->opt_local_impl == 0 || c->opt_local_impl == 4) && local_big_supported(c->types[t]);
+      const double d_scale = (sched || fast || big) ? 1.0 - c->types[t].gamma : 1.0;
       if ((rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "local step", [&] {
              if (sched) return launch_local_sched(c->types[t], c->views[t], c->n_sm, fused[t] && k > 0, d_scale, c->stream);
              if (fast) return launch_local_smem(c->types[t], c->views[t], c->n_sm, c->stream);
+             if (big) return launch_local_big(c->types[t], c->views[t], c->n_sm, c->stream);
              return launch_local_generic(c->types[t], c->views[t], c->buckets[t].scratch, c->precision, c->n_sm,
                                          c->stream); })))
         return rc;

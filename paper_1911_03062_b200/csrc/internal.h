@@ -155,6 +155,10 @@ bool local_sched_supported(const TypeDev &td);
 int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, bool apply_u, double d_scale,
                        cudaStream_t s);
 
+// fp32 reduced-gradient local step for types too large for the scheduled kernel (chunked corner forces)
+bool local_big_supported(const TypeDev &td);
+int launch_local_big(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
+
 int launch_monotone_flags(const double *history, int n_entries, int64_t cells, int32_t *flags, cudaStream_t s);
 
 }  // namespace npfem

@@ -46,10 +46,12 @@ def test_config3_mixed_types_redrawn_forces(precision):
     _check(pop, precision, n_steps=4, n_iterations=5)
 
 
-@pytest.mark.parametrize("precision", ["fp32", "fp64"])
-def test_config5_level4_mesh(precision):
-    # 2562 vertices: the shared-memory budget is exceeded -> global-scratch variant of the local step
-    _check(make_config(5, n_cells=3), precision, n_steps=2, n_iterations=3)
+@pytest.mark.parametrize("precision,impl", [("fp32", 0), ("fp32", 1), ("fp32", 4), ("fp64", 0)])
+def test_config5_level4_mesh(precision, impl):
+    # 2562 vertices / 5120 triangles: too large for the scheduled kernel -> large-mesh kernel (fp32 default,
+    # corner forces in chunks) or the generic kernel with its global scratch (impl 1, fp64)
+    from paper_1911_03062_b200 import binding
+    _check(make_config(5, n_cells=40), precision, n_steps=2, n_iterations=3, options=[(binding.OPT_LOCAL_STEP_IMPL, impl)])
 
 
 def test_icosahedron_cell_fp64():
