@@ -7,14 +7,17 @@
 // the path where tensor cores apply.  Increment form keeps TF32 safe: the rounding lands on the
 // small update g W, not on d.
 //
-// Kernel: persistent, one CTA per SM, warp-specialised.
-//   warp 0   TMA producer : G tile [128 x 32 fp32] and W tile [N_pass x 32] per K chunk, 128B swizzle
-//   warp 1   MMA issuer   : tcgen05.mma.cta_group::1.kind::tf32, M = 128, N <= 256 per instruction,
-//                           accumulators for N_pass <= 512 columns in TMEM; A negated in the
-//                           instruction descriptor so the accumulator is -G W
-//   warps 2-5 epilogue    : tcgen05.ld -> d += acc (vectorised read-modify-write of the d tile)
-// Work item = (M tile, N pass); a CTA takes consecutive items so the G tile of pass 2 is an L2 hit,
-// and the producer runs ahead into the next item while the epilogue drains TMEM.
+// Kernel: persistent, one CTA per SM in clusters of CL = 2, warp-specialised.
+//   warp 0   TMA producer : own G tile [128 x 32 fp32] + this CTA's 1/CL of the W tile [N_pass x 32],
+//                           multicast to every CTA of the cluster, per K chunk; 128B swizzle; ring of up to
+//                           4 stages sized per launch
+//   warp 1   MMA issuer   : tcgen05.mma.cta_group::1.kind::tf32, M = 128, N = N_pass <= 256, two accumulators
+//                           in the 512 TMEM columns; A negated in the instruction descriptor (acc = -G W);
+//                           its commit frees the ring slot in every CTA of the cluster
+//   warps 2-5 epilogue    : [32 x 32] tiles: TMA load of d into swizzled shared memory -> tcgen05.ld ->
+//                           d_scale d + acc in place (row per lane, conflict-free) -> TMA store
+// Work item of a cluster = (CL consecutive M tiles, N pass); the passes of one group are adjacent items
+// (neighbouring clusters at about the same time), so the repeated G reads are L2 hits.
 #include <cuda.h>
 
 #include "internal.h"

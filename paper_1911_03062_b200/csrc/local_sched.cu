@@ -14,15 +14,16 @@
 //   * membrane gradient from the metric G = [e_i . e_j]:  I1 + 1 = tr(R G) - 1,
 //     I2 = det(Dm^-1)^2 |e1 x e2|^2 - 1,  [g1 g2] = [e1 e2] Q,  Q = 2 A0 (W1 R + W2 det^2 adj G);
 //   * hinges from UNIT normals stored once per triangle (1 rsqrt per triangle instead of 3);
-//   * cell volume: per-warp float partial -> fixed-point shared atomics on two 32-bit digits
-//     (exact, order independent, deterministic);
+//   * cell volume in fixed point: one REDUX per warp + integer shared atomics (exact, order
+//     independent, deterministic);
 //   * x_n, d, b of the next cells stream in through 1-D TMA bulk copies (cp.async.bulk + mbarrier)
-//     into a NSTAGE-deep ring, issued NSTAGE-1 cells ahead.
-// Phases per cell (3 block barriers):
-//   0  stage -> sx[slot(v)] = (x_n + d, 0)                                           | barrier 1
-//   A  per triangle: e1, e2, unit normal, 1/|N| -> sN[slot(t)]; volume partial       | barrier 2
-//   B  per triangle: membrane + 3 hinge sides + volume term -> 3 corner forces in sC | barrier 3
-//   C  per vertex: gather <= MAXV corner forces, r = coef d - b + sum -> global
+//     into a NSTAGE-deep ring, issued NSTAGE-1 cells ahead;
+//   * the block barriers are mbarriers with early arrive / late wait (software pipeline across cells),
+//     and no single warp carries extra serial work (TMA issue, overflow vertices: different warps).
+// Per cell:  wait B1 | A: edges, unit normal, 1/|N| -> sN; volume partial | arrive B2, BV | membrane |
+//   wait B2 | hinges | wait BV | corner forces -> sC | arrive B3 | phase 0 of the NEXT cell:
+//   sx[slot(v)] = (x_n + d, 0) | arrive B1 | wait B3 | C: gather <= MAXV corner forces,
+//   r = coef d - b + sum -> global.
 #include "internal.h"
 
 namespace npfem {
