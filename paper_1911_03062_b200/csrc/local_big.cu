@@ -52,6 +52,15 @@ __global__ void __launch_bounds__(THREADS, 1) local_big_kernel(const BigParams p
   for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x) {
     const size_t base = size_t(cell) * 3 * n_pad;
     const float *xg = p.x + base, *dg = p.d + base, *bg = p.b + base;
+    {   // pull the NEXT cell's x, d, b towards L2 while this one is computed (one 128-byte line per thread)
+      const int64_t nxt = cell + gridDim.x;
+      const int lines = (3 * n_pad * 4 + 127) / 128;
+      if (nxt < p.cells)
+        for (int l = tid; l < 3 * lines; l += THREADS) {
+          const float *f = (l < lines ? p.x : (l < 2 * lines ? p.d : p.b)) + size_t(nxt) * 3 * n_pad;
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(f) + size_t(l % lines) * 128));
+        }
+    }
     // ---- phase 0 ----------------------------------------------------------------------------
     for (int i = tid; i < n; i += THREADS)
       sx[i] = make_float4(xg[i] + dg[i], xg[n_pad + i] + dg[n_pad + i], xg[2 * n_pad + i] + dg[2 * n_pad + i], 0.f);
@@ -85,9 +94,28 @@ __global__ void __launch_bounds__(THREADS, 1) local_big_kernel(const BigParams p
     for (int r = 0; r < VPT; ++r) acc[r][0] = acc[r][1] = acc[r][2] = 0.f;
     for (int t0 = 0; t0 < nt; t0 += tc) {
       const int t1 = min(t0 + tc, nt);
-      for (int t = t0 + tid; t < t1; t += THREADS) {
-        const uint4 pk = __ldg(p.tri_pack + t);
-        const float4 rest = __ldg(p.tri_rest + t);
+      // the per-type tables come from L2: the next triangle's entries are requested before this one is
+      // worked on (one L2 latency per chunk instead of one per triangle)
+      int t = t0 + tid;
+      uint4 pk_n = make_uint4(0, 0, 0, 0);
+      float4 rest_n = make_float4(0.f, 0.f, 0.f, 0.f);
+      float2 h_n[3] = {};
+      if (t < t1) {
+        pk_n = __ldg(p.tri_pack + t);
+        rest_n = __ldg(p.tri_rest + t);
+#pragma unroll
+        for (int sd = 0; sd < 3; ++sd) h_n[sd] = __ldg(p.hinge_rest + 3 * t + sd);
+      }
+      for (; t < t1; t += THREADS) {
+        const uint4 pk = pk_n;
+        const float4 rest = rest_n;
+        const float2 hh[3] = {h_n[0], h_n[1], h_n[2]};
+        if (t + THREADS < t1) {
+          pk_n = __ldg(p.tri_pack + t + THREADS);
+          rest_n = __ldg(p.tri_rest + t + THREADS);
+#pragma unroll
+          for (int sd = 0; sd < 3; ++sd) h_n[sd] = __ldg(p.hinge_rest + 3 * (t + THREADS) + sd);
+        }
         const float4 X0 = sx[pk.x & 0xffffu], X1 = sx[pk.x >> 16], X2 = sx[pk.y & 0xffffu];
         const float4 NA = sN[t];
         const float a = rest.x, b = rest.y, c = rest.z, A0 = rest.w;
@@ -110,7 +138,7 @@ __global__ void __launch_bounds__(THREADS, 1) local_big_kernel(const BigParams p
 #pragma unroll
         for (int s = 0; s < 3; ++s) {
           const float4 NB = sN[nbr[s]];
-          const float2 h0 = __ldg(p.hinge_rest + 3 * t + s);
+          const float2 h0 = hh[s];
           const float ex = s == 0 ? e1[0] : (s == 1 ? e2[0] - e1[0] : -e2[0]);
           const float ey = s == 0 ? e1[1] : (s == 1 ? e2[1] - e1[1] : -e2[1]);
           const float ez = s == 0 ? e1[2] : (s == 1 ? e2[2] - e1[2] : -e2[2]);
