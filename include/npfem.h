@@ -71,6 +71,8 @@ extern "C" {
 #define NPFEM_OPT_KERNEL_TIMING    4  /* 1: bracket every kernel of npfem_step with CUDA events */
 #define NPFEM_OPT_FORCE_MEDIAN_FILTER 6  /* 1: npfem_set_forces median-filters F_ext over the one-ring of every vertex
                                             (per component, vertex + neighbours, even counts average) */
+#define NPFEM_OPT_FUSED_STEP       7  /* whole step of a cell in ONE kernel (fp32, small batches): 0 = auto (a bucket of at
+                                         most 1.5 cells per SM), 1 = never, 2 = whenever the cell type allows it */
 #define NPFEM_OPT_UPDATE_MODE      5  /* fp32 tensor-core global step: 0 = auto (= 1), 1 = the GEMM epilogue updates d in place,
                                          2 = the GEMM writes its product, the next local step applies it */
 
@@ -80,7 +82,8 @@ extern "C" {
 #define NPFEM_KIND_GLOBAL   2
 #define NPFEM_KIND_EPILOGUE 3
 #define NPFEM_KIND_LINE_SEARCH 4   /* objective evaluations + accept / backtrack kernels */
-#define NPFEM_KIND_COUNT    5
+#define NPFEM_KIND_FUSED_STEP  5   /* whole-step kernel of the small-batch path */
+#define NPFEM_KIND_COUNT    6
 
 #define NPFEM_MAX_ITERATIONS 256
 

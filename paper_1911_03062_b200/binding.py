@@ -15,7 +15,8 @@ NPFEM_F32, NPFEM_F64 = 32, 64
 NPFEM_DEVICE, NPFEM_HOST = 0, 1
 OPT_DIAGNOSTICS, OPT_GLOBAL_STEP_MATH, OPT_LOCAL_STEP_IMPL, OPT_KERNEL_TIMING, OPT_UPDATE_MODE = 1, 2, 3, 4, 5
 OPT_FORCE_MEDIAN_FILTER = 6
-KIND_NAMES = ("prologue", "local", "global", "epilogue", "line_search")
+OPT_FUSED_STEP = 7
+KIND_NAMES = ("prologue", "local", "global", "epilogue", "line_search", "fused_step")
 _ERR_NAMES = {-1: "NPFEM_EINVAL", -2: "NPFEM_EMESH", -3: "NPFEM_ECUDA", -4: "NPFEM_ENOMEM", -5: "NPFEM_ESTATE"}
 
 EXPORTED_SYMBOLS = (

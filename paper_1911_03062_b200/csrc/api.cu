@@ -43,7 +43,7 @@ struct npfem_ctx {
   bool diagnostics = false;
   double *history_dev = nullptr;
   int history_cap = 0, history_entries = 0;
-  int64_t opt_global_math = 0, opt_local_impl = 0, opt_update_mode = 0;
+  int64_t opt_global_math = 0, opt_local_impl = 0, opt_update_mode = 0, opt_fused_step = 0;
   // line search (npfem_set_line_search)
   int ls_max_halvings = 0;
   double ls_c1 = 1e-4, ls_tol = 0.0;
@@ -553,6 +553,10 @@ int npfem_set_option(npfem_ctx *c, int32_t option, int64_t value) {
       return NPFEM_OK;
     case NPFEM_OPT_KERNEL_TIMING: c->timing = value != 0; return NPFEM_OK;
     case NPFEM_OPT_FORCE_MEDIAN_FILTER: c->median_filter = value != 0; return NPFEM_OK;
+    case NPFEM_OPT_FUSED_STEP:
+      if (value < 0 || value > 2) return fail(c, NPFEM_EINVAL, "fused-step option must be 0, 1 or 2");
+      c->opt_fused_step = value;
+      return NPFEM_OK;
     case NPFEM_OPT_UPDATE_MODE:
       if (value < 0 || value > 2) return fail(c, NPFEM_EINVAL, "update mode must be 0, 1 or 2");
       c->opt_update_mode = value;
@@ -678,8 +682,20 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
     return NPFEM_OK;
   };
   if (c->spans.size() > 200000 && (rc = drain_spans(c))) return rc;
+  // Small-batch path: a bucket with only a few cells per SM runs its whole step in one
+  // kernel, one CTA per cell (step_fused.cu); everything else goes through the batched kernels below.
+  std::vector<char> whole(nb, 0);
+  for (size_t t = 0; t < nb; ++t) {
+    const bool plain = c->precision == NPFEM_F32 && !c->diagnostics && c->ls_max_halvings == 0 && !c->col_active &&
+                       c->opt_local_impl == 0 && c->opt_global_math == 0 && c->opt_update_mode != 2;
+    whole[t] = plain && c->opt_fused_step != 1 && step_fused_supported(c->types[t]) &&
+               (c->opt_fused_step == 2 || 2 * c->buckets[t].cells <= int64_t(3) * c->n_sm);
+    if (whole[t] && (rc = timed_launch(c, NPFEM_KIND_FUSED_STEP, int(t), "fused step", [&] {
+                       return launch_step_fused(c->types[t], c->views[t], c->n_sm, n_iterations, c->v_max, c->stream); })))
+      return rc;
+  }
   for (size_t t = 0; t < nb; ++t)
-    if ((rc = timed_launch(c, NPFEM_KIND_PROLOGUE, int(t), "prologue", [&] {
+    if (!whole[t] && (rc = timed_launch(c, NPFEM_KIND_PROLOGUE, int(t), "prologue", [&] {
            return launch_prologue(c->types[t], c->views[t], c->precision, c->stream); })))
       return rc;
   // Product-out mode (NPFEM_OPT_UPDATE_MODE = 2; fp32, scheduled local step + tensor-core global step,
@@ -715,6 +731,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   for (int k = 0; k < n_iterations; ++k) {
     if (c->diagnostics && (rc = diag(k))) return rc;
     for (size_t t = 0; t < nb; ++t) {
+      if (whole[t]) continue;
       const bool f32 = c->precision == NPFEM_F32 && !ls_on;   // the line search needs the FULL gradient: generic kernel
       const bool sched = f32 && (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]);
       const bool fast = f32 && !sched && (c->opt_local_impl == 0 || c->opt_local_impl == 2) && local_smem_supported(c->types[t]);
@@ -768,7 +785,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   }
   if (c->diagnostics && (rc = diag(n_iterations))) return rc;
   for (size_t t = 0; t < nb; ++t)
-    if ((rc = timed_launch(c, NPFEM_KIND_EPILOGUE, int(t), "epilogue", [&] {
+    if (!whole[t] && (rc = timed_launch(c, NPFEM_KIND_EPILOGUE, int(t), "epilogue", [&] {
            return launch_epilogue(c->types[t], c->views[t], c->precision, fused[t] != 0, 1.0 - c->types[t].gamma,
                                   c->v_max, c->stream); })))
       return rc;

@@ -159,6 +159,10 @@ int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, bool a
 bool local_big_supported(const TypeDev &td);
 int launch_local_big(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
 
+// whole time step of a cell in one kernel (small batches; step_fused.cu)
+bool step_fused_supported(const TypeDev &td);
+int launch_step_fused(const TypeDev &td, const BucketView &bv, int n_sm, int n_iterations, double v_max, cudaStream_t s);
+
 int launch_monotone_flags(const double *history, int n_entries, int64_t cells, int32_t *flags, cudaStream_t s);
 
 }  // namespace npfem

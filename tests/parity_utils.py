@@ -20,14 +20,17 @@ def run_oracle(pop, n_steps=None, n_iterations=None):
     return out
 
 
-def run_gpu(pop, precision, n_steps=None, n_iterations=None, io="fp64", where="device", options=()):
-    """-> per-type (x, v) after the run as fp64 numpy, plus the solver (still open)."""
+def run_gpu(pop, precision, n_steps=None, n_iterations=None, io="fp64", where="device", options=(), fused_step=1):
+    """-> per-type (x, v) after the run as fp64 numpy, plus the solver (still open).
+    fused_step: NPFEM_OPT_FUSED_STEP (1 = batched kernels, the path the large workloads take; 2 = the
+    whole-step kernel of the small-batch path; 0 = the library's own choice by batch size)."""
     import torch
-    from paper_1911_03062_b200 import Solver
+    from paper_1911_03062_b200 import Solver, binding
     n_steps = pop.n_steps if n_steps is None else n_steps
     n_iterations = pop.n_iterations if n_iterations is None else n_iterations
     np_dt = np.float32 if io == "fp32" else np.float64
     solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision=precision)
+    solver.set_option(binding.OPT_FUSED_STEP, fused_step)
     for opt, val in options:
         solver.set_option(opt, val)
 

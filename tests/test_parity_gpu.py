@@ -213,7 +213,7 @@ def test_irregular_mesh_valence_up_to_8(precision, impl):
                      velocities=[0.01 * rng.standard_normal(pos.shape)], dt=0.1, n_steps=3, n_iterations=6,
                      box=(80.0,) * 3, force_sigma=1.0, shear_gamma=0.0, redraw_noise_each_step=False,
                      _force_seed=np.random.SeedSequence(12), _shear_height=[pos[..., 2]])
-    gpu, solver = run_gpu(pop, precision, options=[(binding.OPT_LOCAL_STEP_IMPL, impl)])
+    gpu, solver = run_gpu(pop, precision, options=[(binding.OPT_LOCAL_STEP_IMPL, impl)], fused_step=2 if impl == 0 else 1)
     solver.close()
     ref = run_oracle(pop)
     for r in compare(pop, gpu, ref):
@@ -385,6 +385,38 @@ def test_collision_term_matches_oracle(precision, where):
     # clearing restores the plain step
     solver.clear_collisions()
     solver.close()
+
+
+@pytest.mark.parametrize("config,cells,fused", [(6, None, 2), (6, None, 0), (3, 60, 2), (2, 9, 2)])
+def test_whole_step_fused_kernel(config, cells, fused):
+    """the small-batch path, one kernel per time step and one CTA per cell (prologue, K
+    iterations with the per-cell FP32 product by H~^-1, epilogue), against the oracle: the paper's own
+    load (config 6: forced and auto-selected), mixed RBC-642 / PLT-162 cells, forces redrawn every step."""
+    pop = make_config(config, n_cells=cells)
+    gpu, solver = run_gpu(pop, "fp32", n_steps=4, n_iterations=5, fused_step=fused)
+    times = solver.get_kernel_times(reset=False)
+    solver.close()
+    ref = run_oracle(pop, 4, 5)
+    for r in compare(pop, gpu, ref):
+        print(config, fused, r)
+        assert r["pos"] <= TOL_POS["fp32"] and r["worst_cell_pos"] <= TOL_POS["fp32"], r
+        assert r["disp"] <= TOL_DISP["fp32"] and r["vel"] <= TOL_DISP["fp32"], r
+
+
+def test_whole_step_fused_kernel_is_the_one_that_ran():
+    """The fused path really replaces the batched launches: 1 launch per type and step."""
+    import torch
+    from paper_1911_03062_b200 import Solver, binding
+    pop = make_config(6)
+    for fused, per_step in ((2, 2), (1, 2 * (2 + 2 * 5))):
+        solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision="fp32")
+        solver.set_option(binding.OPT_FUSED_STEP, fused)
+        solver.set_state(torch.from_numpy(pop.packed(pop.positions)).cuda())
+        solver.set_forces(torch.from_numpy(pop.packed(pop.forces(0))).cuda())
+        before = solver.launch_count
+        solver.step(5)
+        assert solver.launch_count - before == per_step
+        solver.close()
 
 
 @pytest.mark.parametrize("precision", ["fp32", "fp64"])
