@@ -473,3 +473,51 @@ def test_full_size_config5_10k_level4_cells_sampled(precision):
     for name, pos, disp, vel in _sampled_full_size(5, precision, n_steps=1, n_iterations=5, samples_per_type=3):
         print(name, pos, disp, vel)
         assert pos <= TOL_POS[precision] and disp <= TOL_DISP[precision] and vel <= TOL_DISP[precision]
+
+
+@pytest.mark.parametrize("kappa", [0.7, 0.8, 0.9])
+def test_kappa_damping_sweep_config6(kappa):
+    """the paper's parameter sweep kappa_damping in {0.5, 0.7, 0.8, 0.9} on its
+    own meshes; 0.5 is the default of every other test.  Batched kernels in fp64, whole-step kernel in fp32."""
+    import dataclasses
+    pop = make_config(6, n_cells=36)
+    pop.types = [dataclasses.replace(ct, material=dataclasses.replace(ct.material, kappa_damping=kappa))
+                 for ct in pop.types]
+    _check(pop, "fp64", n_steps=5, n_iterations=5)
+    _check(pop, "fp32", n_steps=5, n_iterations=5, fused_step=2)
+
+
+@pytest.mark.parametrize("precision", ["fp32", "fp64"])
+def test_static_partition_shards_match_the_unsharded_solver(precision):
+    """cells are independent within a step, so the shards of a
+    static partition, each stepped by its own solver (here one after the other on the one GPU there is),
+    reproduce the unsharded run bit for bit, whatever the batch a cell finds itself in."""
+    import torch
+    from paper_1911_03062_b200 import Solver, binding
+    from paper_1911_03062_b200.partition import ShardedSolver
+    pop = make_config(3, n_cells=45)
+    x0 = pop.packed(pop.positions)
+    forces = [pop.packed(pop.forces(s)) for s in range(3)]
+
+    def factory(types, toc, dt):
+        s = Solver(types, toc, dt, precision=precision)
+        s.set_option(binding.OPT_FUSED_STEP, 1)
+        return s
+
+    whole = ShardedSolver(pop.types, pop.type_of_cell, pop.dt, 0, 1, solver_factory=factory)
+    shards = [ShardedSolver(pop.types, pop.type_of_cell, pop.dt, r, 3, solver_factory=factory) for r in range(3)]
+    assert sorted(int(c) for s in shards for c in s.cell_ids) == list(range(pop.n_cells))
+    for s in [whole] + shards:
+        s.set_state(x0)
+        for f in forces:
+            s.set_forces(f)
+            s.step(5)
+    torch.cuda.synchronize()
+    xw, vw = whole.gather_state()
+    part = shards[0].partition
+    xs = part.assemble([s.local_state()[0] for s in shards])
+    vs = part.assemble([s.local_state()[1] for s in shards])
+    assert np.array_equal(xs, xw) and np.array_equal(vs, vw)
+    assert np.linalg.norm(xw - x0) > 0
+    for s in [whole] + shards:
+        s.solver.close()
