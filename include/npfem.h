@@ -156,6 +156,21 @@ int npfem_set_forces(npfem_ctx *ctx, const int64_t *cell_ids, int64_t n_ids,
  */
 int npfem_step(npfem_ctx *ctx, int32_t n_iterations);
 
+/*
+ * The same time step as npfem_set_forces(all cells) + npfem_step + npfem_get_state(all cells) with HOST
+ * buffers, pipelined: cells are independent within a step, so the population is cut
+ * into `n_chunks` ranges of cell ids (0 = chosen from the buffer size, at most 64); chunk i's solver
+ * kernels run while chunk i+1's forces are copied in and chunk i-1's state is copied out on two copy
+ * streams.  Results are bit-identical to the unpipelined sequence.  `forces` [in], `positions` and
+ * `velocities` [out] are HOST buffers of all cells in cell-id order, each `[n][3]`, dtype `dtype`; use
+ * page-locked memory or the copies do not overlap.  Owned by the caller, not retained.  Synchronous:
+ * returns when the state is in the host buffers.  With diagnostics, line search, collisions or the
+ * median filter on, the three calls run one after the other instead.  Errors: NPFEM_EINVAL (NULL
+ * pointer, n_chunks, n_iterations), NPFEM_ESTATE (cells without state), NPFEM_ECUDA.
+ */
+int npfem_step_host(npfem_ctx *ctx, const void *forces, int32_t n_iterations, void *positions, void *velocities,
+                    int32_t dtype, int32_t n_chunks);
+
 /* Current {x, v} of the listed cells (either pointer may be NULL). */
 int npfem_get_state(npfem_ctx *ctx, const int64_t *cell_ids, int64_t n_ids,
                     void *positions, void *velocities, int32_t dtype, int32_t where);

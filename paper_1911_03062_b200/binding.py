@@ -21,7 +21,7 @@ _ERR_NAMES = {-1: "NPFEM_EINVAL", -2: "NPFEM_EMESH", -3: "NPFEM_ECUDA", -4: "NPF
 
 EXPORTED_SYMBOLS = (
     "npfem_create", "npfem_workspace_bytes", "npfem_bind_workspace", "npfem_set_option",
-    "npfem_set_state", "npfem_set_forces", "npfem_step", "npfem_get_state", "npfem_get_objective",
+    "npfem_set_state", "npfem_set_forces", "npfem_step", "npfem_step_host", "npfem_get_state", "npfem_get_objective",
     "npfem_get_kernel_times", "npfem_launch_count", "npfem_last_error", "npfem_version", "npfem_destroy",
     "npfem_local_schedule_stats", "npfem_set_line_search", "npfem_get_step_lengths", "npfem_set_velocity_cap", "npfem_set_collisions",
     "npfem_clear_collisions",
@@ -80,6 +80,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.npfem_set_forces.restype = C.c_int
     lib.npfem_step.argtypes = [vp, i32]
     lib.npfem_step.restype = C.c_int
+    lib.npfem_step_host.argtypes = [vp, vp, i32, vp, vp, i32, i32]
+    lib.npfem_step_host.restype = C.c_int
     lib.npfem_get_state.argtypes = [vp, C.POINTER(i64), i64, vp, vp, i32, i32]
     lib.npfem_get_state.restype = C.c_int
     lib.npfem_get_objective.argtypes = [vp, vp, i32, C.POINTER(i32), vp, i32]
@@ -249,6 +251,16 @@ class Solver:
 
     def step(self, n_iterations: int) -> None:
         self._check(self._lib.npfem_step(self._ctx, int(n_iterations)))
+
+    def step_host(self, forces, n_iterations: int, positions, velocities, n_chunks: int = 0) -> None:
+        """npfem_step_host: forces in, one step, {x, v} out with HOST buffers, pipelined over chunks of cells."""
+        count = 3 * self.total_vertices
+        f, code, where, _k0 = self._buffer(forces, count, "forces")
+        p, pcode, pwhere, _k1 = self._buffer(positions, count, "positions")
+        v, vcode, vwhere, _k2 = self._buffer(velocities, count, "velocities")
+        if {where, pwhere, vwhere} != {NPFEM_HOST} or not (code == pcode == vcode):
+            raise ValueError("step_host takes host buffers of one dtype")
+        self._check(self._lib.npfem_step_host(self._ctx, f, int(n_iterations), p, v, code, int(n_chunks)))
 
     def get_state(self, cell_ids=None, dtype="fp64", where="device", positions=None, velocities=None):
         """Returns (positions, velocities) as flat tensors (device) or numpy arrays (host)."""

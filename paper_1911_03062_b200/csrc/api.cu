@@ -33,12 +33,15 @@ struct npfem_ctx {
   struct Layout {
     std::vector<size_t> type_off[18];     // per type: tri, nbr, rest, hinge, corner, vnbr, w, mass, inv_area, Hinv, Hinv_tf32
     std::vector<size_t> field_off[F_COUNT], origin_off, cellid_off, scratch_off;
-    size_t views_off = 0, refs_all_off = 0, refs_tmp_off = 0, stage_a_off = 0, stage_b_off = 0, total = 0;
+    size_t views_off = 0, refs_all_off = 0, refs_tmp_off = 0, stage_a_off = 0, stage_b_off = 0, stage_c_off = 0, total = 0;
   } lay;
   BucketView *views_dev = nullptr;
   CellRef *refs_all_dev = nullptr, *refs_tmp_dev = nullptr;
   std::vector<int64_t *> cell_id_dev;
-  void *stage_a = nullptr, *stage_b = nullptr;
+  void *stage_a = nullptr, *stage_b = nullptr, *stage_c = nullptr;
+  // npfem_step_host: copy streams and per-chunk events, created on first use
+  cudaStream_t h2d_stream = nullptr, d2h_stream = nullptr;
+  std::vector<cudaEvent_t> io_events;
   // diagnostics
   bool diagnostics = false;
   double *history_dev = nullptr;
@@ -197,6 +200,7 @@ void compute_layout(npfem_ctx *c) {
   L.refs_tmp_off = take(size_t(c->n_cells) * sizeof(CellRef));
   L.stage_a_off = take(size_t(c->total_vertices) * 3 * sizeof(double));
   L.stage_b_off = take(size_t(c->total_vertices) * 3 * sizeof(double));
+  L.stage_c_off = take(size_t(c->total_vertices) * 3 * sizeof(double));
   L.total = off;
 }
 
@@ -376,6 +380,7 @@ int ensure_ready(npfem_ctx *c) {
   c->refs_tmp_dev = reinterpret_cast<CellRef *>(c->ws + L.refs_tmp_off);
   c->stage_a = c->ws + L.stage_a_off;
   c->stage_b = c->ws + L.stage_b_off;
+  c->stage_c = c->ws + L.stage_c_off;
   int rc;
   if ((rc = upload_raw(c, L.views_off, c->views))) return rc;
   std::vector<CellRef> refs(size_t(c->n_cells));
@@ -792,6 +797,105 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   return NPFEM_OK;
 }
 
+// One time step with HOST buffers, pipelined (include/npfem.h).  Cells are independent within a step
+// and a range of cell ids is one contiguous slab of every bucket and of the user
+// buffers, so the population is cut into chunks and chunk i's solver kernels run while chunk i+1's
+// forces come in and chunk i-1's state goes out, on two copy streams (PCIe is full duplex).
+int npfem_step_host(npfem_ctx *c, const void *forces, int32_t n_iterations, void *positions, void *velocities,
+                    int32_t dtype, int32_t n_chunks) {
+  int rc = common_checks(c, dtype, NPFEM_HOST);
+  if (rc) return rc;
+  if (!forces || !positions || !velocities) return fail(c, NPFEM_EINVAL, "forces / positions / velocities is NULL");
+  if (n_chunks < 0 || n_chunks > 64) return fail(c, NPFEM_EINVAL, "n_chunks must be in 0..64 (0 = auto)");
+  if (n_iterations < 1 || n_iterations > NPFEM_MAX_ITERATIONS) return fail(c, NPFEM_EINVAL, "n_iterations out of range");
+  if (!c->ready || c->n_set != c->n_cells) return fail(c, NPFEM_ESTATE, "step before every cell has been given a state");
+  const size_t es = dtype == NPFEM_F32 ? 4 : 8;
+  const int64_t total = c->total_vertices * 3;
+  if (n_chunks == 0) n_chunks = int32_t(std::min<int64_t>(16, std::max<int64_t>(1, int64_t(total * es) / (48 << 20))));
+  n_chunks = int32_t(std::max<int64_t>(1, std::min<int64_t>(n_chunks, c->n_cells)));
+  // per-cell reductions over the whole bucket (history rows, line-search state, collision tables) are
+  // indexed by bucket slot: those modes take the unchunked sequence
+  if (c->diagnostics || c->ls_max_halvings > 0 || c->col_active || c->median_filter || n_chunks == 1) {
+    if ((rc = npfem_set_forces(c, nullptr, 0, forces, dtype, NPFEM_HOST))) return rc;
+    if ((rc = npfem_step(c, n_iterations))) return rc;
+    return npfem_get_state(c, nullptr, 0, positions, velocities, dtype, NPFEM_HOST);
+  }
+  if (!c->h2d_stream) {
+    NPFEM_CUDA(c, cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking));
+    NPFEM_CUDA(c, cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking));
+  }
+  while (c->io_events.size() < size_t(2 * n_chunks + 1)) {
+    cudaEvent_t e;
+    NPFEM_CUDA(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    c->io_events.push_back(e);
+  }
+  const size_t nb = c->buckets.size();
+  const std::vector<BucketView> full_views = c->views;
+  std::vector<int64_t> full_cells(nb), slot0(nb, 0);
+  for (size_t t = 0; t < nb; ++t) full_cells[t] = c->buckets[t].cells;
+  auto restore = [&] {
+    c->views = full_views;
+    for (size_t t = 0; t < nb; ++t) c->buckets[t].cells = full_cells[t];
+  };
+  // the copy-in stream starts after whatever the caller's stream still has in flight on the staging buffers
+  cudaEvent_t ev_start = c->io_events[size_t(2 * n_chunks)];
+  NPFEM_CUDA(c, cudaEventRecord(ev_start, c->stream));
+  NPFEM_CUDA(c, cudaStreamWaitEvent(c->h2d_stream, ev_start, 0));
+  NPFEM_CUDA(c, cudaStreamWaitEvent(c->d2h_stream, ev_start, 0));
+  const unsigned char *f_host = static_cast<const unsigned char *>(forces);
+  unsigned char *x_host = static_cast<unsigned char *>(positions), *v_host = static_cast<unsigned char *>(velocities);
+  unsigned char *sa = static_cast<unsigned char *>(c->stage_a), *sb = static_cast<unsigned char *>(c->stage_b),
+                *sc = static_cast<unsigned char *>(c->stage_c);
+  // all copies in are queued first: the copy engine runs ahead of the solver as far as it can
+  for (int i = 0; i < n_chunks; ++i) {
+    const int64_t c0 = c->n_cells * i / n_chunks, c1 = c->n_cells * (i + 1) / n_chunks;
+    const size_t b0 = size_t(c->user_offset_all[c0]) * es, b1 = size_t(c->user_offset_all[c1]) * es;
+    NPFEM_CUDA(c, cudaMemcpyAsync(sc + b0, f_host + b0, b1 - b0, cudaMemcpyHostToDevice, c->h2d_stream));
+    NPFEM_CUDA(c, cudaEventRecord(c->io_events[size_t(i)], c->h2d_stream));
+  }
+  for (int i = 0; i < n_chunks; ++i) {
+    const int64_t c0 = c->n_cells * i / n_chunks, c1 = c->n_cells * (i + 1) / n_chunks;
+    const size_t b0 = size_t(c->user_offset_all[c0]) * es, b1 = size_t(c->user_offset_all[c1]) * es;
+    std::vector<int64_t> count(nb, 0);
+    for (int64_t cell = c0; cell < c1; ++cell) ++count[size_t(c->type_of_cell[cell])];
+    PackArgs a{};
+    a.refs = c->refs_all_dev + c0;
+    a.n_refs = c1 - c0;
+    a.io_dtype = dtype;
+    a.src_a = sc;
+    NPFEM_CUDA(c, cudaStreamWaitEvent(c->stream, c->io_events[size_t(i)], 0));
+    if ((rc = check_launch(c, launch_set_forces(c->views_dev, a, c->precision, c->stream), "set_forces"))) return rc;
+    for (size_t t = 0; t < nb; ++t) {
+      BucketView bv = full_views[t];
+      const size_t shift = size_t(slot0[t]) * 3 * size_t(bv.n_pad) * esize(c->precision);
+      for (int f = 0; f < F_COUNT; ++f) bv.field[f] = static_cast<unsigned char *>(bv.field[f]) + shift;
+      bv.origin += slot0[t] * 3;
+      bv.cells = count[t];
+      c->views[t] = bv;
+      c->buckets[t].cells = count[t];
+    }
+    rc = npfem_step(c, n_iterations);
+    restore();
+    if (rc) return rc;
+    for (size_t t = 0; t < nb; ++t) slot0[t] += count[t];
+    PackArgs g{};
+    g.refs = c->refs_all_dev + c0;
+    g.n_refs = c1 - c0;
+    g.io_dtype = dtype;
+    g.dst_a = sa;
+    g.dst_b = sb;
+    if ((rc = check_launch(c, launch_get_state(c->views_dev, g, c->precision, c->stream), "get_state"))) return rc;
+    cudaEvent_t packed = c->io_events[size_t(n_chunks + i)];
+    NPFEM_CUDA(c, cudaEventRecord(packed, c->stream));
+    NPFEM_CUDA(c, cudaStreamWaitEvent(c->d2h_stream, packed, 0));
+    NPFEM_CUDA(c, cudaMemcpyAsync(x_host + b0, sa + b0, b1 - b0, cudaMemcpyDeviceToHost, c->d2h_stream));
+    NPFEM_CUDA(c, cudaMemcpyAsync(v_host + b0, sb + b0, b1 - b0, cudaMemcpyDeviceToHost, c->d2h_stream));
+  }
+  NPFEM_CUDA(c, cudaStreamSynchronize(c->d2h_stream));
+  NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  return NPFEM_OK;
+}
+
 int npfem_set_line_search(npfem_ctx *c, int32_t max_halvings, double armijo_c1, double grad_tol) {
   if (!c) return NPFEM_EINVAL;
   if (max_halvings < 0 || max_halvings > 30 || !(armijo_c1 >= 0) || !(armijo_c1 < 1) || !(grad_tol >= 0))
@@ -1037,6 +1141,9 @@ void npfem_destroy(npfem_ctx *c) {
     cudaEventDestroy(sp.b);
   }
   for (auto e : c->event_pool) cudaEventDestroy(e);
+  for (auto e : c->io_events) cudaEventDestroy(e);
+  if (c->h2d_stream) cudaStreamDestroy(c->h2d_stream);
+  if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
   cudaGetLastError();
   delete c;
 }

@@ -521,3 +521,56 @@ def test_static_partition_shards_match_the_unsharded_solver(precision):
     assert np.linalg.norm(xw - x0) > 0
     for s in [whole] + shards:
         s.solver.close()
+
+
+@pytest.mark.parametrize("precision,n_chunks", [("fp32", 7), ("fp32", 0), ("fp64", 4), ("fp32", 64)])
+def test_step_host_pipelined_equals_the_three_calls(precision, n_chunks):
+    """npfem_step_host (include/npfem.h): forces in, step, state out over chunks of cell ids on copy streams.
+    Chunks are contiguous slabs of every bucket, cells are independent: bit-identical to
+    set_forces + step + get_state, with ragged chunk sizes, interleaved types and more chunks than PLT cells."""
+    import torch
+    from paper_1911_03062_b200 import Solver, binding
+    pop = make_config(3, n_cells=45)
+    np_io = np.float32 if precision == "fp32" else np.float64
+    x0 = pop.packed(pop.positions, dtype=np_io)
+    out = []
+    for pipelined in (False, True):
+        s = Solver(pop.types, pop.type_of_cell, pop.dt, precision=precision)
+        s.set_option(binding.OPT_FUSED_STEP, 1)
+        s.set_state(x0)
+        x = torch.empty(x0.size, dtype=torch.from_numpy(x0[:1]).dtype).pin_memory()
+        v = torch.empty_like(x).pin_memory()
+        for k in range(3):
+            f = torch.from_numpy(pop.packed(pop.forces(k), dtype=np_io)).pin_memory()
+            if pipelined:
+                s.step_host(f, 5, x, v, n_chunks=n_chunks)
+            else:
+                s.set_forces(f)
+                s.step(5)
+                s.get_state(positions=x, velocities=v)
+        out.append((x.numpy().copy(), v.numpy().copy()))
+        s.close()
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    assert np.linalg.norm(out[0][0] - x0) > 0 and np.all(np.isfinite(out[0][1]))
+
+
+def test_step_host_with_line_search_takes_the_unchunked_sequence():
+    import torch
+    from paper_1911_03062_b200 import Solver
+    pop = make_config(2, n_cells=6)
+    x0 = pop.packed(pop.positions)
+    f = torch.from_numpy(pop.packed(pop.forces(0))).pin_memory()
+    res = []
+    for pipelined in (False, True):
+        s = Solver(pop.types, pop.type_of_cell, pop.dt, precision="fp64")
+        s.set_line_search(3)
+        s.set_state(x0)
+        x = torch.empty(x0.size, dtype=torch.float64).pin_memory()
+        v = torch.empty_like(x).pin_memory()
+        if pipelined:
+            s.step_host(f, 4, x, v, n_chunks=3)
+        else:
+            s.set_forces(f); s.step(4); s.get_state(positions=x, velocities=v)
+        res.append(x.numpy().copy())
+        s.close()
+    assert np.array_equal(res[0], res[1])
