@@ -254,14 +254,15 @@ def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: 
         solver.step(n_iterations)
     barrier()
     launches0 = solver.launch_count
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    marks = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     with ClockSampler(local_rank) as clocks:
-        ev0.record()
-        for _ in range(args.steps):
+        marks[0].record()
+        for k in range(args.steps):
             solver.step(n_iterations)
-        ev1.record()
+            marks[k + 1].record()                     # one event between steps: per-step times for median / best
         barrier()
-    elapsed_ms = ev0.elapsed_time(ev1)
+    elapsed_ms = marks[0].elapsed_time(marks[-1])
+    step_ms = sorted(marks[k].elapsed_time(marks[k + 1]) for k in range(args.steps))
     launches = solver.launch_count - launches0
     # per-kernel breakdown: the same K steps again with a CUDA-event pair around every launch (kept out of
     # the timed region above: the events cost as much as a small kernel in the small-batch regime)
@@ -324,6 +325,8 @@ def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: 
         "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32" if args.precision == "fp32" else "f64",
         "data": "synthetic", "config": config_desc, "clocks": clocks.summary(), "gpu_launches": launches,
+        "ms_per_step_median": step_ms[len(step_ms) // 2] if len(step_ms) % 2 else 0.5 * (step_ms[len(step_ms) // 2 - 1] + step_ms[len(step_ms) // 2]),
+        "ms_per_step_best": step_ms[0],
         "roofline": roofline, "kernels": kernels,
         "kernel_ms_per_step": {k: sum(ms for ms, _ in v) / args.steps for k, v in ktimes.items()},
     }
