@@ -48,11 +48,11 @@ __device__ __forceinline__ double dot3(const double *u, const double *v) {
 __device__ __forceinline__ float rsq(float x) { return rsqrtf(x); }
 __device__ __forceinline__ double rsq(double x) { return rsqrt(x); }
 
-template <typename T>
-__global__ void __launch_bounds__(256, 2)
+template <typename T, int NT>
+__global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1)
 local_generic_kernel(const LocalParams<T> p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  __shared__ double red[8];
+  __shared__ double red[16];
   __shared__ T vol_coef_sh;
   const int n = p.n, n_pad = p.n_pad, nt = p.T_;
   T *sx = reinterpret_cast<T *>(smem_raw);   // [3][n] current positions x_n + d (cell-local)
@@ -340,13 +340,18 @@ int launch_local_T(const TypeDev &td, const BucketView &bv, void *scratch, int n
   }
   static bool attr_set[2] = {false, false};
   if (!attr_set[sizeof(T) == 8]) {
-    cudaFuncSetAttribute(local_generic_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kMaxSmem));
+    cudaFuncSetAttribute(local_generic_kernel<T, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kMaxSmem));
+    cudaFuncSetAttribute(local_generic_kernel<T, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kMaxSmem));
     attr_set[sizeof(T) == 8] = true;
   }
   const int per_sm = smem * 2 + 4096 <= 227 * 1024 ? 2 : 1;
   int64_t grid = int64_t(n_sm) * per_sm;
   if (grid > bv.cells) grid = bv.cells;
-  local_generic_kernel<T><<<unsigned(grid), 256, smem, s>>>(p);
+  // one CTA per SM (fp64, large meshes): 512 threads with up to 128 registers each hide the FP64 latencies
+  if (per_sm == 1)
+    local_generic_kernel<T, 512><<<unsigned(grid), 512, smem, s>>>(p);
+  else
+    local_generic_kernel<T, 256><<<unsigned(grid), 256, smem, s>>>(p);
   return 1;
 }
 
