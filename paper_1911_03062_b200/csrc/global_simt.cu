@@ -79,26 +79,36 @@ global_dmma_kernel(const double *__restrict__ G, const double *__restrict__ W, d
     for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
   const int ar = tid >> 1, ak = (tid & 1) * 8;             // A tile: thread loads 8 consecutive doubles of row ar
   const int bk = tid >> 4, bc = (tid & 15) * 4;            // B tile: thread loads 4 consecutive doubles of row bk
+  // register-prefetched pipeline: the next K-slice is loaded from global memory while the current one is multiplied
+  const bool ok = row0 + ar < rows, okb = col0 + bc < n_pad;   // n_pad is a multiple of 16: a group of 4 is in or out
+  const double2 *src = reinterpret_cast<const double2 *>(G + (row0 + ar) * n_pad + ak);
+  const double2 *srcb = reinterpret_cast<const double2 *>(W + size_t(bk) * n_pad + col0 + bc);
+  const double2 zero2 = make_double2(0.0, 0.0);
+  double2 ra[4], rb[2];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) ra[q] = ok ? src[q] : zero2;
+#pragma unroll
+  for (int q = 0; q < 2; ++q) rb[q] = okb ? srcb[q] : zero2;
   for (int k0 = 0; k0 < n_pad; k0 += BK) {
-    {
-      const bool ok = row0 + ar < rows;
-      const double2 *src = reinterpret_cast<const double2 *>(G + (row0 + ar) * n_pad + k0 + ak);
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const double2 v = ok ? src[q] : make_double2(0.0, 0.0);
-        As[ar * AS + ak + 2 * q] = v.x;
-        As[ar * AS + ak + 2 * q + 1] = v.y;
-      }
-      const bool okb = col0 + bc < n_pad;                  // n_pad is a multiple of 16: a group of 4 is in or out
-      const double2 *srcb = reinterpret_cast<const double2 *>(W + size_t(k0 + bk) * n_pad + col0 + bc);
+    for (int q = 0; q < 4; ++q) {
+      As[ar * AS + ak + 2 * q] = ra[q].x;
+      As[ar * AS + ak + 2 * q + 1] = ra[q].y;
+    }
 #pragma unroll
-      for (int q = 0; q < 2; ++q) {
-        const double2 v = okb ? srcb[q] : make_double2(0.0, 0.0);
-        Bs[bk * BS + bc + 2 * q] = v.x;
-        Bs[bk * BS + bc + 2 * q + 1] = v.y;
-      }
+    for (int q = 0; q < 2; ++q) {
+      Bs[bk * BS + bc + 2 * q] = rb[q].x;
+      Bs[bk * BS + bc + 2 * q + 1] = rb[q].y;
     }
     __syncthreads();
+    if (k0 + BK < n_pad) {
+      const double2 *na = src + (k0 + BK) / 2;
+      const double2 *nb = srcb + size_t(k0 + BK) * n_pad / 2;
+#pragma unroll
+      for (int q = 0; q < 4; ++q) ra[q] = ok ? na[q] : zero2;
+#pragma unroll
+      for (int q = 0; q < 2; ++q) rb[q] = okb ? nb[q] : zero2;
+    }
 #pragma unroll
     for (int kk = 0; kk < BK; kk += 4) {
       double a[4], b[4];
