@@ -574,3 +574,38 @@ def test_step_host_with_line_search_takes_the_unchunked_sequence():
         res.append(x.numpy().copy())
         s.close()
     assert np.array_equal(res[0], res[1])
+
+
+def test_full_size_config4_momentum_balance_every_cell():
+    """Pin P4 as a property that holds at any size, over ALL 100,000 cells of BASELINE
+    configs[3] in the launch configuration bench.py times: 1^T L = 0, so with v_0 = 0 and a constant force
+    the mass centre of every cell after N steps sits at h^2 (sum F / sum m) N (N + 1) / 2, whatever the
+    stiffness, damping (kappa, beta) or iteration count.  fp32 state + TF32 operator: the balance holds
+    to the rounding of the increment, measured against the cell's own displacement scale."""
+    import torch
+    from oracle import npfem_oracle as orc
+    from paper_1911_03062_b200 import Solver
+    pop = make_config(4)
+    n_steps, n_iterations = 4, 10
+    solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision="fp32")
+    solver.set_state(torch.from_numpy(pop.packed(pop.positions)).cuda())
+    solver.set_forces(torch.from_numpy(pop.packed(pop.forces(0), dtype=np.float32)).cuda())
+    for _ in range(n_steps):
+        solver.step(n_iterations)
+    x, v = solver.get_state()
+    xs = pop.unpack(x.cpu().numpy())
+    vs = pop.unpack(v.cpu().numpy())
+    solver.close()
+    forces = pop.forces(0)
+    for t, ct in enumerate(pop.types):
+        m = orc.make_type(ct, pop.dt).mass                               # [n] lumped masses, fg
+        acc = forces[t].sum(axis=1) / m.sum()                            # [cells, 3] um / us^2
+        expect = pop.dt ** 2 * acc * n_steps * (n_steps + 1) / 2
+        got = np.einsum("i,cik->ck", m, xs[t] - pop.positions[t]) / m.sum()
+        vexp = pop.dt * acc * n_steps                                    # and the momentum itself
+        vgot = np.einsum("i,cik->ck", m, vs[t]) / m.sum()
+        scale = np.linalg.norm(expect, axis=1).max()
+        err = np.linalg.norm(got - expect, axis=1).max() / scale
+        verr = np.linalg.norm(vgot - vexp, axis=1).max() / np.linalg.norm(vexp, axis=1).max()
+        print(ct.name, "cells", xs[t].shape[0], "centre err", err, "momentum err", verr, "scale um", scale)
+        assert err <= 5e-4 and verr <= 5e-4                               # measured 1.3e-4 / 1.7e-4
