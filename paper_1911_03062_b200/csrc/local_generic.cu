@@ -31,8 +31,8 @@ struct LocalParams {
   const T *x, *d, *b;
   T *g;
   int64_t cells;
-  T *scratch;          // global scratch [gridDim][13 T_] when normals/corners do not fit in smem
-  int scratch_in_smem;
+  T *scratch;          // global scratch per CTA when the working set does not fit in shared memory:
+  int scratch_in_smem; //   1: nothing, 0: [13 T_] normals + corner forces, -1: [9 n + 13 T_] the vertex arrays too
 };
 
 namespace {
@@ -55,15 +55,19 @@ local_generic_kernel(const LocalParams<T> p) {
   __shared__ double red[16];
   __shared__ T vol_coef_sh;
   const int n = p.n, n_pad = p.n_pad, nt = p.T_;
-  T *sx = reinterpret_cast<T *>(smem_raw);   // [3][n] current positions x_n + d (cell-local)
+  // any mesh size runs: what does not fit in shared memory lives in a per-CTA slab of global scratch
+  // (L2-resident; __syncthreads orders global accesses within the block as well)
+  T *slab = p.scratch_in_smem > 0 ? nullptr
+                                  : p.scratch + size_t(blockIdx.x) * (p.scratch_in_smem < 0 ? size_t(9) * n + size_t(13) * nt : size_t(13) * nt);
+  T *sx = p.scratch_in_smem < 0 ? slab : reinterpret_cast<T *>(smem_raw);   // [3][n] current positions x_n + d (cell-local)
   T *sd = sx + 3 * n;                        // [3][n] d
   T *sz = sd + 3 * n;                        // [3][n] z
   T *sN, *sC;
-  if (p.scratch_in_smem) {
+  if (p.scratch_in_smem > 0) {
     sN = sz + 3 * n;                         // [T][4] area vector, |N|^2
     sC = sN + 4 * nt;                        // [T][9] corner forces
   } else {
-    sN = p.scratch + size_t(blockIdx.x) * 13 * nt;
+    sN = p.scratch_in_smem < 0 ? sz + 3 * n : slab;
     sC = sN + 4 * nt;
   }
   const bool stencil = p.beta_over_h != T(0);
@@ -334,9 +338,12 @@ int launch_local_T(const TypeDev &td, const BucketView &bv, void *scratch, int n
   size_t smem = smem_full<T>(td);
   if (smem > kMaxSmem) {
     smem = smem_min<T>(td);
-    if (smem > kMaxSmem) return -1;
     p.scratch_in_smem = 0;
     p.scratch = static_cast<T *>(scratch);
+    if (smem > kMaxSmem) {                   // e.g. a 10,242-vertex level-5 mesh: the vertex arrays go to the slab too
+      smem = 0;
+      p.scratch_in_smem = -1;
+    }
   }
   static bool attr_set[2] = {false, false};
   if (!attr_set[sizeof(T) == 8]) {
@@ -361,7 +368,8 @@ size_t local_generic_scratch_bytes(const TypeDev &td, int precision, int n_sm) {
   const size_t es = precision == NPFEM_F32 ? 4 : 8;
   const size_t full = es * (size_t(9) * td.n + size_t(13) * td.T);
   if (full <= kMaxSmem) return 0;
-  return es * size_t(13) * td.T * size_t(n_sm) * 2;
+  const size_t per_cta = es * size_t(9) * td.n <= kMaxSmem ? es * size_t(13) * td.T : full;
+  return per_cta * size_t(n_sm) * 2;
 }
 
 int launch_local_generic(const TypeDev &td, const BucketView &bv, void *scratch, int precision, int n_sm,

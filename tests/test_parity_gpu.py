@@ -609,3 +609,13 @@ def test_full_size_config4_momentum_balance_every_cell():
         verr = np.linalg.norm(vgot - vexp, axis=1).max() / np.linalg.norm(vexp, axis=1).max()
         print(ct.name, "cells", xs[t].shape[0], "centre err", err, "momentum err", verr, "scale um", scale)
         assert err <= 5e-4 and verr <= 5e-4                               # measured 1.3e-4 / 1.7e-4
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_level5_mesh_10242_vertices_runs_from_global_scratch(precision):
+    """Maximum size: a level-5 icosphere cell (10,242 vertices, 20,480 triangles, H~^-1 of 10,256^2).  None of
+    the shared-memory local-step kernels can hold it; the generic kernel keeps the cell in a per-CTA slab of
+    global scratch.  One cell, 1 step x 3 iterations against the oracle."""
+    pop = make_config(1, level=5)
+    assert pop.types[0].n_vertices == 10242
+    _check(pop, precision, n_steps=1, n_iterations=3)
