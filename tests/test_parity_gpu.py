@@ -461,8 +461,9 @@ def _sampled_full_size(config, precision, n_steps, n_iterations, samples_per_typ
 
 
 def test_full_size_config4_100k_cells_sampled():
-    """BASELINE configs[3] at its full 100,000 cells, fp32, default kernels (what bench.py times)."""
-    for name, pos, disp, vel in _sampled_full_size(4, "fp32", n_steps=2, n_iterations=10):
+    """BASELINE configs[3] at its full 100,000 cells, fp32, default kernels (what bench.py times); the oracle
+    recomputes a seeded sample of ~1,000 cells per type, about a minute of host time."""
+    for name, pos, disp, vel in _sampled_full_size(4, "fp32", n_steps=2, n_iterations=10, samples_per_type=1000):
         print(name, pos, disp, vel)
         assert pos <= TOL_POS["fp32"] and disp <= TOL_DISP["fp32"] and vel <= TOL_DISP["fp32"]
 
