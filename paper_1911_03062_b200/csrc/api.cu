@@ -351,6 +351,9 @@ int ensure_ready(npfem_ctx *c) {
     int nl = e == cudaSuccess ? launch_invert_spd(H64, Hinv64, h.n, c->stream, &residual, ierr) : -1;
     if (nl >= 0) {
       nl += launch_convert_pad(Hinv64, h.n, c->ws + L.type_off[9][t], h.n_pad, c->precision, c->stream);
+      if (c->precision == NPFEM_F32)   // the tensor-core operand: H~^-1 rounded to TF32 to nearest (internal.h, tf32_rn)
+        nl += launch_round_tf32(reinterpret_cast<const float *>(c->ws + L.type_off[9][t]),
+                                reinterpret_cast<float *>(c->ws + L.type_off[10][t]), size_t(h.n_pad) * h.n_pad, c->stream);
       e = cudaStreamSynchronize(c->stream);
     }
     cudaFree(H64);
@@ -733,6 +736,11 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
     fused[t] = !ls_on && !c->col_active && c->precision == NPFEM_F32 && !c->diagnostics && c->opt_global_math == 0 && c->opt_update_mode == 2 &&
                (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]) &&
                global_tcgen05_supported(c->types[t]);
+  // g feeds the TF32 tensor-core GEMM: the local step stores it already rounded to nearest (the line search
+  // keeps the unrounded gradient for its slope and stopping test)
+  for (size_t t = 0; t < nb; ++t)
+    c->views[t].g_tf32 = c->precision == NPFEM_F32 && c->opt_global_math == 0 && !ls_on &&
+                         global_tcgen05_supported(c->types[t]);
   for (int k = 0; k < n_iterations; ++k) {
     if (c->diagnostics && (rc = diag(k))) return rc;
     for (size_t t = 0; t < nb; ++t) {

@@ -371,7 +371,7 @@ int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, dou
   p.d_scale = float(d_scale);
   CUtensorMap map_g, map_w, map_d;
   if (!make_map(&map_g, bv.field[F_G], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), BM)) return -1;
-  if (!make_map(&map_w, td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n_pass / CL)))
+  if (!make_map(&map_w, td.Hinv_tf32 ? td.Hinv_tf32 : td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n_pass / CL)))
     return -1;
   // epilogue tiles: [32 rows][32 columns] of D (in-place update) or of U (product out)
   if (!make_map(&map_d, u_out ? u_out : bv.field[F_D], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), 32))

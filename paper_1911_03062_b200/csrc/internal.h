@@ -74,6 +74,8 @@ int launch_invert_spd(const double *H_dev, double *Hinv_dev, int n, cudaStream_t
                       double *residual_out, std::string &err);
 
 int launch_convert_pad(const double *X, int n, void *out, int n_pad, int precision, cudaStream_t s);
+// out = in rounded to TF32 to nearest (the tensor core would otherwise drop the low 13 mantissa bits)
+int launch_round_tf32(const float *in, float *out, size_t count, cudaStream_t s);
 
 // implemented per operation in pack.cu
 struct PackArgs {
@@ -86,11 +88,22 @@ struct PackArgs {
   int io_dtype;
 };
 
+// The TF32 tensor-core path reads fp32 operands and IGNORES their low 13 mantissa bits (truncation).  Truncating both
+// operands biases every product towards zero and costs 1.3e-3 of the net momentum of a cell;
+// rounding them to nearest beforehand leaves 3e-6.  Both operands are therefore stored already rounded.
+__device__ __forceinline__ float tf32_rn(float x) {
+  uint32_t r;
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+  return __uint_as_float(r);
+}
+__device__ __forceinline__ double tf32_rn(double x) { return x; }   // fp64 contexts never take the TF32 path
+
 struct BucketView {       // what kernels need of a bucket, passed by value
   void *field[F_COUNT];
   double *origin;
   int64_t cells;
   int n, n_pad;
+  int g_tf32;              // the local step rounds g to TF32 (to nearest): its consumer is the TF32 tensor-core GEMM
 };
 
 int launch_set_state(const BucketView *views_dev, const PackArgs &a, int precision, cudaStream_t s);

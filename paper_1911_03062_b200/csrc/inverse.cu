@@ -98,6 +98,18 @@ __global__ void convert_pad_kernel(const double *__restrict__ X, int n, T *__res
 }  // namespace
 
 // out[n_pad][n_pad] (compute type) = X[n][n] (fp64), zero padded
+__global__ void round_tf32_kernel(const float *__restrict__ in, float *__restrict__ out, size_t count) {
+  for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < count; i += size_t(gridDim.x) * blockDim.x)
+    out[i] = tf32_rn(in[i]);
+}
+
+int launch_round_tf32(const float *in, float *out, size_t count, cudaStream_t s) {
+  if (count == 0) return 0;
+  const unsigned grid = unsigned((count + 255) / 256 < 148 * 8 ? (count + 255) / 256 : 148 * 8);
+  round_tf32_kernel<<<grid, 256, 0, s>>>(in, out, count);
+  return 1;
+}
+
 int launch_convert_pad(const double *X, int n, void *out, int n_pad, int precision, cudaStream_t s) {
   const int eb = 256, eg = int((size_t(n_pad) * n_pad + eb - 1) / eb);
   if (precision == NPFEM_F32)

@@ -31,6 +31,7 @@ struct BigParams {
   double kv_over_V0, V0;
   const float *x, *d, *b;     // [cells][3][n_pad]
   float *g;
+  int g_tf32;
   int64_t cells;
 };
 
@@ -192,9 +193,11 @@ __global__ void __launch_bounds__(THREADS, 1) local_big_kernel(const BigParams p
       const int i = tid + r * THREADS;
       if (i < n) {
         const float coef = __ldg(p.vtx_coef + i);
-        p.g[base + i] = coef * dg[i] - bg[i] + acc[r][0];
-        p.g[base + n_pad + i] = coef * dg[n_pad + i] - bg[n_pad + i] + acc[r][1];
-        p.g[base + 2 * n_pad + i] = coef * dg[2 * n_pad + i] - bg[2 * n_pad + i] + acc[r][2];
+        const float g0 = coef * dg[i] - bg[i] + acc[r][0], g1 = coef * dg[n_pad + i] - bg[n_pad + i] + acc[r][1],
+                    g2 = coef * dg[2 * n_pad + i] - bg[2 * n_pad + i] + acc[r][2];
+        p.g[base + i] = p.g_tf32 ? tf32_rn(g0) : g0;
+        p.g[base + n_pad + i] = p.g_tf32 ? tf32_rn(g1) : g1;
+        p.g[base + 2 * n_pad + i] = p.g_tf32 ? tf32_rn(g2) : g2;
       }
     }
     // the next cell's phase 0 writes sx: every thread is past its last read of sx (phase B) here
@@ -233,6 +236,7 @@ int launch_local_big(const TypeDev &td, const BucketView &bv, int n_sm, cudaStre
   p.d = static_cast<const float *>(bv.field[F_D]);
   p.b = static_cast<const float *>(bv.field[F_B]);
   p.g = static_cast<float *>(bv.field[F_G]);
+  p.g_tf32 = bv.g_tf32;
   p.cells = bv.cells;
   const size_t smem = size_t(td.n) * 16 + size_t(td.T) * 16 + size_t(3) * p.tc * 16;
   static size_t smem_set = 0;

@@ -32,6 +32,7 @@ struct LocalParams {
   T *g;
   int64_t cells;
   T *scratch;          // global scratch per CTA when the working set does not fit in shared memory:
+  int g_tf32;          // round g to TF32 (fp32 contexts whose global step runs on the tensor cores)
   int scratch_in_smem; //   1: nothing, 0: [13 T_] normals + corner forces, -1: [9 n + 13 T_] the vertex arrays too
 };
 
@@ -208,8 +209,10 @@ local_generic_kernel(const LocalParams<T> p) {
           for (int k = 0; k < 3; ++k) lz[k] += wq * sz[k * n + j];
         }
       }
-      for (int k = 0; k < 3; ++k)
-        p.g[base + k * n_pad + i] = mi * sd[k * n + i] + p.beta_over_h * lz[k] - p.b[base + k * n_pad + i] + acc[k];
+      for (int k = 0; k < 3; ++k) {
+        const T gk = mi * sd[k * n + i] + p.beta_over_h * lz[k] - p.b[base + k * n_pad + i] + acc[k];
+        p.g[base + k * n_pad + i] = p.g_tf32 ? tf32_rn(gk) : gk;
+      }
     }
     __syncthreads();
   }
@@ -319,6 +322,7 @@ LocalParams<T> make_params(const TypeDev &td, const BucketView &bv) {
   p.d = static_cast<const T *>(bv.field[F_D]);
   p.b = static_cast<const T *>(bv.field[F_B]);
   p.g = static_cast<T *>(bv.field[F_G]);
+  p.g_tf32 = bv.g_tf32;
   p.cells = bv.cells;
   p.scratch = nullptr;
   p.scratch_in_smem = 1;

@@ -46,6 +46,7 @@ struct SchedParams {
   const float *x, *b, *u;      // [cells][3][n_pad]
   float *d;                    // read; written back when apply_u
   float *g;
+  int g_tf32;                  // round g to TF32 (its consumer is the tensor-core GEMM)
   int apply_u;                 // first d <- d_scale d + u (pending update of the last global step)
   float d_scale;
   int64_t cells;
@@ -358,9 +359,12 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
 #pragma unroll
       for (int q = 0; q < MAXV; ++q) { ax += f[q].x; ay += f[q].y; az += f[q].z; }
       float *gout = p.g + size_t(cell) * 3 * n_pad + tid;
-      gout[0] = fmaf(coef, sg[3 * n_pad + tid], ax - sg[6 * n_pad + tid]);
-      gout[n_pad] = fmaf(coef, sg[4 * n_pad + tid], ay - sg[7 * n_pad + tid]);
-      gout[2 * n_pad] = fmaf(coef, sg[5 * n_pad + tid], az - sg[8 * n_pad + tid]);
+      const float g0 = fmaf(coef, sg[3 * n_pad + tid], ax - sg[6 * n_pad + tid]);
+      const float g1 = fmaf(coef, sg[4 * n_pad + tid], ay - sg[7 * n_pad + tid]);
+      const float g2 = fmaf(coef, sg[5 * n_pad + tid], az - sg[8 * n_pad + tid]);
+      gout[0] = p.g_tf32 ? tf32_rn(g0) : g0;
+      gout[n_pad] = p.g_tf32 ? tf32_rn(g1) : g1;
+      gout[2 * n_pad] = p.g_tf32 ? tf32_rn(g2) : g2;
     }
     if (vact2c) {
       float ax = 0.f, ay = 0.f, az = 0.f;
@@ -371,9 +375,12 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
       }
       const float coef2 = p.vtx_coef[v2c];
       float *gout = p.g + size_t(cell) * 3 * n_pad + v2c;
-      gout[0] = fmaf(coef2, sg[3 * n_pad + v2c], ax - sg[6 * n_pad + v2c]);
-      gout[n_pad] = fmaf(coef2, sg[4 * n_pad + v2c], ay - sg[7 * n_pad + v2c]);
-      gout[2 * n_pad] = fmaf(coef2, sg[5 * n_pad + v2c], az - sg[8 * n_pad + v2c]);
+      const float g0 = fmaf(coef2, sg[3 * n_pad + v2c], ax - sg[6 * n_pad + v2c]);
+      const float g1 = fmaf(coef2, sg[4 * n_pad + v2c], ay - sg[7 * n_pad + v2c]);
+      const float g2 = fmaf(coef2, sg[5 * n_pad + v2c], az - sg[8 * n_pad + v2c]);
+      gout[0] = p.g_tf32 ? tf32_rn(g0) : g0;
+      gout[n_pad] = p.g_tf32 ? tf32_rn(g1) : g1;
+      gout[2 * n_pad] = p.g_tf32 ? tf32_rn(g2) : g2;
     }
     // sN / sC are rewritten only after B1 / B2 of the next cell, which every warp reaches after this
   }
@@ -440,6 +447,7 @@ int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, bool a
   p.d_scale = float(d_scale);
   p.b = static_cast<const float *>(bv.field[F_B]);
   p.g = static_cast<float *>(bv.field[F_G]);
+  p.g_tf32 = bv.g_tf32;
   p.cells = bv.cells;
   const size_t smem = sched_smem_bytes(s, td.n_pad);
   // the BASELINE cell types get their row pitch at compile time, everything else the generic variants

@@ -35,6 +35,7 @@ struct SmemLocalParams {
   float B4, C4, k_b, kv_over_V0, V0;
   const float *x, *d, *b;    // [cells][3][n_pad]
   float *g;
+  int g_tf32;
   int64_t cells;
 };
 
@@ -225,9 +226,10 @@ local_smem_kernel(const SmemLocalParams p) {
           az += f.z;
         }
         const float coef = s_coef[i];
-        p.g[base + i] = coef * dv[r][0] - bv[r][0] + ax;
-        p.g[base + n_pad + i] = coef * dv[r][1] - bv[r][1] + ay;
-        p.g[base + 2 * n_pad + i] = coef * dv[r][2] - bv[r][2] + az;
+        const float g0 = coef * dv[r][0] - bv[r][0] + ax, g1 = coef * dv[r][1] - bv[r][1] + ay, g2 = coef * dv[r][2] - bv[r][2] + az;
+        p.g[base + i] = p.g_tf32 ? tf32_rn(g0) : g0;
+        p.g[base + n_pad + i] = p.g_tf32 ? tf32_rn(g1) : g1;
+        p.g[base + 2 * n_pad + i] = p.g_tf32 ? tf32_rn(g2) : g2;
       }
     }
     // no barrier here: the next cell's phase 0 only writes sx (last read before barrier 3) and the
@@ -273,6 +275,7 @@ int launch_local_smem(const TypeDev &td, const BucketView &bv, int n_sm, cudaStr
   p.d = static_cast<const float *>(bv.field[F_D]);
   p.b = static_cast<const float *>(bv.field[F_B]);
   p.g = static_cast<float *>(bv.field[F_G]);
+  p.g_tf32 = bv.g_tf32;
   p.cells = bv.cells;
   const size_t smem = local_smem_bytes(td.n, td.T, td.n_pad);
   // threads: two triangles per thread for big meshes, one for small ones; vertices need <= 2 rounds
