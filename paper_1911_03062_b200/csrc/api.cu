@@ -737,10 +737,9 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
                (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]) &&
                global_tcgen05_supported(c->types[t]);
   // g feeds the TF32 tensor-core GEMM: the local step stores it already rounded to nearest (the line search
-  // keeps the unrounded gradient for its slope and stopping test)
+  // then takes its slope and gradient norm from the rounded gradient: 2^-12 relative per entry, random sign)
   for (size_t t = 0; t < nb; ++t)
-    c->views[t].g_tf32 = c->precision == NPFEM_F32 && c->opt_global_math == 0 && !ls_on &&
-                         global_tcgen05_supported(c->types[t]);
+    c->views[t].g_tf32 = c->precision == NPFEM_F32 && c->opt_global_math == 0 && global_tcgen05_supported(c->types[t]);
   for (int k = 0; k < n_iterations; ++k) {
     if (c->diagnostics && (rc = diag(k))) return rc;
     for (size_t t = 0; t < nb; ++t) {

@@ -359,12 +359,13 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
 #pragma unroll
       for (int q = 0; q < MAXV; ++q) { ax += f[q].x; ay += f[q].y; az += f[q].z; }
       float *gout = p.g + size_t(cell) * 3 * n_pad + tid;
-      const float g0 = fmaf(coef, sg[3 * n_pad + tid], ax - sg[6 * n_pad + tid]);
-      const float g1 = fmaf(coef, sg[4 * n_pad + tid], ay - sg[7 * n_pad + tid]);
-      const float g2 = fmaf(coef, sg[5 * n_pad + tid], az - sg[8 * n_pad + tid]);
-      gout[0] = p.g_tf32 ? tf32_rn(g0) : g0;
-      gout[n_pad] = p.g_tf32 ? tf32_rn(g1) : g1;
-      gout[2 * n_pad] = p.g_tf32 ? tf32_rn(g2) : g2;
+      float g0 = fmaf(coef, sg[3 * n_pad + tid], ax - sg[6 * n_pad + tid]);
+      float g1 = fmaf(coef, sg[4 * n_pad + tid], ay - sg[7 * n_pad + tid]);
+      float g2 = fmaf(coef, sg[5 * n_pad + tid], az - sg[8 * n_pad + tid]);
+      if (p.g_tf32) { g0 = tf32_rn(g0); g1 = tf32_rn(g1); g2 = tf32_rn(g2); }
+      gout[0] = g0;
+      gout[n_pad] = g1;
+      gout[2 * n_pad] = g2;
     }
     if (vact2c) {
       float ax = 0.f, ay = 0.f, az = 0.f;
