@@ -822,7 +822,14 @@ int npfem_step_host(npfem_ctx *c, const void *forces, int32_t n_iterations, void
   n_chunks = int32_t(std::max<int64_t>(1, std::min<int64_t>(n_chunks, c->n_cells)));
   // per-cell reductions over the whole bucket (history rows, line-search state, collision tables) are
   // indexed by bucket slot: those modes take the unchunked sequence
-  if (c->diagnostics || c->ls_max_halvings > 0 || c->col_active || c->median_filter || n_chunks == 1) {
+  // the small-batch whole-step kernel is chosen by bucket size: a bucket that would take it unchunked is small
+  // enough not to be worth chunking, and no chunk may fall into it when the whole bucket would not
+  bool small_batch = false;
+  if (c->opt_fused_step != 1)
+    for (size_t t = 0; t < c->buckets.size(); ++t)
+      small_batch = small_batch || (c->buckets[t].cells > 0 && step_fused_supported(c->types[t]) &&
+                                    (c->opt_fused_step == 2 || 2 * c->buckets[t].cells <= int64_t(3) * c->n_sm));
+  if (c->diagnostics || c->ls_max_halvings > 0 || c->col_active || c->median_filter || small_batch || n_chunks == 1) {
     if ((rc = npfem_set_forces(c, nullptr, 0, forces, dtype, NPFEM_HOST))) return rc;
     if ((rc = npfem_step(c, n_iterations))) return rc;
     return npfem_get_state(c, nullptr, 0, positions, velocities, dtype, NPFEM_HOST);
@@ -881,7 +888,10 @@ int npfem_step_host(npfem_ctx *c, const void *forces, int32_t n_iterations, void
       c->views[t] = bv;
       c->buckets[t].cells = count[t];
     }
+    const int64_t keep_fused = c->opt_fused_step;
+    c->opt_fused_step = 1;                       // see small_batch above: chunks take the kernels the whole bucket takes
     rc = npfem_step(c, n_iterations);
+    c->opt_fused_step = keep_fused;
     restore();
     if (rc) return rc;
     for (size_t t = 0; t < nb; ++t) slot0[t] += count[t];

@@ -657,3 +657,29 @@ def test_drifting_cells_recentre_their_local_frame(precision):
         assert np.linalg.norm(expect, axis=1).min() > 2.0               # far beyond the 0.5 um threshold
         assert disp <= TOL_DISP[precision] and vel <= TOL_DISP[precision]
         assert cerr <= (1e-4 if precision == "fp32" else 1e-9)       # fp32: measured 1.4e-5 (1.3e-3 with truncated TF32 operands)
+
+
+@pytest.mark.parametrize("cells", [600, 1800])
+def test_step_host_chunks_take_the_kernels_of_the_whole_bucket(cells):
+    """The whole-step kernel is chosen by bucket size (<= 1.5 cells per SM).  600 cells of config 6: the PLT-66 bucket
+    (100 cells) takes it, so npfem_step_host does not chunk; 1,800 cells: no bucket takes it, and no CHUNK (75 PLT
+    cells) may either - both ways the result is bit-identical to the three calls."""
+    import torch
+    from paper_1911_03062_b200 import Solver
+    pop = make_config(6, n_cells=cells)
+    x0 = pop.packed(pop.positions, dtype=np.float32)
+    f = torch.from_numpy(pop.packed(pop.forces(0), dtype=np.float32)).pin_memory()
+    out = []
+    for pipelined in (False, True):
+        s = Solver(pop.types, pop.type_of_cell, pop.dt, precision="fp32")
+        s.set_state(x0)
+        x = torch.empty(x0.size, dtype=torch.float32).pin_memory()
+        v = torch.empty_like(x).pin_memory()
+        for _ in range(2):
+            if pipelined:
+                s.step_host(f, 5, x, v, n_chunks=4)
+            else:
+                s.set_forces(f); s.step(5); s.get_state(positions=x, velocities=v)
+        out.append((x.numpy().copy(), v.numpy().copy()))
+        s.close()
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
