@@ -316,6 +316,12 @@ def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: 
             ach = cap["warp_instructions"] / (dominant["avg_ms"] * 1e-3)
             roofline["alu"] = {"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "warp-instructions/s",
                                "frac": ach / alu_peak, "smem_wavefronts_per_launch": cap.get("smem_wavefronts")}
+            if cap.get("fp32_flop"):
+                # achieved FP32 FLOP/s (fadd + fmul + 2 ffma, ncu op counts) against
+                # 148 SMs x 128 lanes x 2 x the max SM clock
+                fp32_peak = 148 * 128 * 2 * sm_mhz * 1e6 / 1e12
+                tf = cap["fp32_flop"] / (dominant["avg_ms"] * 1e-3) / 1e12
+                roofline["fp32"] = {"achieved": tf, "peak": fp32_peak, "unit": "TFLOP/s", "frac": tf / fp32_peak}
     for row in kernels:
         cap = capture.get("kernels", {}).get(row["kernel"]) if same_workload else None
         row["traffic"] = cap["dram_bytes"] if cap else None
