@@ -679,7 +679,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   auto diag = [&](int row) -> int {
     for (size_t t = 0; t < nb; ++t) {
       double *out = c->history_dev + size_t(row) * c->n_cells;
-      int r = check_launch(c, launch_objective(c->types[t], c->views[t], c->cell_id_dev[t], out, nullptr, c->precision, c->stream),
+      int r = check_launch(c, launch_objective(c->types[t], c->views[t], c->cell_id_dev[t], out, nullptr, c->precision, c->n_sm, c->stream),
                            "objective");
       if (r) return r;
       if (c->col_active &&
@@ -763,8 +763,9 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
       if (ls_on && c->buckets[t].cells) {
         // g(d) of every cell and a copy of d before the global step overwrites it
         const size_t bytes = size_t(c->buckets[t].cells) * 3 * c->types[t].n_pad * esize(c->precision);
-        if ((rc = timed_launch(c, NPFEM_KIND_LINE_SEARCH, int(t), "line search: objective", [&] {
-               int nl = launch_objective(c->types[t], c->views[t], nullptr, c->ls[t].obj0, nullptr, c->precision, c->stream);
+        // (first iteration only: ls_accept leaves the objective of the accepted trial point in obj0)
+        if (k == 0 && (rc = timed_launch(c, NPFEM_KIND_LINE_SEARCH, int(t), "line search: objective", [&] {
+               int nl = launch_objective(c->types[t], c->views[t], nullptr, c->ls[t].obj0, nullptr, c->precision, c->n_sm, c->stream);
                if (c->col_active)
                  nl += launch_collision_energy(c->views[t], c->col[t], nullptr, c->ls[t].obj0, nullptr, c->precision, c->stream);
                return nl; })))
@@ -783,7 +784,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
         if ((rc = timed_launch(c, NPFEM_KIND_LINE_SEARCH, int(t), "line search", [&] {
                int nl = launch_ls_init(c->views[t], c->ls[t], c->ls_tol, c->precision, c->stream);
                for (int l = 0; l <= c->ls_max_halvings; ++l) {
-                 nl += launch_objective(c->types[t], c->views[t], nullptr, c->ls[t].obj1, c->ls[t].done, c->precision, c->stream);
+                 nl += launch_objective(c->types[t], c->views[t], nullptr, c->ls[t].obj1, c->ls[t].done, c->precision, c->n_sm, c->stream);
                  if (c->col_active)
                    nl += launch_collision_energy(c->views[t], c->col[t], nullptr, c->ls[t].obj1, c->ls[t].done, c->precision,
                                                  c->stream);

@@ -136,7 +136,7 @@ int launch_local_generic(const TypeDev &td, const BucketView &bv, void *scratch,
                          cudaStream_t s);
 // cell_id_dev == nullptr: objective_row is indexed by the bucket slot; skip_dev[slot] != 0 skips a cell
 int launch_objective(const TypeDev &td, const BucketView &bv, const int64_t *cell_id_dev, double *objective_row,
-                     const int *skip_dev, int precision, cudaStream_t s);
+                     const int *skip_dev, int precision, int n_sm, cudaStream_t s);
 
 // Armijo backtracking line search, per-cell state of one bucket
 struct LineSearchDev {

@@ -5,7 +5,8 @@
 // iteration of Eq. (4) diverges.  Per cell and iteration, with grad = grad g(d), p = -H~^-1 grad:
 //   frozen if ||grad||_2 <= grad_tol ||b||_2 (alpha = 0);  otherwise alpha = 1 and alpha is halved while
 //   g(d + alpha p) > g(d) + c1 alpha <grad, p>, at most max_halvings times;  d <- d + alpha p.
-// npfem_step drives it (api.cu): local step (full gradient) -> objective g(d) -> d_old := d ->
+// npfem_step drives it (api.cu): local step (full gradient) -> objective g(d) (first iteration of a step
+// only: afterwards it is the objective of the accepted trial point) -> d_old := d ->
 // global step (d := d_old + p) -> ls_init -> (max_halvings + 1) x [objective at the trial point ->
 // ls_accept].  All decisions are taken in fp64 on per-cell fp64 reductions; one warp per cell.
 #include "internal.h"
@@ -71,7 +72,12 @@ ls_accept_kernel(BucketView bv, LineSearchDev ls, double c1, int last) {
     const bool ok = ls.obj1[cell] <= ls.obj0[cell] + c1 * alpha * ls.slope[cell];
     __syncwarp();
     if (ok || last) {
-      if (lane == 0) ls.done[cell] = 1;
+      // d stays at this trial point, so its objective is g(d) of the next iteration of this step (api.cu
+      // evaluates obj0 at the first iteration only); frozen cells never get here and keep theirs
+      if (lane == 0) {
+        ls.done[cell] = 1;
+        ls.obj0[cell] = ls.obj1[cell];
+      }
       continue;
     }
     const double half = 0.5 * alpha;

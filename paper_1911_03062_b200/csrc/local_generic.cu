@@ -305,6 +305,101 @@ objective_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_id, do
   (void)h;
 }
 
+// ---- objective, shared-memory version (line search): the same sum as objective_kernel
+// with x_n + d and the UNIT triangle normals of the cell staged once in shared memory in fp64, so a hinge
+// costs one rsqrt (|e|) instead of three neighbour-normal cross products, two sqrt and a division.
+// Shared memory: 8 (3 n + 3 T) bytes (RBC-642: 46 KB, RBC-2562: 184 KB); larger meshes keep objective_kernel.
+template <typename T, int NT>
+__global__ void __launch_bounds__(NT)
+objective_smem_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_id, double *__restrict__ out_row,
+                      const int *__restrict__ skip) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ double red[2][NT / 32];
+  const int n = p.n, n_pad = p.n_pad, nt = p.T_;
+  double *sp = reinterpret_cast<double *>(smem_raw);   // [3][n] x_n + d
+  double *sn = sp + 3 * n;                              // [T][3] unit normals
+  for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x) {
+    if (skip && skip[cell]) continue;                   // uniform over the CTA
+    const size_t base = size_t(cell) * 3 * n_pad;
+    for (int k = 0; k < 3; ++k)
+      for (int i = threadIdx.x; i < n; i += NT)
+        sp[k * n + i] = double(p.x[base + k * n_pad + i]) + double(p.d[base + k * n_pad + i]);
+    __syncthreads();
+    double acc = 0.0, vol = 0.0;
+    for (int t = threadIdx.x; t < nt; t += NT) {
+      const int4 tv = p.tri[t];
+      double x0[3], e1[3], e2[3], N[3];
+      for (int k = 0; k < 3; ++k) {
+        x0[k] = sp[k * n + tv.x];
+        e1[k] = sp[k * n + tv.y] - x0[k];
+        e2[k] = sp[k * n + tv.z] - x0[k];
+      }
+      cross3(e1, e2, N);
+      vol += dot3(x0, N);
+      const double a = p.tri_rest[4 * t], b = p.tri_rest[4 * t + 1], c = p.tri_rest[4 * t + 2], A0 = p.tri_rest[4 * t + 3];
+      const double e11 = dot3(e1, e1), e12 = dot3(e1, e2), e22 = dot3(e2, e2);
+      const double C11 = a * a * e11, C12 = a * (b * e11 + c * e12), C22 = b * b * e11 + 2 * b * c * e12 + c * c * e22;
+      const double I1 = C11 + C22 - 2.0, I2 = C11 * C22 - C12 * C12 - 1.0;
+      acc += A0 * (double(p.B4) * (0.5 * I1 * I1 + I1 - I2) + 0.5 * double(p.C4) * I2 * I2);
+      const double rn = 1.0 / sqrt(dot3(N, N));
+      for (int k = 0; k < 3; ++k) sn[3 * t + k] = N[k] * rn;
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t < nt; t += NT) {
+      const int4 tv = p.tri[t];
+      const int4 tn = p.tri_nbr[t];
+      const int nb[3] = {tn.x, tn.y, tn.z};
+      const int vs[3] = {tv.x, tv.y, tv.z};
+      const double N[3] = {sn[3 * t], sn[3 * t + 1], sn[3 * t + 2]};
+      for (int s = 0; s < 3; ++s) {   // every hinge is seen from both of its triangles: half each
+        const double NB[3] = {sn[3 * nb[s]], sn[3 * nb[s] + 1], sn[3 * nb[s] + 2]};
+        double e[3], cr[3];
+        for (int k = 0; k < 3; ++k) e[k] = sp[k * n + vs[(s + 1) % 3]] - sp[k * n + vs[s]];
+        cross3(N, NB, cr);
+        const double sin_t = dot3(cr, e) / sqrt(dot3(e, e)), cos_t = dot3(N, NB);
+        const double c0 = p.hinge_rest[6 * t + 2 * s], s0 = p.hinge_rest[6 * t + 2 * s + 1];
+        acc += 0.5 * double(p.k_b) * (1.0 - (cos_t * c0 + sin_t * s0));
+      }
+    }
+    for (int i = threadIdx.x; i < n; i += NT) {
+      double di[3], u[3];
+      const double w0 = p.vtx_w[i];
+      for (int k = 0; k < 3; ++k) {
+        di[k] = double(p.d[base + k * n_pad + i]);
+        u[k] = w0 * di[k];
+      }
+      for (int q = 0; q < p.valence_max; ++q) {
+        const int j = p.vtx_nbr[q * n + i];
+        const double w = p.vtx_w[(q + 1) * n + i];
+        for (int k = 0; k < 3; ++k) u[k] += w * double(p.d[base + k * n_pad + j]);
+      }
+      const double dd = dot3(di, di), du = dot3(di, u), uu = dot3(u, u);
+      acc += 0.5 * (double(p.inertia_coef) * double(p.vtx_mass[i]) * dd +
+                    double(p.beta_over_h) * (double(p.k_mem) * du + double(p.k_b) * double(p.vtx_inv_area[i]) * uu));
+      for (int k = 0; k < 3; ++k) acc -= di[k] * double(p.b[base + k * n_pad + i]);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+      acc += __shfl_xor_sync(0xffffffffu, acc, o);
+      vol += __shfl_xor_sync(0xffffffffu, vol, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+      red[0][threadIdx.x >> 5] = acc;
+      red[1][threadIdx.x >> 5] = vol;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      double sa = 0.0, sv = 0.0;
+      for (int i = 0; i < NT / 32; ++i) {
+        sa += red[0][i];
+        sv += red[1][i];
+      }
+      const double V = sv / 6.0, V0 = double(p.V0);
+      out_row[cell_id ? cell_id[cell] : cell] = sa + 0.5 * double(p.kv_over_V0) * (V - V0) * (V - V0);
+    }
+    __syncthreads();   // red and the staged cell are reused by the next cell
+  }
+}
+
 template <typename T>
 LocalParams<T> make_params(const TypeDev &td, const BucketView &bv) {
   LocalParams<T> p;
@@ -383,15 +478,30 @@ int launch_local_generic(const TypeDev &td, const BucketView &bv, void *scratch,
                                 : launch_local_T<double>(td, bv, scratch, n_sm, s);
 }
 
-int launch_objective(const TypeDev &td, const BucketView &bv, const int64_t *cell_id_dev, double *objective_row,
-                     const int *skip_dev, int precision, cudaStream_t s) {
-  if (bv.cells == 0) return 0;
-  const unsigned grid = unsigned(bv.cells < 148 * 8 ? bv.cells : 148 * 8);
-  if (precision == NPFEM_F32)
-    objective_kernel<float><<<grid, 256, 0, s>>>(make_params<float>(td, bv), cell_id_dev, objective_row, skip_dev, td.h);
-  else
-    objective_kernel<double><<<grid, 256, 0, s>>>(make_params<double>(td, bv), cell_id_dev, objective_row, skip_dev, td.h);
+template <typename T>
+int launch_objective_T(const TypeDev &td, const BucketView &bv, const int64_t *cell_id_dev, double *objective_row,
+                       const int *skip_dev, int n_sm, cudaStream_t s) {
+  const LocalParams<T> p = make_params<T>(td, bv);
+  const size_t smem = sizeof(double) * (size_t(3) * td.n + size_t(3) * td.T);
+  if (smem <= 56 * 1024) {                    // 4 CTAs of 256 threads per SM (RBC-642: 46 KB each)
+    cudaFuncSetAttribute(objective_smem_kernel<T, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 56 * 1024);
+    const int64_t cap = int64_t(n_sm) * 4 * 4;
+    objective_smem_kernel<T, 256><<<unsigned(bv.cells < cap ? bv.cells : cap), 256, smem, s>>>(p, cell_id_dev, objective_row, skip_dev);
+  } else if (smem <= kMaxSmem) {              // one CTA of 1024 threads per SM (RBC-2562: 184 KB)
+    cudaFuncSetAttribute(objective_smem_kernel<T, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kMaxSmem));
+    const int64_t cap = int64_t(n_sm) * 4;
+    objective_smem_kernel<T, 1024><<<unsigned(bv.cells < cap ? bv.cells : cap), 1024, smem, s>>>(p, cell_id_dev, objective_row, skip_dev);
+  } else {
+    objective_kernel<T><<<unsigned(bv.cells < 148 * 8 ? bv.cells : 148 * 8), 256, 0, s>>>(p, cell_id_dev, objective_row, skip_dev, td.h);
+  }
   return 1;
+}
+
+int launch_objective(const TypeDev &td, const BucketView &bv, const int64_t *cell_id_dev, double *objective_row,
+                     const int *skip_dev, int precision, int n_sm, cudaStream_t s) {
+  if (bv.cells == 0) return 0;
+  return precision == NPFEM_F32 ? launch_objective_T<float>(td, bv, cell_id_dev, objective_row, skip_dev, n_sm, s)
+                                : launch_objective_T<double>(td, bv, cell_id_dev, objective_row, skip_dev, n_sm, s);
 }
 
 }  // namespace npfem
