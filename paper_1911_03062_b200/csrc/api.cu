@@ -744,17 +744,26 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
     if (c->diagnostics && (rc = diag(k))) return rc;
     for (size_t t = 0; t < nb; ++t) {
       if (whole[t]) continue;
-      const bool f32 = c->precision == NPFEM_F32 && !ls_on;   // the line search needs the FULL gradient: generic kernel
+      // the line search needs the FULL gradient: fp32 contexts take the fast kernels' reduced gradient and add the
+      // damping part to it (launch_damping_grad), fp64 contexts take the generic kernel
+      const bool f32 = c->precision == NPFEM_F32 &&
+                       (!ls_on || size_t(24) * size_t(c->types[t].n) <= size_t(200) * 1024);
       const bool sched = f32 && (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]);
       const bool fast = f32 && !sched && (c->opt_local_impl == 0 || c->opt_local_impl == 2) && local_smem_supported(c->types[t]);
       const bool big = f32 && !sched && !fast && (c->opt_local_impl == 0 || c->opt_local_impl == 4) && local_big_supported(c->types[t]);
-      const double d_scale = (sched || fast || big) ? 1.0 - c->types[t].gamma : 1.0;
+      const bool reduced = sched || fast || big;
+      const double d_scale = reduced && !ls_on ? 1.0 - c->types[t].gamma : 1.0;
+      BucketView lv = c->views[t];
+      if (ls_on && reduced) lv.g_tf32 = 0;                    // rounded once, after the damping part is in
       if ((rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "local step", [&] {
-             if (sched) return launch_local_sched(c->types[t], c->views[t], c->n_sm, fused[t] && k > 0, d_scale, c->stream);
-             if (fast) return launch_local_smem(c->types[t], c->views[t], c->n_sm, c->stream);
-             if (big) return launch_local_big(c->types[t], c->views[t], c->n_sm, c->stream);
-             return launch_local_generic(c->types[t], c->views[t], c->buckets[t].scratch, c->precision, c->n_sm,
+             if (sched) return launch_local_sched(c->types[t], lv, c->n_sm, fused[t] && k > 0, d_scale, c->stream);
+             if (fast) return launch_local_smem(c->types[t], lv, c->n_sm, c->stream);
+             if (big) return launch_local_big(c->types[t], lv, c->n_sm, c->stream);
+             return launch_local_generic(c->types[t], lv, c->buckets[t].scratch, c->precision, c->n_sm,
                                          c->stream); })))
+        return rc;
+      if (ls_on && reduced && (rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "damping gradient", [&] {
+                                 return launch_damping_grad(c->types[t], c->views[t], c->n_sm, c->stream); })))
         return rc;
       if (c->col_active && c->buckets[t].cells &&
           (rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "collision gradient", [&] {

@@ -143,6 +143,9 @@ struct LineSearchDev {
   double *obj0 = nullptr, *obj1 = nullptr, *slope = nullptr, *alpha = nullptr;   // [cells]
   int *done = nullptr;                                                            // [cells]
 };
+// fp32: g (reduced gradient of a fast local-step kernel) += gamma m^ d + (beta/h) L z -> the full gradient;
+// rounds to TF32 when bv.g_tf32.  Returns -1 when the cell does not fit shared memory.
+int launch_damping_grad(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
 // after the global step: d holds d_old + p, u holds d_old, g the gradient.  slope = <g, p>, alpha = 1,
 // done = frozen (||g|| <= grad_tol ||b||: alpha = 0, d restored); g is overwritten with p
 int launch_ls_init(const BucketView &bv, const LineSearchDev &ls, double grad_tol, int precision, cudaStream_t s);

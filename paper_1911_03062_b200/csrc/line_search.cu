@@ -94,12 +94,90 @@ ls_accept_kernel(BucketView bv, LineSearchDev ls, double c1, int last) {
   }
 }
 
+// The fast local-step kernels store the REDUCED gradient r = (1 - gamma) m^ d - b + grad E; the
+// line search needs the full one (slope, gradient norm; the global step then runs with d_scale = 1):
+//   grad g = r + gamma m^ d + (beta/h) L z,   z = k_mem d + k_b A^-1 L d   (L = cotangent stencil)
+// One CTA per cell, d and z in shared memory; same arithmetic order as the generic local step's stencil.
+struct DampingParams {
+  int n, n_pad, valence_max, g_tf32;
+  const int *vtx_nbr;
+  const float *vtx_w, *vtx_mass, *vtx_inv_area;
+  float k_mem, k_b, beta_over_h, gamma_inertia;   // gamma (1 + h alpha) / h^2
+  const float *d;
+  float *g;
+  int64_t cells;
+};
+
+__global__ void __launch_bounds__(256)
+damping_grad_kernel(const DampingParams p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int n = p.n, n_pad = p.n_pad;
+  float *sd = reinterpret_cast<float *>(smem_raw);   // [3][n]
+  float *sz = sd + 3 * n;                             // [3][n]
+  for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x) {
+    const size_t base = size_t(cell) * 3 * n_pad;
+    for (int k = 0; k < 3; ++k)
+      for (int i = threadIdx.x; i < n; i += blockDim.x) sd[k * n + i] = p.d[base + k * n_pad + i];
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+      const float w0 = p.vtx_w[i];
+      float u[3] = {w0 * sd[i], w0 * sd[n + i], w0 * sd[2 * n + i]};
+      for (int q = 0; q < p.valence_max; ++q) {
+        const int j = p.vtx_nbr[q * n + i];
+        const float w = p.vtx_w[(q + 1) * n + i];
+        u[0] += w * sd[j];
+        u[1] += w * sd[n + j];
+        u[2] += w * sd[2 * n + j];
+      }
+      const float s = p.k_b * p.vtx_inv_area[i];
+      for (int k = 0; k < 3; ++k) sz[k * n + i] = p.k_mem * sd[k * n + i] + s * u[k];
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+      const float w0 = p.vtx_w[i];
+      float lz[3] = {w0 * sz[i], w0 * sz[n + i], w0 * sz[2 * n + i]};
+      for (int q = 0; q < p.valence_max; ++q) {
+        const int j = p.vtx_nbr[q * n + i];
+        const float w = p.vtx_w[(q + 1) * n + i];
+        for (int k = 0; k < 3; ++k) lz[k] += w * sz[k * n + j];
+      }
+      const float mi = p.gamma_inertia * p.vtx_mass[i];
+      for (int k = 0; k < 3; ++k) {
+        const float gk = p.g[base + k * n_pad + i] + mi * sd[k * n + i] + p.beta_over_h * lz[k];
+        p.g[base + k * n_pad + i] = p.g_tf32 ? tf32_rn(gk) : gk;
+      }
+    }
+    __syncthreads();
+  }
+}
+
 unsigned warp_grid(int64_t cells) {
   const int64_t ctas = (cells + 3) / 4;
   return unsigned(ctas < 148 * 16 ? ctas : 148 * 16);
 }
 
 }  // namespace
+
+int launch_damping_grad(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s) {
+  if (bv.cells == 0 || td.beta_over_h == 0.0) return 0;
+  DampingParams p;
+  p.n = td.n; p.n_pad = td.n_pad; p.valence_max = td.valence_max; p.g_tf32 = bv.g_tf32;
+  p.vtx_nbr = td.vtx_nbr;
+  p.vtx_w = static_cast<const float *>(td.vtx_w);
+  p.vtx_mass = static_cast<const float *>(td.vtx_mass);
+  p.vtx_inv_area = static_cast<const float *>(td.vtx_inv_area);
+  p.k_mem = float(td.k_mem); p.k_b = float(td.k_b); p.beta_over_h = float(td.beta_over_h);
+  p.gamma_inertia = float(td.gamma * td.inertia_coef);
+  p.d = static_cast<const float *>(bv.field[F_D]);
+  p.g = static_cast<float *>(bv.field[F_G]);
+  p.cells = bv.cells;
+  const size_t smem = sizeof(float) * 6 * size_t(td.n);
+  if (smem > 200 * 1024) return -1;
+  cudaFuncSetAttribute(damping_grad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  const int64_t cap = int64_t(n_sm) * 8 * 2;
+  damping_grad_kernel<<<unsigned(bv.cells < cap ? bv.cells : cap), 256, smem, s>>>(p);
+  return 1;
+}
 
 int launch_ls_init(const BucketView &bv, const LineSearchDev &ls, double grad_tol, int precision, cudaStream_t s) {
   if (bv.cells == 0) return 0;

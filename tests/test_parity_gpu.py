@@ -269,6 +269,48 @@ def test_line_search_violent_case_matches_oracle(precision):
         assert np.all(np.isin(alpha, 0.5 ** np.arange(0, 9)))
 
 
+def test_line_search_fp32_fast_kernels_match_the_generic_full_gradient():
+    """fp32 line search: the fast local kernels' reduced gradient + the damping part (launch_damping_grad)
+    against the generic kernel's full gradient (OPT_LOCAL_STEP_IMPL = 1) and against the oracle, on the
+    violent case (which backtracks) and on mixed RBC-642 / PLT-162 cells."""
+    import torch
+    from oracle import npfem_oracle as orc
+    from paper_1911_03062_b200 import Solver, binding
+    pop = _ls_population(9, 30.0, 3000.0, seed=21)
+    td = orc.make_type(pop.types[0], pop.dt)
+    assert td.beta > 0.0                                             # the damping part is not zero here
+    xr, _ = orc.step_line_search(pop.positions[0], pop.velocities[0], pop.forces(0)[0], td, 15, max_halvings=8, c1=1e-4)
+    out = {}
+    for impl in (0, 1):
+        solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision="fp32")
+        solver.set_option(binding.OPT_LOCAL_STEP_IMPL, impl)
+        solver.set_line_search(8, 1e-4, 0.0)
+        solver.set_state(torch.from_numpy(pop.packed(pop.positions)).cuda())
+        solver.set_forces(torch.from_numpy(pop.packed(pop.forces(0))).cuda())
+        solver.step(15)
+        x, _ = solver.get_state()
+        out[impl] = pop.unpack(x.cpu().numpy())[0]
+        solver.close()
+    x0 = pop.positions[0]
+    for impl in (0, 1):
+        print("impl", impl, "disp error vs oracle", rel_l2(out[impl] - x0, xr - x0))
+        assert rel_l2(out[impl] - x0, xr - x0) <= TOL_DISP["fp32"]
+    pop = make_config(3, n_cells=40)
+    ref = run_oracle(pop, 2, 5)                                      # full steps descend here: plain oracle
+    solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision="fp32")
+    solver.set_line_search(4)
+    solver.set_state(torch.from_numpy(pop.packed(pop.positions)).cuda())
+    for s in range(2):
+        solver.set_forces(torch.from_numpy(pop.packed(pop.forces(s))).cuda())
+        solver.step(5)
+    x, _ = solver.get_state()
+    assert np.all(solver.get_step_lengths() == 1.0)
+    solver.close()
+    xs = pop.unpack(x.cpu().numpy())
+    for t in range(2):
+        assert rel_l2(xs[t], ref[t][0]) <= 1e-4
+
+
 def test_line_search_is_neutral_on_a_tame_case_and_freezes_by_tolerance():
     import torch
     from paper_1911_03062_b200 import Solver
