@@ -730,6 +730,30 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
       l.alpha = l.slope + cells;
       l.done = static_cast<int *>(pi);
     }
+    // fp32 + tensor-core global step: TF32 rounding of g and H~^-1 (2^-11 per entry) spoils the search direction in
+    // the stiff modes - on the violent case of tests/test_parity_gpu.py every cell ends up rejecting all step
+    // lengths by iteration 11 - so the line search takes its direction from a 3xTF32 product (fp32-grade)
+    for (size_t t = 0; t < nb; ++t) {
+      LineSearchDev &l = c->ls[t];
+      const size_t cells = size_t(c->buckets[t].cells);
+      if (l.g_lo || cells == 0 || c->precision != NPFEM_F32 || c->opt_global_math != 0 || !c->types[t].Hinv_tf32 ||
+          !global_tcgen05_supported(c->types[t]))
+        continue;
+      const size_t nn = size_t(c->types[t].n_pad) * c->types[t].n_pad;
+      void *pg = nullptr, *pw = nullptr;
+      if (cudaMalloc(&pg, cells * 3 * c->types[t].n_pad * sizeof(float)) != cudaSuccess ||
+          cudaMalloc(&pw, nn * sizeof(float)) != cudaSuccess) {
+        cudaGetLastError();
+        cudaFree(pg);
+        return fail(c, NPFEM_ENOMEM, "cannot allocate the line-search operands");
+      }
+      l.g_lo = static_cast<float *>(pg);
+      l.w_lo = static_cast<float *>(pw);
+      if ((rc = check_launch(c, launch_ls_split_w(static_cast<const float *>(c->types[t].Hinv),
+                                                  static_cast<const float *>(c->types[t].Hinv_tf32), l.w_lo, nn, c->stream),
+                             "line search: split of H~^-1")))
+        return rc;
+    }
   }
   std::vector<char> fused(nb, 0);
   for (size_t t = 0; t < nb; ++t)
@@ -739,7 +763,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   // g feeds the TF32 tensor-core GEMM: the local step stores it already rounded to nearest (the line search
   // then takes its slope and gradient norm from the rounded gradient: 2^-12 relative per entry, random sign)
   for (size_t t = 0; t < nb; ++t)
-    c->views[t].g_tf32 = c->precision == NPFEM_F32 && c->opt_global_math == 0 && global_tcgen05_supported(c->types[t]);
+    c->views[t].g_tf32 = !ls_on && c->precision == NPFEM_F32 && c->opt_global_math == 0 && global_tcgen05_supported(c->types[t]);
   for (int k = 0; k < n_iterations; ++k) {
     if (c->diagnostics && (rc = diag(k))) return rc;
     for (size_t t = 0; t < nb; ++t) {
@@ -753,8 +777,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
       const bool big = f32 && !sched && !fast && (c->opt_local_impl == 0 || c->opt_local_impl == 4) && local_big_supported(c->types[t]);
       const bool reduced = sched || fast || big;
       const double d_scale = reduced && !ls_on ? 1.0 - c->types[t].gamma : 1.0;
-      BucketView lv = c->views[t];
-      if (ls_on && reduced) lv.g_tf32 = 0;                    // rounded once, after the damping part is in
+      const BucketView &lv = c->views[t];
       if ((rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "local step", [&] {
              if (sched) return launch_local_sched(c->types[t], lv, c->n_sm, fused[t] && k > 0, d_scale, c->stream);
              if (fast) return launch_local_smem(c->types[t], lv, c->n_sm, c->stream);
@@ -762,8 +785,12 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
              return launch_local_generic(c->types[t], lv, c->buckets[t].scratch, c->precision, c->n_sm,
                                          c->stream); })))
         return rc;
+      // 3xTF32 operands of the line search's global step: split by the damping kernel, unless the collision term is
+      // still to come or the generic kernel ran (then by launch_ls_split_g just before the GEMMs)
+      const bool split_early = ls_on && reduced && !c->col_active && c->ls[t].g_lo;
       if (ls_on && reduced && (rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "damping gradient", [&] {
-                                 return launch_damping_grad(c->types[t], c->views[t], c->n_sm, c->stream); })))
+                                 return launch_damping_grad(c->types[t], c->views[t], split_early ? c->ls[t].g_lo : nullptr,
+                                                            c->n_sm, c->stream); })))
         return rc;
       if (c->col_active && c->buckets[t].cells &&
           (rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "collision gradient", [&] {
@@ -782,6 +809,15 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
         NPFEM_CUDA(c, cudaMemcpyAsync(c->views[t].field[F_U], c->views[t].field[F_D], bytes, cudaMemcpyDeviceToDevice, c->stream));
       }
       if ((rc = timed_launch(c, NPFEM_KIND_GLOBAL, int(t), "global step", [&] {
+             if (ls_on && c->ls[t].g_lo) {     // 3xTF32: d <- d - (g_hi W_hi + g_lo W_hi + g_hi W_lo)
+               const LineSearchDev &l = c->ls[t];
+               const size_t count = size_t(c->buckets[t].cells) * 3 * c->types[t].n_pad;
+               int nl = split_early ? 0 : launch_ls_split_g(static_cast<float *>(c->views[t].field[F_G]), l.g_lo, count, c->stream);
+               const int n1 = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, 1.0, nullptr, c->stream);
+               const int n2 = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, 1.0, nullptr, c->stream, l.g_lo, nullptr);
+               const int n3 = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, 1.0, nullptr, c->stream, nullptr, l.w_lo);
+               return n1 < 0 || n2 < 0 || n3 < 0 ? -1 : nl + n1 + n2 + n3;
+             }
              if (c->precision == NPFEM_F32 && c->opt_global_math == 0) {
                const int n = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, d_scale,
                                                    fused[t] ? c->views[t].field[F_U] : nullptr, c->stream);
@@ -1160,6 +1196,8 @@ void npfem_destroy(npfem_ctx *c) {
   }
   if (c->col_dev) cudaFree(c->col_dev);
   for (auto &l : c->ls) {
+    if (l.g_lo) cudaFree(l.g_lo);
+    if (l.w_lo) cudaFree(l.w_lo);
     if (l.obj0) cudaFree(l.obj0);
     if (l.done) cudaFree(l.done);
   }

@@ -359,8 +359,9 @@ bool global_tcgen05_supported(const TypeDev &td) {
 
 // d <- d_scale d - g Hinv (u_out == nullptr) or u_out <- -g Hinv.  Returns #launches, or -1 if the
 // configuration is unsupported (caller falls back to the SIMT GEMM).
+// g_op / w_op: other operands than bv.field[F_G] / the type's TF32 H~^-1 (the line search's 3xTF32 product).
 int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, double d_scale, void *u_out,
-                          cudaStream_t s) {
+                          cudaStream_t s, const void *g_op, const void *w_op) {
   if (bv.cells == 0) return 0;
   GemmParams p{};
   if (!gemm_shape(td, p)) return -1;
@@ -370,8 +371,8 @@ int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, dou
   p.m_tiles = (p.rows + BM - 1) / BM;
   p.d_scale = float(d_scale);
   CUtensorMap map_g, map_w, map_d;
-  if (!make_map(&map_g, bv.field[F_G], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), BM)) return -1;
-  if (!make_map(&map_w, td.Hinv_tf32 ? td.Hinv_tf32 : td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n_pass / CL)))
+  if (!make_map(&map_g, g_op ? g_op : bv.field[F_G], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), BM)) return -1;
+  if (!make_map(&map_w, w_op ? w_op : td.Hinv_tf32 ? td.Hinv_tf32 : td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n_pass / CL)))
     return -1;
   // epilogue tiles: [32 rows][32 columns] of D (in-place update) or of U (product out)
   if (!make_map(&map_d, u_out ? u_out : bv.field[F_D], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), 32))

@@ -142,10 +142,18 @@ int launch_objective(const TypeDev &td, const BucketView &bv, const int64_t *cel
 struct LineSearchDev {
   double *obj0 = nullptr, *obj1 = nullptr, *slope = nullptr, *alpha = nullptr;   // [cells]
   int *done = nullptr;                                                            // [cells]
+  // fp32 contexts whose global step runs on the TF32 tensor cores: the search direction comes from a 3xTF32
+  // product (g = g_hi + g_lo, H~^-1 = W_hi + W_lo, the lo x lo term dropped), see launch_ls_split_g
+  float *g_lo = nullptr;                                                          // [cells][3][n_pad]
+  float *w_lo = nullptr;                                                          // [n_pad][n_pad]
 };
+// g <- tf32(g), g_lo <- tf32(g - tf32(g)) over count elements; w_lo <- tf32(w - w_hi)
+int launch_ls_split_g(float *g, float *g_lo, size_t count, cudaStream_t s);
+int launch_ls_split_w(const float *w, const float *w_hi, float *w_lo, size_t count, cudaStream_t s);
 // fp32: g (reduced gradient of a fast local-step kernel) += gamma m^ d + (beta/h) L z -> the full gradient;
 // rounds to TF32 when bv.g_tf32.  Returns -1 when the cell does not fit shared memory.
-int launch_damping_grad(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
+// g_lo != nullptr: also leaves the 3xTF32 split g = tf32(grad), g_lo = tf32(grad - g) (launch_ls_split_g)
+int launch_damping_grad(const TypeDev &td, const BucketView &bv, float *g_lo, int n_sm, cudaStream_t s);
 // after the global step: d holds d_old + p, u holds d_old, g the gradient.  slope = <g, p>, alpha = 1,
 // done = frozen (||g|| <= grad_tol ||b||: alpha = 0, d restored); g is overwritten with p
 int launch_ls_init(const BucketView &bv, const LineSearchDev &ls, double grad_tol, int precision, cudaStream_t s);
@@ -158,7 +166,7 @@ int launch_global_simt(const TypeDev &td, const BucketView &bv, int precision, d
 bool global_tcgen05_supported(const TypeDev &td);
 // u_out == nullptr: d <- d_scale d - g Hinv;  else u_out <- -g Hinv (the next local step / the epilogue applies it)
 int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, double d_scale, void *u_out,
-                          cudaStream_t s);
+                          cudaStream_t s, const void *g_op = nullptr, const void *w_op = nullptr);
 
 // fp32 fast local step; writes the reduced gradient (global step must then use d_scale = 1 - gamma)
 bool local_smem_supported(const TypeDev &td);

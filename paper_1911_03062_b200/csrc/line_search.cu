@@ -20,37 +20,52 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
+// 16-byte accesses over the PADDED rows (n_pad is a multiple of 16, padding columns are zero in every field)
+template <typename T> struct Vec16;
+template <> struct Vec16<float> { typedef float4 type; };
+template <> struct Vec16<double> { typedef double2 type; };
+
 template <typename T>
 __global__ void __launch_bounds__(128)
 ls_init_kernel(BucketView bv, LineSearchDev ls, double grad_tol) {
+  typedef typename Vec16<T>::type V;
+  constexpr int W = int(sizeof(V) / sizeof(T));
   const int lane = threadIdx.x & 31;
   const int64_t warp0 = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) >> 5;
   const int64_t n_warps = (int64_t(gridDim.x) * blockDim.x) >> 5;
-  const int n = bv.n, n_pad = bv.n_pad;
+  const int nv = 3 * bv.n_pad / W;               // vectors per cell
   for (int64_t cell = warp0; cell < bv.cells; cell += n_warps) {
-    const size_t base = size_t(cell) * 3 * n_pad;
-    T *g = static_cast<T *>(bv.field[F_G]) + base;
-    T *d = static_cast<T *>(bv.field[F_D]) + base;
-    const T *d_old = static_cast<const T *>(bv.field[F_U]) + base;
-    const T *b = static_cast<const T *>(bv.field[F_B]) + base;
+    const size_t base = size_t(cell) * 3 * bv.n_pad;
+    V *g = reinterpret_cast<V *>(static_cast<T *>(bv.field[F_G]) + base);
+    V *d = reinterpret_cast<V *>(static_cast<T *>(bv.field[F_D]) + base);
+    const V *d_old = reinterpret_cast<const V *>(static_cast<const T *>(bv.field[F_U]) + base);
+    const V *b = reinterpret_cast<const V *>(static_cast<const T *>(bv.field[F_B]) + base);
+    const float4 *g_lo = ls.g_lo ? reinterpret_cast<const float4 *>(ls.g_lo + base) : nullptr;   // 3xTF32 mode: gradient = g + g_lo
     double slope = 0.0, gg = 0.0, bb = 0.0;
-    for (int k = 0; k < 3; ++k)
-      for (int i = lane; i < n; i += 32) {
-        const int o = k * n_pad + i;
-        const T p = d[o] - d_old[o];            // the search direction, rounded once to the compute type
-        const double gi = double(g[o]), bi = double(b[o]);
+    for (int i = lane; i < nv; i += 32) {
+      V gv = g[i];
+      const V dv = d[i], ov = d_old[i], bv4 = b[i];
+      T *ge = reinterpret_cast<T *>(&gv);
+      const T *de = reinterpret_cast<const T *>(&dv), *oe = reinterpret_cast<const T *>(&ov), *be = reinterpret_cast<const T *>(&bv4);
+      float lo[4] = {0.f, 0.f, 0.f, 0.f};
+      if (sizeof(T) == 4 && g_lo) *reinterpret_cast<float4 *>(lo) = g_lo[i];
+#pragma unroll
+      for (int e = 0; e < W; ++e) {
+        const T p = de[e] - oe[e];                // the search direction, rounded once to the compute type
+        const double gi = double(ge[e]) + double(lo[e]), bi = double(be[e]);
         slope += gi * double(p);
         gg += gi * gi;
         bb += bi * bi;
-        g[o] = p;                               // the gradient is not needed any more: keep p in its place
+        ge[e] = p;                                // the gradient is not needed any more: keep p in its place
       }
+      g[i] = gv;
+    }
     slope = warp_sum(slope);
     gg = warp_sum(gg);
     bb = warp_sum(bb);
     const bool frozen = sqrt(gg) <= grad_tol * sqrt(bb);
     if (frozen)
-      for (int k = 0; k < 3; ++k)
-        for (int i = lane; i < n; i += 32) d[k * n_pad + i] = d_old[k * n_pad + i];
+      for (int i = lane; i < nv; i += 32) d[i] = d_old[i];
     if (lane == 0) {
       ls.slope[cell] = slope;
       ls.alpha[cell] = frozen ? 0.0 : 1.0;
@@ -105,6 +120,7 @@ struct DampingParams {
   float k_mem, k_b, beta_over_h, gamma_inertia;   // gamma (1 + h alpha) / h^2
   const float *d;
   float *g;
+  float *g_lo;                                     // != nullptr: g <- tf32(grad), g_lo <- tf32(grad - g) (3xTF32 operands)
   int64_t cells;
 };
 
@@ -144,11 +160,30 @@ damping_grad_kernel(const DampingParams p) {
       const float mi = p.gamma_inertia * p.vtx_mass[i];
       for (int k = 0; k < 3; ++k) {
         const float gk = p.g[base + k * n_pad + i] + mi * sd[k * n + i] + p.beta_over_h * lz[k];
-        p.g[base + k * n_pad + i] = p.g_tf32 ? tf32_rn(gk) : gk;
+        if (p.g_lo) {
+          const float hi = tf32_rn(gk);
+          p.g[base + k * n_pad + i] = hi;
+          p.g_lo[base + k * n_pad + i] = tf32_rn(gk - hi);
+        } else {
+          p.g[base + k * n_pad + i] = p.g_tf32 ? tf32_rn(gk) : gk;
+        }
       }
     }
     __syncthreads();
   }
+}
+
+__global__ void __launch_bounds__(256) split_g_kernel(float *__restrict__ g, float *__restrict__ g_lo, size_t count) {
+  for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < count; i += size_t(gridDim.x) * blockDim.x) {
+    const float v = g[i], hi = tf32_rn(v);
+    g[i] = hi;
+    g_lo[i] = tf32_rn(v - hi);
+  }
+}
+__global__ void __launch_bounds__(256) split_w_kernel(const float *__restrict__ w, const float *__restrict__ w_hi,
+                                                     float *__restrict__ w_lo, size_t count) {
+  for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < count; i += size_t(gridDim.x) * blockDim.x)
+    w_lo[i] = tf32_rn(w[i] - w_hi[i]);
 }
 
 unsigned warp_grid(int64_t cells) {
@@ -158,8 +193,10 @@ unsigned warp_grid(int64_t cells) {
 
 }  // namespace
 
-int launch_damping_grad(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s) {
-  if (bv.cells == 0 || td.beta_over_h == 0.0) return 0;
+int launch_damping_grad(const TypeDev &td, const BucketView &bv, float *g_lo, int n_sm, cudaStream_t s) {
+  if (bv.cells == 0) return 0;
+  if (td.beta_over_h == 0.0)   // nothing to add: only the split, if asked for
+    return g_lo ? launch_ls_split_g(static_cast<float *>(bv.field[F_G]), g_lo, size_t(bv.cells) * 3 * td.n_pad, s) : 0;
   DampingParams p;
   p.n = td.n; p.n_pad = td.n_pad; p.valence_max = td.valence_max; p.g_tf32 = bv.g_tf32;
   p.vtx_nbr = td.vtx_nbr;
@@ -170,12 +207,27 @@ int launch_damping_grad(const TypeDev &td, const BucketView &bv, int n_sm, cudaS
   p.gamma_inertia = float(td.gamma * td.inertia_coef);
   p.d = static_cast<const float *>(bv.field[F_D]);
   p.g = static_cast<float *>(bv.field[F_G]);
+  p.g_lo = g_lo;
   p.cells = bv.cells;
   const size_t smem = sizeof(float) * 6 * size_t(td.n);
   if (smem > 200 * 1024) return -1;
   cudaFuncSetAttribute(damping_grad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   const int64_t cap = int64_t(n_sm) * 8 * 2;
   damping_grad_kernel<<<unsigned(bv.cells < cap ? bv.cells : cap), 256, smem, s>>>(p);
+  return 1;
+}
+
+int launch_ls_split_g(float *g, float *g_lo, size_t count, cudaStream_t s) {
+  if (count == 0) return 0;
+  const size_t ctas = (count + 1023) / 1024;
+  split_g_kernel<<<unsigned(ctas < 148 * 16 ? ctas : 148 * 16), 256, 0, s>>>(g, g_lo, count);
+  return 1;
+}
+
+int launch_ls_split_w(const float *w, const float *w_hi, float *w_lo, size_t count, cudaStream_t s) {
+  if (count == 0) return 0;
+  const size_t ctas = (count + 1023) / 1024;
+  split_w_kernel<<<unsigned(ctas < 148 * 16 ? ctas : 148 * 16), 256, 0, s>>>(w, w_hi, w_lo, count);
   return 1;
 }
 

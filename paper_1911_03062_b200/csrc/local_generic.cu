@@ -307,7 +307,7 @@ objective_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_id, do
 
 // ---- objective, shared-memory version (line search): the same sum as objective_kernel
 // with x_n + d and the UNIT triangle normals of the cell staged once in shared memory in fp64, so a hinge
-// costs one rsqrt (|e|) instead of three neighbour-normal cross products, two sqrt and a division.
+// costs one rsqrt (1/|e|) instead of three neighbour-normal cross products, two sqrt and a division.
 // Shared memory: 8 (3 n + 3 T) bytes (RBC-642: 46 KB, RBC-2562: 184 KB); larger meshes keep objective_kernel.
 template <typename T, int NT>
 __global__ void __launch_bounds__(NT)
@@ -341,7 +341,7 @@ objective_smem_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_i
       const double C11 = a * a * e11, C12 = a * (b * e11 + c * e12), C22 = b * b * e11 + 2 * b * c * e12 + c * c * e22;
       const double I1 = C11 + C22 - 2.0, I2 = C11 * C22 - C12 * C12 - 1.0;
       acc += A0 * (double(p.B4) * (0.5 * I1 * I1 + I1 - I2) + 0.5 * double(p.C4) * I2 * I2);
-      const double rn = 1.0 / sqrt(dot3(N, N));
+      const double rn = rsqrt(dot3(N, N));
       for (int k = 0; k < 3; ++k) sn[3 * t + k] = N[k] * rn;
     }
     __syncthreads();
@@ -356,7 +356,7 @@ objective_smem_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_i
         double e[3], cr[3];
         for (int k = 0; k < 3; ++k) e[k] = sp[k * n + vs[(s + 1) % 3]] - sp[k * n + vs[s]];
         cross3(N, NB, cr);
-        const double sin_t = dot3(cr, e) / sqrt(dot3(e, e)), cos_t = dot3(N, NB);
+        const double sin_t = dot3(cr, e) * rsqrt(dot3(e, e)), cos_t = dot3(N, NB);
         const double c0 = p.hinge_rest[6 * t + 2 * s], s0 = p.hinge_rest[6 * t + 2 * s + 1];
         acc += 0.5 * double(p.k_b) * (1.0 - (cos_t * c0 + sin_t * s0));
       }

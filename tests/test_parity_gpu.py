@@ -267,6 +267,11 @@ def test_line_search_violent_case_matches_oracle(precision):
         assert np.array_equal(alpha, hist["alpha"][-1])
     else:
         assert np.all(np.isin(alpha, 0.5 ** np.arange(0, 9)))
+        # the search must not stall: with a plain TF32 search direction every cell rejected all nine step lengths
+        # from iteration 11 on (alpha = 2^-8 everywhere, displacement error 2.7e-3); the 3xTF32 direction tracks the
+        # oracle's step lengths (1.6e-4)
+        assert np.median(alpha) > 0.5 ** 8
+        assert rel_l2(xg - x0, xr - x0) <= 1e-3
 
 
 def test_line_search_fp32_fast_kernels_match_the_generic_full_gradient():
