@@ -142,11 +142,12 @@ def test_zero_cells_and_empty_bucket():
     empty.close()
 
 
+@pytest.mark.parametrize("config", [2, 5])     # 5: RBC-2562, the objective kernel's one-CTA-per-SM variant
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
-def test_objective_history_matches_oracle(precision):
+def test_objective_history_matches_oracle(precision, config):
     from oracle import npfem_oracle as orc
     from paper_1911_03062_b200 import binding
-    pop = make_config(2, n_cells=4)
+    pop = make_config(config, n_cells=4)
     gpu, solver = run_gpu(pop, precision, n_steps=1, n_iterations=6,
                           options=[(binding.OPT_DIAGNOSTICS, 1)])
     hist, mono = solver.get_objective()
