@@ -305,6 +305,18 @@ objective_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_id, do
   (void)h;
 }
 
+// two consecutive table entries with one 8- / 16-byte load (a strided scalar load costs a wavefront per 128 bytes touched)
+__device__ __forceinline__ void load_pair(const float *p, double &a, double &b) {
+  const float2 v = *reinterpret_cast<const float2 *>(p);
+  a = double(v.x);
+  b = double(v.y);
+}
+__device__ __forceinline__ void load_pair(const double *p, double &a, double &b) {
+  const double2 v = *reinterpret_cast<const double2 *>(p);
+  a = v.x;
+  b = v.y;
+}
+
 // ---- objective, shared-memory version (line search): the same sum as objective_kernel
 // with x_n + d and the UNIT triangle normals of the cell staged once in shared memory in fp64, so a hinge
 // costs one rsqrt (1/|e|) instead of three neighbour-normal cross products, two sqrt and a division.
@@ -336,7 +348,9 @@ objective_smem_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_i
       }
       cross3(e1, e2, N);
       vol += dot3(x0, N);
-      const double a = p.tri_rest[4 * t], b = p.tri_rest[4 * t + 1], c = p.tri_rest[4 * t + 2], A0 = p.tri_rest[4 * t + 3];
+      double a, b, c, A0;
+      load_pair(p.tri_rest + 4 * t, a, b);
+      load_pair(p.tri_rest + 4 * t + 2, c, A0);
       const double e11 = dot3(e1, e1), e12 = dot3(e1, e2), e22 = dot3(e2, e2);
       const double C11 = a * a * e11, C12 = a * (b * e11 + c * e12), C22 = b * b * e11 + 2 * b * c * e12 + c * c * e22;
       const double I1 = C11 + C22 - 2.0, I2 = C11 * C22 - C12 * C12 - 1.0;
@@ -357,7 +371,8 @@ objective_smem_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_i
         for (int k = 0; k < 3; ++k) e[k] = sp[k * n + vs[(s + 1) % 3]] - sp[k * n + vs[s]];
         cross3(N, NB, cr);
         const double sin_t = dot3(cr, e) * rsqrt(dot3(e, e)), cos_t = dot3(N, NB);
-        const double c0 = p.hinge_rest[6 * t + 2 * s], s0 = p.hinge_rest[6 * t + 2 * s + 1];
+        double c0, s0;
+        load_pair(p.hinge_rest + 6 * t + 2 * s, c0, s0);
         acc += 0.5 * double(p.k_b) * (1.0 - (cos_t * c0 + sin_t * s0));
       }
     }
