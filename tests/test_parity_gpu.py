@@ -317,6 +317,44 @@ def test_line_search_fp32_fast_kernels_match_the_generic_full_gradient():
         assert rel_l2(xs[t], ref[t][0]) <= 1e-4
 
 
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_line_search_with_collisions_is_neutral_when_full_steps_descend(precision):
+    """Line search + PIK collision term (energy in the objective, gradient added after the local step; in fp32 the
+    3xTF32 split then happens just before the GEMMs): on a tame case every full step descends, so the result is the
+    oracle's plain run with collisions."""
+    import torch
+    from oracle import npfem_oracle as orc
+    from paper_1911_03062_b200 import Solver
+    pop = make_config(3, n_cells=12)
+    rng = np.random.default_rng(5)
+    targets, stiff = [], []
+    for t in range(len(pop.types)):
+        shape = pop.positions[t].shape[:2]
+        stiff.append(np.where(rng.random(shape) < 0.15, rng.uniform(20, 300, shape), 0.0))
+        targets.append(pop.positions[t] + 0.02 * rng.standard_normal(pop.positions[t].shape))
+    solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision=precision)
+    solver.set_line_search(4)
+    solver.set_state(torch.from_numpy(pop.packed(pop.positions)).cuda())
+    solver.set_collisions(pop.packed(targets).astype(np.float64),
+                          pop.packed([k[..., None].repeat(3, -1) for k in stiff])[::3].copy().astype(np.float64))
+    np_io = np.float64 if precision == "fp64" else np.float32
+    for s in range(2):
+        solver.set_forces(torch.from_numpy(pop.packed(pop.forces(s), dtype=np_io)).cuda())
+        solver.step(5)
+    x, _ = solver.get_state()
+    assert np.all(solver.get_step_lengths() == 1.0)
+    solver.close()
+    xs = pop.unpack(x.cpu().numpy())
+    for t, ct in enumerate(pop.types):
+        td = orc.make_type(ct, pop.dt)
+        xr, _ = orc.run(pop.positions[t], pop.velocities[t], lambda s, t=t: pop.forces(s)[t], td, 2, 5,
+                        collisions=(targets[t], stiff[t]))
+        x0 = pop.positions[t]
+        print(precision, ct.name, rel_l2(xs[t], xr), rel_l2(xs[t] - x0, xr - x0))
+        assert rel_l2(xs[t], xr) <= TOL_POS[precision]
+        assert rel_l2(xs[t] - x0, xr - x0) <= TOL_DISP[precision]
+
+
 def test_line_search_is_neutral_on_a_tame_case_and_freezes_by_tolerance():
     import torch
     from paper_1911_03062_b200 import Solver
