@@ -534,3 +534,31 @@ def test_step_with_collisions_pulls_flagged_vertices_to_their_targets(rbc162):
     # k = 0 everywhere is exactly the plain step
     xc, _ = orc.step(x, 0 * x, f, td, 10, collisions=(targets, 0 * k))
     assert np.array_equal(xc, xa)
+
+
+def test_reduced_gradient_form_of_the_iteration(rbc162):
+    """The identity the fast GPU kernels are built on, checked on the ORACLE's matrices:
+    with H~ = M~/h^2 + L, M~ = (1 + h alpha) M + h beta L and gamma = (beta/h) / (1 + beta/h),
+        M~/h^2 = (1 - gamma) m^ + gamma H~,      m^ = (1 + h alpha) M / h^2,
+    so grad g = r + gamma H~ d with the reduced gradient r = (1 - gamma) m^ d - b + grad E, and Eq. (4)
+    d <- d - H~^-1 grad g is exactly d <- (1 - gamma) d - H~^-1 r.  The line search's damping kernel adds
+    gamma m^ d + (beta/h) L d to r, which is the same full gradient."""
+    ct, td = rbc162
+    assert td.beta > 0.0
+    rng = np.random.default_rng(3)
+    n = td.mass.shape[0]
+    d = 0.01 * rng.standard_normal((n, 3))
+    b = rng.standard_normal((n, 3))
+    x_n = ct.rest_positions + 0.02 * rng.standard_normal((n, 3))
+    gamma = (td.beta / td.h) / (1.0 + td.beta / td.h)
+    m_hat = (1.0 + td.h * td.alpha) * td.mass[:, None] / td.h ** 2
+    assert np.allclose(td.M_tilde / td.h ** 2, (1.0 - gamma) * np.diag(m_hat[:, 0]) + gamma * td.H_tilde,
+                       rtol=1e-12, atol=1e-12 * np.abs(td.H_tilde).max())
+    full = orc.gradient_g(d, x_n, b, td)
+    r = (1.0 - gamma) * m_hat * d - b + orc.grad_energy(x_n + d, td)
+    scale = np.abs(full).max()
+    assert np.abs(r + gamma * (td.H_tilde @ d) - full).max() <= 1e-12 * scale
+    assert np.abs(r + gamma * m_hat * d + (td.beta / td.h) * (td.L @ d) - full).max() <= 1e-12 * scale
+    plain = d - orc.solve_H_tilde(full, td)
+    reduced = (1.0 - gamma) * d - orc.solve_H_tilde(r, td)
+    assert np.abs(plain - reduced).max() <= 1e-10 * np.abs(plain).max()
