@@ -192,8 +192,11 @@ int npfem_get_objective(npfem_ctx *ctx, double *history, int32_t max_entries,
  * PAPER.md:37, :264).  max_halvings = 0 switches it off (default: plain Eq. (4), step length 1).
  * Per cell and iteration: frozen if ||grad g||_2 <= grad_tol ||b||_2; otherwise alpha = 1 and alpha is
  * halved while g(d + alpha p) > g(d) + armijo_c1 alpha <grad g, p>, at most max_halvings (<= 30) times,
- * p = -H~^-1 grad g; d <- d + alpha p.  With it on, the local step runs the generic kernel (full
- * gradient) and every iteration costs max_halvings + 2 extra objective evaluations.
+ * p = -H~^-1 grad g; d <- d + alpha p.  With it on, every iteration evaluates the objective (fp64) at the
+ * trial point of every cell not yet accepted, up to max_halvings + 1 times; fp32 contexts take p from a
+ * 3xTF32 product on the tensor cores (fp32-grade: a plain TF32 direction makes the search stall) and hold
+ * one more field-sized buffer per bucket plus one n_pad^2 matrix per type for it (NPFEM_ENOMEM if they
+ * cannot be allocated at the next npfem_step).
  */
 int npfem_set_line_search(npfem_ctx *ctx, int32_t max_halvings, double armijo_c1, double grad_tol);
 
