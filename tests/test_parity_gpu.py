@@ -222,11 +222,11 @@ def test_irregular_mesh_valence_up_to_8(precision, impl):
         assert r["pos"] <= TOL_POS[precision] and r["disp"] <= TOL_DISP[precision] and r["vel"] <= TOL_DISP[precision], r
 
 
-def _ls_population(n_cells, h, force_sigma, seed):
+def _ls_population(n_cells, h, force_sigma, seed, level=2):
     """RBC-162 cells at rest shape under N(0, force_sigma) forces: with h = 30 us and 3000 pN the plain
     iteration of Eq. (4) diverges (tests/test_oracle_pins.py), the line search must not."""
     from workloads.meshes import rbc_cell_type
-    ct = rbc_cell_type(2)
+    ct = rbc_cell_type(level)
     rng = np.random.default_rng(seed)
     pos = ct.rest_positions[None] + rng.uniform(0, 60, (n_cells, 1, 3))
     return Population(name="ls", types=[ct], type_of_cell=np.zeros(n_cells, np.int32), positions=[pos],
@@ -273,6 +273,35 @@ def test_line_search_violent_case_matches_oracle(precision):
         # oracle's step lengths (1.6e-4)
         assert np.median(alpha) > 0.5 ** 8
         assert rel_l2(xg - x0, xr - x0) <= 1e-3
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_line_search_large_time_step_rbc642(precision):
+    """SURVEY.md 8(f)-1's own case on the BASELINE mesh: h = 10 us (100 x the BASELINE step), N(0, 100 pN) forces,
+    RBC-642 (fp32: scheduled local step + damping kernel + 3xTF32 product in three column passes)."""
+    import torch
+    from oracle import npfem_oracle as orc
+    from paper_1911_03062_b200 import Solver
+    pop = _ls_population(5, 10.0, 100.0, seed=8, level=3)
+    td = orc.make_type(pop.types[0], pop.dt)
+    xr, vr, hist = orc.step_line_search(pop.positions[0], pop.velocities[0], pop.forces(0)[0], td, 8, max_halvings=6, c1=1e-4,
+                                        record=True)
+    assert np.all(np.diff(np.array(hist["objective"]), axis=0) <= 0.0)   # the oracle's objective decreases
+    solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision=precision)
+    solver.set_line_search(6, 1e-4, 0.0)
+    solver.set_state(torch.from_numpy(pop.packed(pop.positions)).cuda())
+    solver.set_forces(torch.from_numpy(pop.packed(pop.forces(0))).cuda())
+    solver.step(8)
+    x, v = solver.get_state()
+    alpha = solver.get_step_lengths()
+    solver.close()
+    xg = pop.unpack(x.cpu().numpy())[0]
+    x0 = pop.positions[0]
+    print(precision, "disp", rel_l2(xg - x0, xr - x0), "alpha gpu", alpha, "oracle", hist["alpha"][-1])
+    assert np.all(np.isfinite(xg))
+    assert rel_l2(xg - x0, xr - x0) <= TOL_DISP[precision]
+    if precision == "fp64":
+        assert np.array_equal(alpha, hist["alpha"][-1])
 
 
 def test_line_search_fp32_fast_kernels_match_the_generic_full_gradient():
