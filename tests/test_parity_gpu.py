@@ -304,6 +304,32 @@ def test_line_search_large_time_step_rbc642(precision):
         assert np.array_equal(alpha, hist["alpha"][-1])
 
 
+def test_line_search_violent_case_rbc642_fp32():
+    """The violent case on the BASELINE mesh (RBC-642: scheduled local step, 3xTF32 product in three column passes):
+    the search backtracks, does not stall, and the result stays within the fp32 displacement bound of the oracle."""
+    import torch
+    from oracle import npfem_oracle as orc
+    from paper_1911_03062_b200 import Solver
+    pop = _ls_population(4, 30.0, 3000.0, seed=33, level=3)
+    td = orc.make_type(pop.types[0], pop.dt)
+    xr, vr, hist = orc.step_line_search(pop.positions[0], pop.velocities[0], pop.forces(0)[0], td, 12, max_halvings=8, c1=1e-4,
+                                        record=True)
+    assert np.array(hist["alpha"]).min() < 1.0                       # the case does backtrack
+    solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision="fp32")
+    solver.set_line_search(8, 1e-4, 0.0)
+    solver.set_state(torch.from_numpy(pop.packed(pop.positions)).cuda())
+    solver.set_forces(torch.from_numpy(pop.packed(pop.forces(0))).cuda())
+    solver.step(12)
+    x, _ = solver.get_state()
+    alpha = solver.get_step_lengths()
+    solver.close()
+    xg = pop.unpack(x.cpu().numpy())[0]
+    x0 = pop.positions[0]
+    print("disp", rel_l2(xg - x0, xr - x0), "alpha gpu", alpha, "oracle", hist["alpha"][-1])
+    assert np.median(alpha) > 0.5 ** 8
+    assert rel_l2(xg - x0, xr - x0) <= TOL_DISP["fp32"]
+
+
 def test_line_search_fp32_fast_kernels_match_the_generic_full_gradient():
     """fp32 line search: the fast local kernels' reduced gradient + the damping part (launch_damping_grad)
     against the generic kernel's full gradient (OPT_LOCAL_STEP_IMPL = 1) and against the oracle, on the
