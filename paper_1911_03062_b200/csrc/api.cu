@@ -809,14 +809,12 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
         NPFEM_CUDA(c, cudaMemcpyAsync(c->views[t].field[F_U], c->views[t].field[F_D], bytes, cudaMemcpyDeviceToDevice, c->stream));
       }
       if ((rc = timed_launch(c, NPFEM_KIND_GLOBAL, int(t), "global step", [&] {
-             if (ls_on && c->ls[t].g_lo) {     // 3xTF32: d <- d - (g_hi W_hi + g_lo W_hi + g_hi W_lo)
+             if (ls_on && c->ls[t].g_lo) {     // 3xTF32: d <- d - (g_hi W_hi + g_lo W_hi + g_hi W_lo), one K-concatenated GEMM
                const LineSearchDev &l = c->ls[t];
                const size_t count = size_t(c->buckets[t].cells) * 3 * c->types[t].n_pad;
                int nl = split_early ? 0 : launch_ls_split_g(static_cast<float *>(c->views[t].field[F_G]), l.g_lo, count, c->stream);
-               const int n1 = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, 1.0, nullptr, c->stream);
-               const int n2 = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, 1.0, nullptr, c->stream, l.g_lo, nullptr);
-               const int n3 = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, 1.0, nullptr, c->stream, nullptr, l.w_lo);
-               return n1 < 0 || n2 < 0 || n3 < 0 ? -1 : nl + n1 + n2 + n3;
+               const int n1 = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, 1.0, nullptr, c->stream, l.g_lo, l.w_lo);
+               return n1 < 0 ? -1 : nl + n1;
              }
              if (c->precision == NPFEM_F32 && c->opt_global_math == 0) {
                const int n = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, d_scale,

@@ -133,6 +133,7 @@ struct GemmParams {
   int n_pass;          // accumulator columns per pass = N of the MMA (multiple of 16, <= MAX_NPASS)
   int passes;          // ceil(n_pad / n_pass)
   int k_chunks;        // ceil(n_pad / BK)
+  int k_segs;          // 1, or 3: K-concatenated 3xTF32 product [g_hi g_lo g_hi] . [W_hi; W_hi; W_lo] (line search)
   int64_t m_tiles;
   float d_scale;       // d <- d_scale * d + acc
   int stages;          // depth of the operand ring (<= MAX_STAGES)
@@ -149,7 +150,8 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
 
 __global__ void __launch_bounds__(192, 1)
 global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_constant__ CUtensorMap map_w,
-                      const __grid_constant__ CUtensorMap map_d, const GemmParams p) {
+                      const __grid_constant__ CUtensorMap map_d, const __grid_constant__ CUtensorMap map_g2,
+                      const __grid_constant__ CUtensorMap map_w2, const GemmParams p) {
   extern __shared__ unsigned char smem_raw[];
   __shared__ uint64_t full_bar[MAX_STAGES], empty_bar[MAX_STAGES], tmem_full_bar[2], tmem_empty_bar[2], epi_full[4 * EBUF];
   __shared__ uint32_t tmem_base_sh;
@@ -194,14 +196,17 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
       const int w_rows = p.n_pass / CL;                     // this CTA's slice of the W tile (multiple of 8 rows)
       for (int64_t item = first_item; item < n_items; item += item_step) {
         const int row0 = int(((item / p.passes) * CL + rank) * BM), col0 = int(item % p.passes) * p.n_pass;
-        for (int kc = 0; kc < p.k_chunks; ++kc) {
-          mbar_wait(&empty_bar[stage], phase ^ 1);          // this slot is free in EVERY CTA of the cluster
-          unsigned char *sa = smem + stage * p.stage_bytes, *sb = sa + A_BYTES;
-          mbar_expect_tx(&full_bar[stage], tx);             // own G tile + all CL slices of the W tile
-          tma_load_2d(sa, &map_g, kc * BK, row0, &full_bar[stage]);
-          tma_load_2d_mc(sb + size_t(rank) * w_rows * BK * 4, &map_w, kc * BK, col0 + int(rank) * w_rows,
-                         &full_bar[stage], MASK);
-          if (++stage == p.stages) { stage = 0; phase ^= 1; }
+        for (int seg = 0; seg < p.k_segs; ++seg) {          // segment 1 reads g_lo, segment 2 reads W_lo
+          const CUtensorMap *mg = seg == 1 ? &map_g2 : &map_g, *mw = seg == 2 ? &map_w2 : &map_w;
+          for (int kc = 0; kc < p.k_chunks; ++kc) {
+            mbar_wait(&empty_bar[stage], phase ^ 1);        // this slot is free in EVERY CTA of the cluster
+            unsigned char *sa = smem + stage * p.stage_bytes, *sb = sa + A_BYTES;
+            mbar_expect_tx(&full_bar[stage], tx);           // own G tile + all CL slices of the W tile
+            tma_load_2d(sa, mg, kc * BK, row0, &full_bar[stage]);
+            tma_load_2d_mc(sb + size_t(rank) * w_rows * BK * 4, mw, kc * BK, col0 + int(rank) * w_rows,
+                           &full_bar[stage], MASK);
+            if (++stage == p.stages) { stage = 0; phase ^= 1; }
+          }
         }
       }
     }
@@ -216,7 +221,7 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
         mbar_wait(&tmem_empty_bar[acc], acc_phase ^ 1);     // epilogue has drained this accumulator
         asm volatile("tcgen05.fence::after_thread_sync;");
         const uint32_t tacc = tmem_base + acc * MAX_NPASS;
-        for (int kc = 0; kc < p.k_chunks; ++kc) {
+        for (int kc = 0; kc < p.k_chunks * p.k_segs; ++kc) {
           mbar_wait(&full_bar[stage], phase);
           asm volatile("tcgen05.fence::after_thread_sync;");
           const uint32_t sa = smem_u32(smem + stage * p.stage_bytes), sb = sa + A_BYTES;
@@ -359,9 +364,10 @@ bool global_tcgen05_supported(const TypeDev &td) {
 
 // d <- d_scale d - g Hinv (u_out == nullptr) or u_out <- -g Hinv.  Returns #launches, or -1 if the
 // configuration is unsupported (caller falls back to the SIMT GEMM).
-// g_op / w_op: other operands than bv.field[F_G] / the type's TF32 H~^-1 (the line search's 3xTF32 product).
+// g_lo / w_lo (both or neither): the line search's 3xTF32 product d <- d_scale d - (g W + g_lo W + g W_lo) as ONE
+// GEMM with the three products concatenated along K (g = bv.field[F_G] holds the TF32 high part, W = Hinv_tf32).
 int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, double d_scale, void *u_out,
-                          cudaStream_t s, const void *g_op, const void *w_op) {
+                          cudaStream_t s, const void *g_lo, const void *w_lo) {
   if (bv.cells == 0) return 0;
   GemmParams p{};
   if (!gemm_shape(td, p)) return -1;
@@ -371,9 +377,16 @@ int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, dou
   p.m_tiles = (p.rows + BM - 1) / BM;
   p.d_scale = float(d_scale);
   CUtensorMap map_g, map_w, map_d;
-  if (!make_map(&map_g, g_op ? g_op : bv.field[F_G], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), BM)) return -1;
-  if (!make_map(&map_w, w_op ? w_op : td.Hinv_tf32 ? td.Hinv_tf32 : td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n_pass / CL)))
+  if (!make_map(&map_g, bv.field[F_G], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), BM)) return -1;
+  if (!make_map(&map_w, td.Hinv_tf32 ? td.Hinv_tf32 : td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n_pass / CL)))
     return -1;
+  CUtensorMap map_g2 = map_g, map_w2 = map_w;
+  p.k_segs = 1;
+  if (g_lo && w_lo) {
+    if (!make_map(&map_g2, g_lo, uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), BM)) return -1;
+    if (!make_map(&map_w2, w_lo, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n_pass / CL))) return -1;
+    p.k_segs = 3;
+  }
   // epilogue tiles: [32 rows][32 columns] of D (in-place update) or of U (product out)
   if (!make_map(&map_d, u_out ? u_out : bv.field[F_D], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), 32))
     return -1;
@@ -404,7 +417,7 @@ int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, dou
   attrs[0].val.clusterDim.z = 1;
   cfg.attrs = attrs;
   cfg.numAttrs = 1;
-  if (cudaLaunchKernelEx(&cfg, global_tcgen05_kernel, map_g, map_w, map_d, p) != cudaSuccess) return -1;
+  if (cudaLaunchKernelEx(&cfg, global_tcgen05_kernel, map_g, map_w, map_d, map_g2, map_w2, p) != cudaSuccess) return -1;
   return 1;
 }
 

@@ -166,7 +166,7 @@ int launch_global_simt(const TypeDev &td, const BucketView &bv, int precision, d
 bool global_tcgen05_supported(const TypeDev &td);
 // u_out == nullptr: d <- d_scale d - g Hinv;  else u_out <- -g Hinv (the next local step / the epilogue applies it)
 int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, double d_scale, void *u_out,
-                          cudaStream_t s, const void *g_op = nullptr, const void *w_op = nullptr);
+                          cudaStream_t s, const void *g_lo = nullptr, const void *w_lo = nullptr);
 
 // fp32 fast local step; writes the reduced gradient (global step must then use d_scale = 1 - gamma)
 bool local_smem_supported(const TypeDev &td);
