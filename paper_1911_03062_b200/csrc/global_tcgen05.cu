@@ -18,6 +18,8 @@
 //                           d_scale d + acc in place (row per lane, conflict-free) -> TMA store
 // Work item of a cluster = (CL consecutive M tiles, N pass); the passes of one group are adjacent items
 // (neighbouring clusters at about the same time), so the repeated G reads are L2 hits.
+// Line-search mode (k_segs = 3): the 3xTF32 product [g_hi g_lo g_hi] . [W_hi; W_hi; W_lo] as one GEMM with K = 3 n_pad;
+// the producer switches tensor maps per K segment, nothing else changes.
 #include <cuda.h>
 
 #include "internal.h"
