@@ -422,7 +422,9 @@ def step_line_search(x_n: np.ndarray, v_n: np.ndarray, f_ext: np.ndarray, td: Ty
     frozen (d unchanged).  Otherwise p = -H~^-1 grad, slope = <grad, p> (< 0 because H~ is SPD),
     alpha = 1, and alpha is halved while  g(d + alpha p) > g(d) + c1 alpha slope,  at most
     `max_halvings` times (the last alpha is taken even if the test still fails).  d <- d + alpha p.
-    Returns (x_next, v_next[, history]); history["alpha"] is [n_iterations] arrays of step lengths.
+    Returns (x_next, v_next[, history]); history["alpha"] is [n_iterations] arrays of step lengths;
+    history also keeps, per iteration, the slope, the iterate d and the direction p the search started from
+    (and b once), so that a test can re-evaluate the Armijo inequality itself.
     """
     h = td.h
     v = pbd_damping(x_n, v_n, td.mass, td.kappa)
@@ -430,7 +432,7 @@ def step_line_search(x_n: np.ndarray, v_n: np.ndarray, f_ext: np.ndarray, td: Ty
     d = h * v
     lead = d.shape[:-2]
     b_norm = np.sqrt(np.sum(b * b, axis=(-2, -1)))
-    history = {"objective": [], "alpha": [], "grad_norm": []}
+    history = {"objective": [], "alpha": [], "grad_norm": [], "slope": [], "d": [], "p": [], "b": b}
     for _ in range(n_iterations):
         grad = gradient_g(d, x_n, b, td)
         g_norm = np.sqrt(np.sum(grad * grad, axis=(-2, -1)))
@@ -448,6 +450,10 @@ def step_line_search(x_n: np.ndarray, v_n: np.ndarray, f_ext: np.ndarray, td: Ty
                 break
             alpha = np.where(done, alpha, 0.5 * alpha)
         alpha = np.where(frozen, 0.0, alpha)
+        if record:
+            history["slope"].append(slope)
+            history["d"].append(d)
+            history["p"].append(p)
         d = d + alpha[..., None, None] * p
         if record:
             history["objective"].append(g0)

@@ -191,6 +191,52 @@ def test_p7_converged_step_satisfies_newton_second_law(ico):
     assert np.abs(orc.eq2_residual(ha["v_damped"], xa, va, F, td)).max() > 1e-4
 
 
+def _rayleigh_type(ct, alpha, beta, kappa=0.0):
+    import dataclasses
+    mat = dataclasses.replace(ct.material, rayleigh_alpha=alpha, rayleigh_beta=beta, kappa_damping=kappa)
+    return dataclasses.replace(ct, material=mat)
+
+
+def test_p6_p7_rayleigh_alpha_nonzero_system_matrices(rbc162, ico, monkeypatch):
+    """The alpha_D != 0 branch of `system_matrices` (PAPER.md:234 lists alpha_D = 0, but PAPER.md:264 defines
+    C = alpha_D M + beta_D K as part of the model): M~ = M + h C = (1 + h alpha) M + h beta L, written out HERE from
+    M, L_cot, alpha, beta, h - not taken from the oracle's M~.  A dropped or mis-scaled alpha term (e.g. M~ = M +
+    h beta L, or alpha M without the factor h) fails both parts."""
+    alpha, beta = 0.3, 0.01                                    # 1/us, us
+    # ---- P6 with alpha: one iteration on a purely quadratic energy equals the dense solve ----------
+    ct, _ = rbc162
+    td = orc.make_type(_rayleigh_type(ct, alpha, beta), H)
+    M = np.diag(td.rho * td.volume0 * td.area_vertex / td.area_total)
+    L = (td.B + 2 * td.C) * td.L_cot + td.k_b * td.L_cot.T @ np.diag(1.0 / td.area_vertex) @ td.L_cot
+    C_damp = alpha * M + beta * L                              # PAPER.md:264
+    M_tilde = M + H * C_damp                                   # PAPER.md:268
+    assert np.allclose(td.M_tilde, M_tilde, rtol=1e-13, atol=0)
+    assert not np.allclose(td.M_tilde, M + H * beta * L, rtol=1e-3)          # the alpha term is not negligible here
+    monkeypatch.setattr(orc, "grad_energy", lambda x, t: np.einsum("ij,...jc->...ic", t.L, x))
+    rng = np.random.default_rng(19)
+    x = ct.rest_positions + 0.02 * rng.standard_normal(ct.rest_positions.shape)
+    v = 0.1 * rng.standard_normal(x.shape)
+    F = rng.standard_normal(x.shape)
+    x1, _ = orc.step(x, v, F, td, 1)
+    x_ref = np.linalg.solve(M_tilde / H ** 2 + L, M_tilde @ x / H ** 2 + M @ v / H + F)
+    assert np.allclose(x1, x_ref, rtol=1e-11, atol=1e-12)
+    monkeypatch.undo()
+    # ---- P7 with alpha: the converged step satisfies Eq. (2) with C = alpha M + beta L spelled out ----
+    ct, _ = ico
+    td = orc.make_type(_rayleigh_type(ct, alpha, beta), H)
+    M = np.diag(td.mass)
+    L = (td.B + 2 * td.C) * td.L_cot + td.k_b * td.L_cot.T @ np.diag(1.0 / td.area_vertex) @ td.L_cot
+    C_damp = alpha * M + beta * L
+    x = ct.rest_positions + 0.05 * rng.standard_normal((12, 3))
+    v = 0.05 * rng.standard_normal((12, 3))
+    F = 5.0 * rng.standard_normal((12, 3))
+    x1, v1, hist = orc.step(x, v, F, td, 400, record=True)
+    res = M @ (v1 - hist["v_damped"]) / H - (-orc.grad_energy(x1, td) + F - C_damp @ v1)      # Eq. (2), PAPER.md:261-264
+    assert np.abs(res).max() < 1e-9 * np.abs(F).max()
+    res_no_alpha = M @ (v1 - hist["v_damped"]) / H - (-orc.grad_energy(x1, td) + F - beta * L @ v1)
+    assert np.abs(res_no_alpha).max() > 1e-4 * np.abs(F).max()                # dropping alpha M v is visible
+
+
 # ---- P8 ------------------------------------------------------------------------------
 def test_p8_icosahedron_brute_force_minimiser(ico):
     ct, td = ico
@@ -430,8 +476,31 @@ def test_ls_keeps_the_objective_monotone_where_the_plain_iteration_blows_up():
     alpha = np.array(hist["alpha"])
     assert alpha.min() < 1.0                                          # the search really backtracked
     assert np.all(np.isin(alpha, 0.5 ** np.arange(0, 9)))             # powers of 1/2 only
-    # Armijo at every accepted step that did not exhaust the halvings: g_new <= g_old + c1 alpha slope, slope < 0
     assert np.all(obj[1:][alpha > 0.5 ** 8] < obj[:-1][alpha > 0.5 ** 8])
+    # The Armijo inequality itself, re-evaluated here from the recorded iterate d, direction p and slope (a search
+    # that ignored c1 alpha slope, or took the slope with the wrong sign, passes plain monotonicity but not this):
+    # at every accepted step that did not exhaust the halvings  g(d + alpha p) <= g(d) + c1 alpha slope with
+    # slope < 0, and the step length tried just before, 2 alpha, VIOLATED it (alpha is the first that passes).
+    c1 = 1e-4
+    slope = np.array(hist["slope"])
+    assert np.all(slope < 0.0)                                        # H~ is SPD: p is a descent direction
+    n_checked = n_rejected = 0
+    for k in range(15):
+        d, p, b = hist["d"][k], hist["p"][k], hist["b"]
+        g0 = orc.objective(d, x, b, td)
+        assert np.array_equal(g0, obj[k])
+        for cell in range(x.shape[0]):
+            a = alpha[k, cell]
+            if a <= 0.5 ** 8:
+                continue                                              # exhausted: taken without passing the test
+            at = lambda s: orc.objective((d + s * p)[cell], x[cell], b[cell], td)   # noqa: E731
+            assert at(a) <= g0[cell] + c1 * a * slope[k, cell]
+            assert at(a) == obj[k + 1, cell]                          # the accepted point is the next iterate
+            n_checked += 1
+            if a < 1.0:
+                assert at(2 * a) > g0[cell] + c1 * 2 * a * slope[k, cell]
+                n_rejected += 1
+    assert n_checked > 10 and n_rejected > 3                          # not vacuous
 
 
 def test_ls_gradient_tolerance_freezes_converged_cells(rbc162):
@@ -485,6 +554,31 @@ def test_median_filter_removes_a_spike_and_keeps_a_constant(ico):
             for k in range(3):
                 vals = sorted([g[c, v, k]] + [g[c, u, k] for u in ring[v]])
                 assert out[c, v, k] == 0.5 * (vals[2] + vals[3])
+
+
+def test_median_filter_odd_count_brute_force(rbc162):
+    """Valence-6 vertices: 7 values per median (the vertex + 6 neighbours), the ODD-count branch of reading R18 -
+    the icosahedron above only has even counts.  Brute force against the definition: the 4th of the 7 sorted values;
+    the 12 valence-5 vertices of the icosphere (6 values) average the two central ones."""
+    ct, td = rbc162
+    ring = orc.one_ring(td.tri, td.n)
+    counts = np.array([len(r) for r in ring])
+    assert set(counts) == {5, 6} and np.sum(counts == 5) == 12
+    rng = np.random.default_rng(2)
+    g = rng.standard_normal((2, td.n, 3))
+    out = orc.median_filter_forces(g, td)
+    for c in range(2):
+        for v in range(td.n):
+            for k in range(3):
+                vals = sorted([g[c, v, k]] + [g[c, u, k] for u in ring[v]])
+                expect = vals[3] if len(vals) == 7 else 0.5 * (vals[2] + vals[3])
+                assert out[c, v, k] == expect
+    # a spike is removed at an odd count too, and lands in no neighbour's median
+    f = np.tile(np.array([1.0, -2.0, 3.0]), (td.n, 1))
+    spike = f.copy()
+    v6 = int(np.nonzero(counts == 6)[0][0])
+    spike[v6] = 1e6
+    assert np.array_equal(orc.median_filter_forces(spike, td), f)
 
 
 def test_step_with_cap_only_changes_the_velocity(rbc162):
