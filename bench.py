@@ -39,35 +39,155 @@ def parse_args():
     ap.add_argument("--cells", type=int, default=None, help="shrink the config to this many cells")
     ap.add_argument("--iterations", type=int, default=None, help="solver iterations per step")
     ap.add_argument("--precision", default="fp32", choices=["fp32", "fp64"])
-    ap.add_argument("--global-math", default="tf32", choices=["tf32", "fp32"])
-    ap.add_argument("--update-mode", type=int, default=0, choices=[0, 1, 2],
-                    help="0 auto, 1 GEMM epilogue updates d in place, 2 product-out applied by the next local step")
+    ap.add_argument("--global-math", default="tf32", choices=["tf32", "fp32", "tf32x2"])
     ap.add_argument("--local-impl", type=int, default=0, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--line-search", type=int, default=0, help="Armijo backtracking with this many halvings (0 = off)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-chunks", type=int, default=0, help="npfem_step_host chunks (0 = library's choice, 1 = unpipelined)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--peaks", action="store_true",
+                    help="measure the FP32 FFMA, FP64 DFMA, TF32 / FP64 / BF16 GEMM and copy peaks of this box and print them "
+                         "as one JSON line (kept as profiles/r2_measured_peaks.json: the roofline denominators)")
     return ap.parse_args()
 
 
-def load_ncu_capture():
-    """Per-launch DRAM bytes and warp instructions of the two hot kernels from the committed ncu
-    `--set full` capture (profiles/r1_ncu_capture.json, written by hand from the .ncu-rep: bench.py
-    cannot run ncu).  Only valid for the workload it was captured on."""
-    path = os.path.join(ROOT, "profiles", "r1_ncu_capture.json")
-    return json.load(open(path)) if os.path.exists(path) else {}
+NCU_RAW = {   # kernel of the bench line -> committed raw export of ONE launch of it on the bench workload
+    "local:RBC-642": "r2_ncu_local_sched_rbc642_raw.csv",
+    "global:RBC-642": "r2_ncu_global_tcgen05_rbc642_raw.csv",
+}
+NCU_WORKLOAD = {"cells": 100000, "precision": "fp32"}   # what the exports were captured on (profiles/r2_ncu.md)
+
+
+def load_ncu_raw(kernel: str):
+    """Per-launch counters of a hot kernel, parsed from the committed `ncu -i <rep> --page raw --csv --print-units base`
+    export of one launch (profiles/r2_ncu.md names the full commands): bench.py cannot run ncu, but every number it
+    quotes from a capture is re-derivable from a tracked file.  Only valid for the workload of the capture."""
+    import csv
+    name = NCU_RAW.get(kernel)
+    path = os.path.join(ROOT, "profiles", name) if name else None
+    if not path or not os.path.exists(path):
+        return None
+    rows = list(csv.reader(open(path)))
+    hdr, vals = rows[0], rows[2]
+
+    def col(metric):
+        for i, h in enumerate(hdr):
+            if h == metric:
+                return float(vals[i]) if vals[i] not in ("", "no data") else None
+        return None
+    fadd, fmul, ffma = (col(f"smsp__sass_thread_inst_executed_op_{op}_pred_on.sum") for op in ("fadd", "fmul", "ffma"))
+    out = {"file": "profiles/" + name,
+           "dram_bytes": (col("dram__bytes_read.sum") or 0) + (col("dram__bytes_write.sum") or 0),
+           "warp_instructions": col("smsp__inst_executed.sum"),
+           "smem_wavefronts": col("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum"),
+           "duration_ns_under_ncu": col("gpu__time_duration.sum"),
+           "tensor_pipe_active_pct": col("sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_elapsed")}
+    if None not in (fadd, fmul, ffma):
+        out["fp32_flop"] = fadd + fmul + 2 * ffma
+    return out
 
 
 def load_peaks():
-    """Measured roofline denominators (driver-written), else the profiling guide's fallback."""
+    """Measured roofline denominators: HBM and bf16 from the driver-written MEASURED_PEAKS.json (else the profiling
+    guide's fallback); TF32 / FP64 GEMM and FP32 FFMA from profiles/r2_measured_peaks.json (`bench.py --peaks` on a
+    B200 of this pool), else the nominal ratios, saying which."""
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
         p = json.load(open(path))
-        return {"hbm_gbs": float(p["hbm_gbs"]), "bf16_tflops": float(p["bf16_tflops"]),
-                "bf16_tflops_sustained": float(p.get("bf16_tflops_sustained", p["bf16_tflops"])),
-                "sm_max_mhz": float(p.get("sm_max_mhz", 1965.0)), "source": "measured"}
-    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+        out = {"hbm_gbs": float(p["hbm_gbs"]), "bf16_tflops": float(p["bf16_tflops"]),
+               "bf16_tflops_sustained": float(p.get("bf16_tflops_sustained", p["bf16_tflops"])),
+               "sm_max_mhz": float(p.get("sm_max_mhz", 1965.0)), "source": "measured"}
+    else:
+        out = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0,
+               "source": "fallback"}
+    own = os.path.join(ROOT, "profiles", "r2_measured_peaks.json")
+    if os.path.exists(own):
+        q = json.load(open(own))
+        out.update({"tf32_tflops": q["tf32_gemm_tflops"], "tf32_tflops_sustained": q["tf32_gemm_tflops_sustained"],
+                    "fp64_tflops": q["fp64_gemm_tflops"], "fp32_ffma_tflops": q["fp32_ffma_tflops"],
+                    "fp64_dfma_tflops": q["fp64_dfma_tflops"],
+                    "own_source": "measured (profiles/r2_measured_peaks.json, bench.py --peaks)"})
+    else:
+        out.update({"tf32_tflops": 0.5 * out["bf16_tflops"], "tf32_tflops_sustained": 0.5 * out["bf16_tflops_sustained"],
+                    "fp64_tflops": 40.0, "fp32_ffma_tflops": 148 * 128 * 2 * out["sm_max_mhz"] * 1e6 / 1e12,
+                    "fp64_dfma_tflops": 40.0, "own_source": "nominal ratios (no profiles/r2_measured_peaks.json)"})
+    return out
+
+
+def run_peaks():
+    """`--peaks`: the roofs this repository's kernels are measured against, taken on the box at hand the way
+    MEASURED_PEAKS.json was (torch.matmul / copy, best of 10 and a 2 s back-to-back loop), plus the plain-ALU roofs
+    from the library's own FMA probe kernel (npfem_probe_fma_peak).  Prints one JSON line."""
+    import ctypes as C
+    import torch
+    from paper_1911_03062_b200 import binding
+    lib = binding.load_library()
+    torch.cuda.set_device(0)
+    dev = "cuda:0"
+    stream = torch.cuda.current_stream(0)
+
+    def timed(fn, reps=10):
+        fn()
+        torch.cuda.synchronize()
+        best = 1e30
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1) * 1e-3)
+        return best
+
+    def sustained(fn, seconds=2.0):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0, n = time.perf_counter(), 0
+        e0.record()
+        while time.perf_counter() - t0 < seconds:
+            for _ in range(8):
+                fn()
+            n += 8
+            torch.cuda.synchronize()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e-3 / n
+
+    out = {"gpu_name": torch.cuda.get_device_name(0), "when": time.strftime("%Y-%m-%dT%H:%M:%SZ", time.gmtime()),
+           "how": "bench.py --peaks: torch.matmul N^3 (2 N^3 flop; tf32 = float32 inputs with allow_tf32, fp64, bf16; N = 8192, "
+                  "fp64 4096), best of 10 and back to back for 2 s; b.copy_(a) over 1 Gi bf16 (read + write bytes); "
+                  "npfem_probe_fma_peak (148 x 32 CTAs x 256 threads, 16 independent FMA chains per thread), best of 10"}
+    with ClockSampler(0) as clocks:
+        for prec, name, iters, dt in ((binding.NPFEM_F32, "fp32_ffma_tflops", 1 << 15, torch.float32),
+                                      (binding.NPFEM_F64, "fp64_dfma_tflops", 1 << 10, torch.float64)):
+            sink = torch.zeros(1, dtype=dt, device=dev)
+            flops = C.c_double(0.0)
+
+            def probe():
+                rc = lib.npfem_probe_fma_peak(C.c_void_p(stream.cuda_stream), prec, 148 * 32, iters, C.c_void_p(sink.data_ptr()),
+                                              C.byref(flops))
+                assert rc == 0
+            secs = timed(probe)
+            out[name] = flops.value / secs / 1e12
+        torch.backends.cuda.matmul.allow_tf32 = True
+        for name, dt, n in (("tf32_gemm_tflops", torch.float32, 8192), ("bf16_gemm_tflops", torch.bfloat16, 8192),
+                            ("fp64_gemm_tflops", torch.float64, 4096)):
+            a = torch.randn(n, n, device=dev, dtype=torch.float32).to(dt)
+            b = torch.randn(n, n, device=dev, dtype=torch.float32).to(dt)
+            c = torch.empty(n, n, device=dev, dtype=dt)
+            fn = lambda: torch.matmul(a, b, out=c)      # noqa: E731
+            out[name] = 2.0 * n ** 3 / timed(fn) / 1e12
+            out[name + "_sustained"] = 2.0 * n ** 3 / sustained(fn) / 1e12
+            del a, b, c
+        torch.backends.cuda.matmul.allow_tf32 = False
+        src = torch.empty(1 << 30, dtype=torch.bfloat16, device=dev)
+        dst = torch.empty_like(src)
+        out["hbm_copy_gbs"] = 2.0 * src.numel() * 2 / timed(lambda: dst.copy_(src)) / 1e9
+    out["clocks"] = clocks.summary()
+    print(json.dumps(out), flush=True)
+    return 0
 
 
 class ClockSampler:
@@ -157,16 +277,22 @@ def oracle_sample(pop, n_sample: int):
     return pop.subset(np.arange(min(n_sample, pop.n_cells)))
 
 
-def time_oracle(sample, n_iterations: int) -> float:
-    """Seconds for ONE time step of the oracle, as it stands, on the sample."""
+def time_oracle(sample, n_iterations: int, busy=None) -> float:
+    """Seconds for ONE time step of the oracle, as it stands, on the sample.  busy (a list) receives the process CPU
+    seconds spent in the timed region: CPU seconds / wall seconds = the cores the oracle actually kept busy."""
     from oracle import npfem_oracle as orc
     tds = [orc.make_type(ct, sample.dt) for ct in sample.types]     # setup, not timed (as on the GPU)
     forces = sample.forces(0)
+    c0 = os.times()
     t0 = time.perf_counter()
     for t, td in enumerate(tds):
         if sample.positions[t].shape[0]:
             orc.step(sample.positions[t], sample.velocities[t], forces[t], td, n_iterations)
-    return time.perf_counter() - t0
+    wall = time.perf_counter() - t0
+    c1 = os.times()
+    if busy is not None:
+        busy.append((c1.user - c0.user) + (c1.system - c0.system))
+    return wall
 
 
 def cpu_baseline(pop, n_iterations: int, target_seconds: float):
@@ -175,13 +301,20 @@ def cpu_baseline(pop, n_iterations: int, target_seconds: float):
     per_cell = max(t_probe / probe.n_cells, 1e-6)
     n_sample = int(max(probe.n_cells, min(pop.n_cells, target_seconds / per_cell, 4000)))
     sample = oracle_sample(pop, n_sample)
-    secs = time_oracle(sample, n_iterations)
+    busy = []
+    secs = time_oracle(sample, n_iterations, busy)
     counts = [int(np.sum(sample.type_of_cell == t)) for t in range(len(pop.types))]
     desc = " + ".join(f"{c} {ct.name}" for c, ct in zip(counts, pop.types) if c)
+    cores_busy = busy[0] / secs
     return {
-        "value": sample.n_cells * n_iterations / secs, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+        # cores = what the oracle actually kept busy (process CPU seconds / wall seconds, rounded up), not what the box
+        # has: it is plain numpy, whose element-wise passes and scatter-adds run on one thread; only the LAPACK /
+        # BLAS calls (Cholesky solve, M~ d) fan out
+        "value": sample.n_cells * n_iterations / secs, "unit": UNIT, "cores": int(max(1, np.ceil(cores_busy - 0.05))),
+        "cores_busy_mean": round(cores_busy, 2), "threads_available": len(os.sched_getaffinity(0)),
+        "blas_threads": blas_threads(), "kind": "oracle",
         "sample": f"first {sample.n_cells} cells of the workload ({desc}), 1 step x {n_iterations} iterations, "
-                  f"{secs:.1f} s; numpy element loops are single-threaded, LAPACK solves use `cores` threads",
+                  f"{secs:.1f} s wall, {busy[0]:.1f} CPU s",
     }, sample
 
 
@@ -234,8 +367,7 @@ def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: 
     peaks = load_peaks()
 
     solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision=args.precision, device=local_rank)
-    solver.set_option(binding.OPT_GLOBAL_STEP_MATH, 0 if args.global_math == "tf32" else 1)
-    solver.set_option(binding.OPT_UPDATE_MODE, args.update_mode)
+    solver.set_option(binding.OPT_GLOBAL_STEP_MATH, {"tf32": 0, "fp32": 1, "tf32x2": 2}[args.global_math])
     solver.set_option(binding.OPT_LOCAL_STEP_IMPL, args.local_impl)
     if args.line_search:
         solver.set_line_search(args.line_search)
@@ -273,39 +405,50 @@ def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: 
     ktimes = solver.get_kernel_times(reset=True)
     solver.set_option(binding.OPT_KERNEL_TIMING, 0)
     elapsed_ms = max_over_ranks(elapsed_ms, world, dev)
+    # the fp32 default path must have run the tcgen05 GEMM: the SIMT GEMM is a different kernel kind and never a
+    # silent fallback (include/npfem.h NPFEM_KIND_GLOBAL_SIMT)
+    simt_launches = sum(n for _, n in ktimes["global_simt"])
+    if args.precision == "fp32" and args.global_math != "fp32" and simt_launches:
+        raise RuntimeError(f"the fp32 tensor-core path launched the SIMT GEMM {simt_launches} times: refusing to report")
     cell_iters = pop.n_cells * n_iterations * args.steps
     value = aggregate_throughput(pop.n_cells, n_iterations, args.steps, world, elapsed_ms)
 
     # ---- per-kernel rooflines from the live CUDA-event times ---------------------------------
     kernels, total_kernel_ms = [], sum(ms for v in ktimes.values() for ms, _ in v)
-    for kind in ("local", "global"):
+    for kind in ("local", "global", "global_simt"):
         for t, ct in enumerate(pop.types):
             ms, cnt = ktimes[kind][t]
             cells_t = int(np.sum(pop.type_of_cell == t))
             if cnt == 0 or cells_t == 0:
                 continue
             per_launch_s = ms * 1e-3 / cnt
-            bytes_launch = algorithmic_bytes(kind, ct.n_vertices, es) * cells_t
+            bytes_launch = algorithmic_bytes("local" if kind == "local" else "global", ct.n_vertices, es) * cells_t
             row = {"kernel": f"{kind}:{ct.name}", "launches": cnt, "avg_ms": ms / cnt,
                    "share_of_kernel_time": ms / total_kernel_ms,
                    "hbm_gbs": bytes_launch / per_launch_s / 1e9,
                    "hbm_frac": bytes_launch / per_launch_s / 1e9 / peaks["hbm_gbs"]}
-            if kind == "global":
+            if kind != "local":
                 tflops = global_flops(ct.n_vertices) * cells_t / per_launch_s / 1e12
-                # TF32 dense peak = measured bf16 peak x nominal ratio 1/2 (B200_PROFILING.md); fp32/fp64 SIMT
-                # paths are reported against the same tensor figure for context only
+                # TF32 / FP64 dense GEMM peaks: measured on the box by `bench.py --peaks` (profiles/r2_measured_peaks.json),
+                # the sustained figure because the kernel is timed inside a long step
                 row["tflops"] = tflops
-                row["tensor_frac_tf32"] = tflops / (0.5 * peaks["bf16_tflops_sustained"])
+                if kind == "global":
+                    row["tensor_frac_tf32"] = tflops / peaks["tf32_tflops_sustained"]
+                else:
+                    row["frac_of_" + ("fp64_gemm" if args.precision == "fp64" else "fp32_ffma") + "_peak"] = \
+                        tflops / (peaks["fp64_tflops"] if args.precision == "fp64" else peaks["fp32_ffma_tflops"])
+                row["peak_source"] = peaks["own_source"]
             kernels.append(row)
     dominant = max(kernels, key=lambda r: r["share_of_kernel_time"]) if kernels else None
     roofline = None
-    capture = load_ncu_capture()
-    same_workload = capture.get("cells") == pop.n_cells and capture.get("precision") == args.precision
+    same_workload = NCU_WORKLOAD["cells"] == pop.n_cells and NCU_WORKLOAD["precision"] == args.precision and \
+        args.global_math == "tf32" and args.local_impl == 0 and not args.line_search
     if dominant:
-        cap = capture.get("kernels", {}).get(dominant["kernel"]) if same_workload else None
+        cap = load_ncu_raw(dominant["kernel"]) if same_workload else None
         roofline = {"kernel": dominant["kernel"], "bound": "hbm", "achieved": dominant["hbm_gbs"],
                     "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": dominant["hbm_frac"],
                     "traffic": cap["dram_bytes"] if cap else None,
+                    "traffic_source": cap["file"] if cap else None,
                     "peak_source": peaks["source"] + " (MEASURED_PEAKS.json hbm_gbs)",
                     "note": "north_star names HBM for the local step; the kernel is bound by instruction issue and "
                             "shared-memory wavefronts (DESIGN.md 7.1), see `alu`"}
@@ -319,12 +462,15 @@ def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: 
             if cap.get("fp32_flop"):
                 # achieved FP32 FLOP/s (fadd + fmul + 2 ffma, ncu op counts) against
                 # 148 SMs x 128 lanes x 2 x the max SM clock
-                fp32_peak = 148 * 128 * 2 * sm_mhz * 1e6 / 1e12
+                fp32_peak = peaks["fp32_ffma_tflops"]
                 tf = cap["fp32_flop"] / (dominant["avg_ms"] * 1e-3) / 1e12
-                roofline["fp32"] = {"achieved": tf, "peak": fp32_peak, "unit": "TFLOP/s", "frac": tf / fp32_peak}
+                roofline["fp32"] = {"achieved": tf, "peak": fp32_peak, "unit": "TFLOP/s", "frac": tf / fp32_peak,
+                                    "peak_source": peaks["own_source"]}
     for row in kernels:
-        cap = capture.get("kernels", {}).get(row["kernel"]) if same_workload else None
+        cap = load_ncu_raw(row["kernel"]) if same_workload else None
         row["traffic"] = cap["dram_bytes"] if cap else None
+        if cap and cap.get("tensor_pipe_active_pct") is not None and row["kernel"].startswith("global"):
+            row["tensor_pipe_active_pct_ncu"] = cap["tensor_pipe_active_pct"]
 
     result = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -366,6 +512,8 @@ def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: 
 
 def main():
     args = parse_args()
+    if args.peaks:
+        return run_peaks()
     rank = int(os.environ.get("RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))
     from workloads import CONFIG_NAMES, make_config

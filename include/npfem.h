@@ -20,7 +20,8 @@
  *   - Units: micrometre, microsecond, femtogram, piconewton.
  *   - Per-cell user buffers hold the paper's x in R^{n x 3}: `[n_vertices][3]`
  *     (xyz interleaved), the listed cells back to back in `cell_ids` order;
- *     `cell_ids == NULL` means all cells in cell-id order 0..n_cells-1.
+ *     `cell_ids == NULL` means all cells in cell-id order 0..n_cells-1.  The ids
+ *     of a list must be distinct (NPFEM_EINVAL otherwise).
  *   - `dtype` of a user buffer is NPFEM_F32 or NPFEM_F64 and is independent of
  *     the context's compute precision (fp64 I/O on an fp32 context keeps the
  *     placement of cells far from the origin exact: state is stored in
@@ -62,8 +63,11 @@ extern "C" {
 #define NPFEM_HOST   1
 
 /* options for npfem_set_option */
-#define NPFEM_OPT_DIAGNOSTICS      1  /* 1: record the objective before every iteration (row a5) */
-#define NPFEM_OPT_GLOBAL_STEP_MATH 2  /* fp32 contexts: 0 = TF32 tensor cores (default), 1 = FP32 FFMA */
+#define NPFEM_OPT_DIAGNOSTICS      1  /* 1: record the objective before every iteration (row a5); needs the scratch of
+                                         NPFEM_FEATURE_DIAGNOSTICS (see npfem_bind_scratch) */
+#define NPFEM_OPT_GLOBAL_STEP_MATH 2  /* fp32 contexts: 0 = TF32 tensor cores (default), 1 = FP32 FFMA, 2 = TF32 tensor cores with
+                                         the operator split in two TF32 terms H~^-1 = W_hi + W_lo (twice the tensor work; removes
+                                         the bias TF32 rounding of H~^-1 leaves in the fixed point) */
 #define NPFEM_OPT_LOCAL_STEP_IMPL  3  /* 0 = auto, 1 = generic kernel, 2 = shared-memory persistent kernel,
                                          3 = scheduled kernel (register-resident topology, conflict-free slots),
                                          4 = large-mesh kernel (chunked corner forces, e.g. 2562-vertex cells) */
@@ -73,8 +77,8 @@ extern "C" {
                                             (per component, vertex + neighbours, even counts average) */
 #define NPFEM_OPT_FUSED_STEP       7  /* whole step of a cell in ONE kernel (fp32, small batches): 0 = auto (a bucket of at
                                          most 1.5 cells per SM), 1 = never, 2 = whenever the cell type allows it */
-#define NPFEM_OPT_UPDATE_MODE      5  /* fp32 tensor-core global step: 0 = auto (= 1), 1 = the GEMM epilogue updates d in place,
-                                         2 = the GEMM writes its product, the next local step applies it */
+#define NPFEM_OPT_UPDATE_MODE      5  /* fp32 tensor-core global step: 0 / 1 = the GEMM epilogue updates d in place (the only
+                                         mode; the product-out mode 2 of earlier versions was slower and is gone) */
 
 /* kernel kinds reported by npfem_get_kernel_times */
 #define NPFEM_KIND_PROLOGUE 0
@@ -83,7 +87,15 @@ extern "C" {
 #define NPFEM_KIND_EPILOGUE 3
 #define NPFEM_KIND_LINE_SEARCH 4   /* objective evaluations + accept / backtrack kernels */
 #define NPFEM_KIND_FUSED_STEP  5   /* whole-step kernel of the small-batch path */
-#define NPFEM_KIND_COUNT    6
+#define NPFEM_KIND_GLOBAL_SIMT 6   /* global step on the SIMT GEMM (fp64 contexts: DMMA; fp32: only when NPFEM_OPT_GLOBAL_STEP_MATH
+                                      = 1 or the shape does not fit the tcgen05 kernel).  NPFEM_KIND_GLOBAL is the tcgen05 kernel
+                                      alone: a tensor-core launch that fails is NPFEM_ECUDA, never a silent fall back */
+#define NPFEM_KIND_COUNT    7
+
+/* optional features that need scratch memory (npfem_scratch_bytes / npfem_bind_scratch) */
+#define NPFEM_FEATURE_DIAGNOSTICS 1   /* objective history, NPFEM_MAX_ITERATIONS + 1 rows of n_cells doubles */
+#define NPFEM_FEATURE_LINE_SEARCH 2   /* per-cell search state, a copy of d, fp32: the 3xTF32 operands */
+#define NPFEM_FEATURE_COLLISIONS  4   /* PIK targets (fp64, global coordinates) and stiffnesses */
 
 #define NPFEM_MAX_ITERATIONS 256
 
@@ -132,6 +144,19 @@ int npfem_create(npfem_ctx **out, const npfem_cell_type *types, int32_t n_types,
 size_t npfem_workspace_bytes(const npfem_ctx *ctx);
 int npfem_bind_workspace(npfem_ctx *ctx, void *dev_ptr, size_t bytes);
 
+/*
+ * The workspace holds everything the plain step needs, the create-time temporaries of the H~ inverse included
+ * (they are overlaid by the state).  The OPTIONAL features (NPFEM_FEATURE_*: diagnostics, line search, collisions)
+ * keep their memory in a separate scratch arena.  A caller that binds its own workspace binds the scratch too,
+ * BEFORE enabling the feature: npfem_scratch_bytes(ctx, mask) bytes for the features in `mask`, 256-byte aligned,
+ * valid until npfem_destroy; enabling a feature without it fails with NPFEM_ENOMEM.  With a library-owned
+ * workspace the enabling call (npfem_set_option(NPFEM_OPT_DIAGNOSTICS), npfem_set_line_search,
+ * npfem_set_collisions) allocates the feature's scratch itself.  Either way npfem_step never allocates.
+ * Errors: NPFEM_EINVAL (mask, alignment), NPFEM_ENOMEM (too small), NPFEM_ESTATE (feature already has memory).
+ */
+size_t npfem_scratch_bytes(const npfem_ctx *ctx, int32_t features);
+int npfem_bind_scratch(npfem_ctx *ctx, void *dev_ptr, size_t bytes, int32_t features);
+
 /* Runtime switches (NPFEM_OPT_*). */
 int npfem_set_option(npfem_ctx *ctx, int32_t option, int64_t value);
 
@@ -159,7 +184,7 @@ int npfem_step(npfem_ctx *ctx, int32_t n_iterations);
 /*
  * The same time step as npfem_set_forces(all cells) + npfem_step + npfem_get_state(all cells) with HOST
  * buffers, pipelined: cells are independent within a step, so the population is cut
- * into `n_chunks` ranges of cell ids (0 = chosen from the buffer size, at most 64); chunk i's solver
+ * into `n_chunks` ranges of cell ids (1..64; 0 = chosen from the buffer size, at most 16); chunk i's solver
  * kernels run while chunk i+1's forces are copied in and chunk i-1's state is copied out on two copy
  * streams.  Results are bit-identical to the unpipelined sequence.  `forces` [in], `positions` and
  * `velocities` [out] are HOST buffers of all cells in cell-id order, each `[n][3]`, dtype `dtype`; use
@@ -194,9 +219,8 @@ int npfem_get_objective(npfem_ctx *ctx, double *history, int32_t max_entries,
  * halved while g(d + alpha p) > g(d) + armijo_c1 alpha <grad g, p>, at most max_halvings (<= 30) times,
  * p = -H~^-1 grad g; d <- d + alpha p.  With it on, every iteration evaluates the objective (fp64) at the
  * trial point of every cell not yet accepted, up to max_halvings + 1 times; fp32 contexts take p from a
- * 3xTF32 product on the tensor cores (fp32-grade: a plain TF32 direction makes the search stall) and hold
- * one more field-sized buffer per bucket plus one n_pad^2 matrix per type for it (NPFEM_ENOMEM if they
- * cannot be allocated at the next npfem_step).
+ * 3xTF32 product on the tensor cores (fp32-grade: a plain TF32 direction makes the search stall).  Needs the
+ * scratch of NPFEM_FEATURE_LINE_SEARCH (see npfem_bind_scratch): NPFEM_ENOMEM from this call if it is missing.
  */
 int npfem_set_line_search(npfem_ctx *ctx, int32_t max_halvings, double armijo_c1, double grad_tol);
 
@@ -206,7 +230,9 @@ int npfem_set_line_search(npfem_ctx *ctx, int32_t max_halvings, double armijo_c1
  * projection points from the caller's collision detection, global coordinates like positions) and
  * stiffness k `[n]` (pN/um, 0 = vertex not in contact), both of `dtype`, living `where` says.  The energy
  * sum_i 1/2 k_i |x_i - p_i|^2 enters grad g and the objective of every following step (not the constant
- * H~: keep k well below m_v / h^2), until overwritten or cleared.  Collision DETECTION is the caller's.
+ * H~: keep k well below m_v / h^2), until overwritten or cleared; the targets are kept in global coordinates, so
+ * they stay valid when a cell drifts (the local frame is re-centred) or gets a new state.  Collision DETECTION is
+ * the caller's.  Needs the scratch of NPFEM_FEATURE_COLLISIONS (see npfem_bind_scratch).
  */
 int npfem_set_collisions(npfem_ctx *ctx, const int64_t *cell_ids, int64_t n_ids, const void *targets,
                          const void *stiffness, int32_t dtype, int32_t where);
@@ -249,6 +275,16 @@ int64_t npfem_launch_count(const npfem_ctx *ctx);
  * Returns NPFEM_OK, NPFEM_EINVAL or NPFEM_EMESH (message via npfem_last_error(NULL)).
  */
 int npfem_local_schedule_stats(const npfem_cell_type *type, double dt, double *stats, int32_t n_stats);
+
+/*
+ * Measurement aid (not on the solver's path; SURVEY.md 8(d) "measure an FFMA peak on the box"): enqueues on
+ * `cuda_stream` a kernel of grid_ctas CTAs x 256 threads, every thread running 16 independent chains of
+ * `iterations` fused multiply-adds in `precision` (NPFEM_F32: FFMA, NPFEM_F64: DFMA).  The caller times it with
+ * CUDA events; *flops_out (HOST, may be NULL) = 2 * 16 * iterations * 256 * grid_ctas.  sink_dev: a DEVICE scalar of
+ * that precision.  Returns NPFEM_OK, NPFEM_EINVAL or NPFEM_ECUDA.
+ */
+int npfem_probe_fma_peak(void *cuda_stream, int32_t precision, int32_t grid_ctas, int32_t iterations, void *sink_dev,
+                         double *flops_out);
 
 /* Message of the last failure on `ctx` (ctx == NULL: of the last failed npfem_create). */
 const char *npfem_last_error(const npfem_ctx *ctx);

@@ -16,15 +16,16 @@ NPFEM_DEVICE, NPFEM_HOST = 0, 1
 OPT_DIAGNOSTICS, OPT_GLOBAL_STEP_MATH, OPT_LOCAL_STEP_IMPL, OPT_KERNEL_TIMING, OPT_UPDATE_MODE = 1, 2, 3, 4, 5
 OPT_FORCE_MEDIAN_FILTER = 6
 OPT_FUSED_STEP = 7
-KIND_NAMES = ("prologue", "local", "global", "epilogue", "line_search", "fused_step")
+KIND_NAMES = ("prologue", "local", "global", "epilogue", "line_search", "fused_step", "global_simt")
+FEATURE_DIAGNOSTICS, FEATURE_LINE_SEARCH, FEATURE_COLLISIONS = 1, 2, 4
 _ERR_NAMES = {-1: "NPFEM_EINVAL", -2: "NPFEM_EMESH", -3: "NPFEM_ECUDA", -4: "NPFEM_ENOMEM", -5: "NPFEM_ESTATE"}
 
 EXPORTED_SYMBOLS = (
-    "npfem_create", "npfem_workspace_bytes", "npfem_bind_workspace", "npfem_set_option",
+    "npfem_create", "npfem_workspace_bytes", "npfem_bind_workspace", "npfem_scratch_bytes", "npfem_bind_scratch", "npfem_set_option",
     "npfem_set_state", "npfem_set_forces", "npfem_step", "npfem_step_host", "npfem_get_state", "npfem_get_objective",
     "npfem_get_kernel_times", "npfem_launch_count", "npfem_last_error", "npfem_version", "npfem_destroy",
     "npfem_local_schedule_stats", "npfem_set_line_search", "npfem_get_step_lengths", "npfem_set_velocity_cap", "npfem_set_collisions",
-    "npfem_clear_collisions",
+    "npfem_clear_collisions", "npfem_probe_fma_peak",
 )
 
 
@@ -72,6 +73,10 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.npfem_workspace_bytes.restype = sz
     lib.npfem_bind_workspace.argtypes = [vp, vp, sz]
     lib.npfem_bind_workspace.restype = C.c_int
+    lib.npfem_scratch_bytes.argtypes = [vp, i32]
+    lib.npfem_scratch_bytes.restype = sz
+    lib.npfem_bind_scratch.argtypes = [vp, vp, sz, i32]
+    lib.npfem_bind_scratch.restype = C.c_int
     lib.npfem_set_option.argtypes = [vp, i32, i64]
     lib.npfem_set_option.restype = C.c_int
     lib.npfem_set_state.argtypes = [vp, C.POINTER(i64), i64, vp, vp, i32, i32]
@@ -108,6 +113,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.npfem_get_step_lengths.restype = C.c_int
     lib.npfem_local_schedule_stats.argtypes = [C.POINTER(_CellType), C.c_double, C.POINTER(C.c_double), i32]
     lib.npfem_local_schedule_stats.restype = C.c_int
+    lib.npfem_probe_fma_peak.argtypes = [vp, i32, i32, i32, vp, C.POINTER(C.c_double)]
+    lib.npfem_probe_fma_peak.restype = C.c_int
     _LIB = lib
     return lib
 
@@ -178,6 +185,7 @@ class Solver:
             raise NpfemError(rc, self._lib.npfem_last_error(None).decode())
         self._ctx = ctx
         self._workspace = None
+        self._scratch = {}            # feature bit -> torch tensor (the caller owns the device memory, npfem.h)
         if bind_torch_workspace:
             nbytes = int(self._lib.npfem_workspace_bytes(self._ctx))
             self._workspace = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=f"cuda:{self.device}")
@@ -218,8 +226,24 @@ class Solver:
             raise ValueError(f"{name} must be C-contiguous with {count} elements, got {arr.size}")
         return C.c_void_p(arr.ctypes.data), NPFEM_F32 if arr.dtype == np.float32 else NPFEM_F64, NPFEM_HOST, arr
 
+    def _ensure_scratch(self, feature: int) -> None:
+        """With a torch-owned workspace the optional features get torch-owned scratch too (npfem_bind_scratch),
+        bound before the call that enables the feature; a library-owned workspace allocates its own."""
+        if self._workspace is None or feature in self._scratch:
+            return
+        nbytes = int(self._lib.npfem_scratch_bytes(self._ctx, feature))
+        buf = self._torch.empty(max(nbytes, 256), dtype=self._torch.uint8, device=f"cuda:{self.device}")
+        self._check(self._lib.npfem_bind_scratch(self._ctx, C.c_void_p(buf.data_ptr()), buf.numel(), feature))
+        self._scratch[feature] = buf
+
+    @property
+    def scratch_bytes(self) -> int:
+        return sum(int(b.numel()) for b in self._scratch.values())
+
     # ---- the C-ABI calls ----------------------------------------------------------------------
     def set_option(self, option: int, value: int) -> None:
+        if option == OPT_DIAGNOSTICS and value:
+            self._ensure_scratch(FEATURE_DIAGNOSTICS)
         self._check(self._lib.npfem_set_option(self._ctx, option, int(value)))
 
     def set_state(self, positions, velocities=None, cell_ids=None) -> None:
@@ -244,6 +268,7 @@ class Solver:
         q, code_q, where_q, _k2 = self._buffer(stiffness, count // 3, "stiffness")
         if code != code_q or where != where_q:
             raise ValueError("targets and stiffness must share dtype and location")
+        self._ensure_scratch(FEATURE_COLLISIONS)
         self._check(self._lib.npfem_set_collisions(self._ctx, ids_p, n_ids, p, q, code, where))
 
     def clear_collisions(self) -> None:
@@ -292,6 +317,8 @@ class Solver:
 
     def set_line_search(self, max_halvings: int, armijo_c1: float = 1e-4, grad_tol: float = 0.0) -> None:
         """Armijo backtracking + gradient-norm stopping test for the following steps (0 = off)."""
+        if max_halvings > 0:
+            self._ensure_scratch(FEATURE_LINE_SEARCH)
         self._check(self._lib.npfem_set_line_search(self._ctx, int(max_halvings), float(armijo_c1), float(grad_tol)))
 
     def set_velocity_cap(self, v_max: float) -> None:
@@ -326,6 +353,7 @@ class Solver:
             self._lib.npfem_destroy(self._ctx)
             self._ctx = None
             self._workspace = None
+            self._scratch = {}
 
     def __del__(self):  # pragma: no cover
         try:

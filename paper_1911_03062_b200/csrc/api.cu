@@ -25,16 +25,26 @@ struct npfem_ctx {
   std::vector<int32_t> type_of_cell, slot_of_cell;
   std::vector<int64_t> user_offset_all;   // [n_cells+1] element offsets in all-cells order
   std::vector<uint8_t> cell_is_set;
+  std::vector<uint32_t> seen_epoch;       // duplicate detection in id lists
+  uint32_t epoch = 0;
   int64_t n_set = 0;
   // workspace
   unsigned char *ws = nullptr;
   size_t ws_bytes = 0;
   bool ws_owned = false, ready = false;
   struct Layout {
-    std::vector<size_t> type_off[18];     // per type: tri, nbr, rest, hinge, corner, vnbr, w, mass, inv_area, Hinv, Hinv_tf32
+    std::vector<size_t> type_off[19];     // per type: tri, nbr, rest, hinge, corner, vnbr, w, mass, inv_area, Hinv, Hinv_tf32
     std::vector<size_t> field_off[F_COUNT], origin_off, cellid_off, scratch_off;
     size_t views_off = 0, refs_all_off = 0, refs_tmp_off = 0, stage_a_off = 0, stage_b_off = 0, stage_c_off = 0, total = 0;
+    // create-time arena (the fp64 H~, its inverse and the Newton-Schulz temporaries of ONE type at a time): starts
+    // right after the per-type tables and is overlaid by the state fields, which are first written by set_state
+    size_t setup_off = 0, setup_bytes = 0;
   } lay;
+  // Optional features (diagnostics history, line-search state and operands, collision tables) live in a SCRATCH
+  // arena: bound by the caller (npfem_bind_scratch) or, when the library owns its workspace, allocated by the call
+  // that enables the feature - never inside npfem_step.
+  struct FeatureMem { unsigned char *base = nullptr; size_t bytes = 0; bool owned = false, wanted = false, live = false; };
+  FeatureMem feat[3];                     // index = log2(NPFEM_FEATURE_*)
   BucketView *views_dev = nullptr;
   CellRef *refs_all_dev = nullptr, *refs_tmp_dev = nullptr;
   std::vector<int64_t *> cell_id_dev;
@@ -44,18 +54,18 @@ struct npfem_ctx {
   std::vector<cudaEvent_t> io_events;
   // diagnostics
   bool diagnostics = false;
-  double *history_dev = nullptr;
-  int history_cap = 0, history_entries = 0;
-  int64_t opt_global_math = 0, opt_local_impl = 0, opt_update_mode = 0, opt_fused_step = 0;
+  double *history_dev = nullptr;          // [NPFEM_MAX_ITERATIONS + 1][n_cells], in feat[0]
+  int history_entries = 0;
+  int64_t opt_global_math = 0, opt_local_impl = 0, opt_fused_step = 0;
   // line search (npfem_set_line_search)
   int ls_max_halvings = 0;
   double ls_c1 = 1e-4, ls_tol = 0.0;
-  std::vector<LineSearchDev> ls;          // per bucket, allocated on first use
+  std::vector<LineSearchDev> ls;          // per bucket, carved from feat[1]
   bool ls_ran = false;
   // coupling-side options
   bool median_filter = false;
   double v_max = 0.0;
-  std::vector<CollisionDev> col;          // per bucket, allocated by the first npfem_set_collisions
+  std::vector<CollisionDev> col;          // per bucket, carved from feat[2]
   CollisionDev *col_dev = nullptr;        // the same table on the device
   bool col_active = false;
   int64_t launches = 0;
@@ -95,6 +105,10 @@ int fail(npfem_ctx *c, int code, const std::string &msg) {
   } while (0)
 
 int check_launch(npfem_ctx *c, int n, const char *what) {
+  if (n == -2) {   // the launch (or its setup: attribute, tensor map) failed: a CUDA error, sticky
+    const cudaError_t e = cudaGetLastError();
+    return fail(c, NPFEM_ECUDA, std::string(what) + ": launch failed: " + (e != cudaSuccess ? cudaGetErrorString(e) : "driver call refused"));
+  }
   if (n < 0) return fail(c, NPFEM_ESTATE, std::string(what) + ": unsupported configuration");
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(c, NPFEM_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
@@ -163,6 +177,7 @@ void compute_layout(npfem_ctx *c) {
   L.origin_off.assign(nt, 0);
   L.cellid_off.assign(nt, 0);
   L.scratch_off.assign(nt, 0);
+  // (1) the constant per-type tables of ALL types, (2) the create-time arena, overlaid by (3) the per-bucket state
   for (size_t t = 0; t < nt; ++t) {
     const HostTypeData &h = c->host_types[t];
     const size_t n = h.n, T = h.T, vm = h.valence_max, np = h.n_pad;
@@ -186,8 +201,16 @@ void compute_layout(npfem_ctx *c) {
     L.type_off[15][t] = take(sc.valid ? sc.tri_consts.size() * 4 : 0);
     L.type_off[16][t] = take(sc.valid ? sc.vtx_words.size() * 4 : 0);
     L.type_off[17][t] = take(sc.valid ? sc.vtx_coef.size() * 4 : 0);
+    L.type_off[18][t] = take(f32 ? np * np * 4 : 0);   // W_lo
+    L.setup_bytes = std::max(L.setup_bytes, (2 * n * n + invert_spd_tmp_doubles(h.n)) * sizeof(double));
+  }
+  L.setup_off = off;
+  for (size_t t = 0; t < nt; ++t) {
+    const HostTypeData &h = c->host_types[t];
+    const size_t np = h.n_pad;
+    const bool f32 = c->precision == NPFEM_F32;
     const size_t cells = size_t(c->buckets[t].cells);
-    for (int f = 0; f < F_COUNT; ++f) L.field_off[f][t] = take(cells * 3 * np * es);
+    for (int f = 0; f < F_COUNT; ++f) L.field_off[f][t] = take(f == F_XL && !f32 ? 0 : cells * 3 * np * es);
     L.origin_off[t] = take(cells * 3 * sizeof(double));
     L.cellid_off[t] = take(cells * sizeof(int64_t));
     TypeDev tmp;
@@ -201,7 +224,104 @@ void compute_layout(npfem_ctx *c) {
   L.stage_a_off = take(size_t(c->total_vertices) * 3 * sizeof(double));
   L.stage_b_off = take(size_t(c->total_vertices) * 3 * sizeof(double));
   L.stage_c_off = take(size_t(c->total_vertices) * 3 * sizeof(double));
-  L.total = off;
+  L.total = std::max(off, align_up(L.setup_off + L.setup_bytes));
+}
+
+// ---- optional features: scratch arena ---------------------------------------------------------
+constexpr int FEAT_DIAG = 0, FEAT_LS = 1, FEAT_COL = 2, FEAT_COUNT = 3;
+
+bool ls_wants_3xtf32(const npfem_ctx *c, size_t t) {
+  return c->precision == NPFEM_F32 && c->host_types[t].n_pad > 0 && c->types.size() > t && c->types[t].Hinv_tf32 &&
+         global_tcgen05_supported(c->types[t]);
+}
+
+// bytes of one feature (a pure function of the context: same answer before and after the workspace is bound)
+size_t feature_bytes(const npfem_ctx *c, int f) {
+  const size_t es = esize(c->precision), nb = c->buckets.size();
+  size_t total = 0;
+  if (f == FEAT_DIAG) return align_up(size_t(NPFEM_MAX_ITERATIONS + 1) * size_t(c->n_cells ? c->n_cells : 1) * sizeof(double));
+  for (size_t t = 0; t < nb; ++t) {
+    const size_t cells = size_t(c->buckets[t].cells), np = size_t(c->host_types[t].n_pad);
+    if (f == FEAT_LS) {
+      total += align_up(4 * cells * sizeof(double)) + align_up(cells * sizeof(int)) + align_up(cells * 3 * np * es);
+      if (c->precision == NPFEM_F32) total += align_up(cells * 3 * np * 4);   // g_lo of the 3xTF32 product
+    } else {
+      total += align_up(cells * 3 * np * sizeof(double)) + align_up(cells * np * es);
+    }
+  }
+  if (f == FEAT_COL) total += align_up(nb * sizeof(CollisionDev));
+  return total;
+}
+
+// carve a live feature out of its arena and initialise it (stream-ordered; called once per feature, never from npfem_step)
+int materialise_feature(npfem_ctx *c, int f) {
+  npfem_ctx::FeatureMem &m = c->feat[f];
+  if (m.live) return NPFEM_OK;
+  const size_t need = feature_bytes(c, f);
+  if (!m.base) {
+    if (c->ws && !c->ws_owned)
+      return fail(c, NPFEM_ENOMEM, "the workspace is caller-owned: bind " + std::to_string(need) +
+                                       " bytes of scratch for this feature first (npfem_scratch_bytes / npfem_bind_scratch)");
+    void *p = nullptr;
+    if (cudaMalloc(&p, need ? need : 256) != cudaSuccess) {
+      cudaGetLastError();
+      return fail(c, NPFEM_ENOMEM, "cannot allocate " + std::to_string(need) + " bytes of scratch");
+    }
+    m.base = static_cast<unsigned char *>(p);
+    m.bytes = need;
+    m.owned = true;
+  }
+  if (m.bytes < need) return fail(c, NPFEM_ENOMEM, "scratch too small for this feature: need " + std::to_string(need) + " bytes");
+  // caller memory arrives with whatever it held: the padding columns of g_lo and d_old are never written by the
+  // kernels but ARE read by the GEMM (a NaN there times a zero of the operator is a NaN)
+  if (need) NPFEM_CUDA(c, cudaMemsetAsync(m.base, 0, need, c->stream));
+  const size_t es = esize(c->precision), nb = c->buckets.size();
+  unsigned char *p = m.base;
+  auto take = [&](size_t bytes) { unsigned char *q = p; p += align_up(bytes); return q; };
+  if (f == FEAT_DIAG) {
+    c->history_dev = reinterpret_cast<double *>(take(need));
+  } else if (f == FEAT_LS) {
+    c->ls.assign(nb, LineSearchDev());
+    for (size_t t = 0; t < nb; ++t) {
+      LineSearchDev &l = c->ls[t];
+      const size_t cells = size_t(c->buckets[t].cells), np = size_t(c->host_types[t].n_pad);
+      l.obj0 = reinterpret_cast<double *>(take(4 * cells * sizeof(double)));
+      l.obj1 = l.obj0 + cells;
+      l.slope = l.obj1 + cells;
+      l.alpha = l.slope + cells;
+      l.done = reinterpret_cast<int *>(take(cells * sizeof(int)));
+      l.d_old = take(cells * 3 * np * es);
+      if (c->precision == NPFEM_F32) {
+        float *g_lo = reinterpret_cast<float *>(take(cells * 3 * np * 4));
+        // fp32 + tensor-core global step: TF32 rounding of g and H~^-1 (2^-11 per entry) spoils the search direction in
+        // the stiff modes - on the violent case of tests/test_parity_gpu.py every cell ends up rejecting all step
+        // lengths by iteration 11 - so the line search takes its direction from a 3xTF32 product (fp32-grade)
+        if (cells && ls_wants_3xtf32(c, t)) l.g_lo = g_lo;
+      }
+    }
+  } else {
+    c->col.assign(nb, CollisionDev());
+    for (size_t t = 0; t < nb; ++t) {
+      const size_t slots = size_t(c->buckets[t].cells) * c->host_types[t].n_pad;
+      c->col[t].targets = reinterpret_cast<double *>(take(3 * slots * sizeof(double)));
+      c->col[t].stiffness = take(slots * es);
+      if (slots) {
+        NPFEM_CUDA(c, cudaMemsetAsync(c->col[t].targets, 0, 3 * slots * sizeof(double), c->stream));
+        NPFEM_CUDA(c, cudaMemsetAsync(c->col[t].stiffness, 0, slots * es, c->stream));
+      }
+    }
+    c->col_dev = reinterpret_cast<CollisionDev *>(take(nb * sizeof(CollisionDev)));
+    NPFEM_CUDA(c, cudaMemcpyAsync(c->col_dev, c->col.data(), nb * sizeof(CollisionDev), cudaMemcpyHostToDevice, c->stream));
+    NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+  }
+  m.live = true;
+  return NPFEM_OK;
+}
+
+// a feature was asked for: materialise it now if the workspace is ready, else when it becomes ready
+int want_feature(npfem_ctx *c, int f) {
+  c->feat[f].wanted = true;
+  return c->ready ? materialise_feature(c, f) : NPFEM_OK;
 }
 
 template <typename T>
@@ -336,36 +456,42 @@ int ensure_ready(npfem_ctx *c) {
       sd.vtx_coef = reinterpret_cast<const float *>(c->ws + L.type_off[17][t]);
     }
 
-    // dense inverse of H~ on the device (fp64), then cast/pad to the compute type
-    double *H64 = nullptr, *Hinv64 = nullptr;
+    // dense inverse of H~ on the device (fp64), then cast/pad to the compute type.  H~, the inverse and the
+    // Newton-Schulz temporaries sit in the create-time arena of the workspace (overlaid by the state fields, which
+    // nothing has written yet): the library allocates no device memory of its own here
     const size_t hb = size_t(h.n) * h.n * sizeof(double);
-    if (cudaMalloc(&H64, hb) != cudaSuccess || cudaMalloc(&Hinv64, hb) != cudaSuccess) {
-      cudaGetLastError();
-      cudaFree(H64);
-      return fail(c, NPFEM_ENOMEM, "cannot allocate the temporaries for the H~ inverse");
-    }
+    double *H64 = reinterpret_cast<double *>(c->ws + L.setup_off), *Hinv64 = H64 + size_t(h.n) * h.n;
+    double *inv_tmp = Hinv64 + size_t(h.n) * h.n;
     cudaError_t e = cudaMemcpyAsync(H64, h.H.data(), hb, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     std::string ierr;
     double residual = 0;
-    int nl = e == cudaSuccess ? launch_invert_spd(H64, Hinv64, h.n, c->stream, &residual, ierr) : -1;
+    int nl = e == cudaSuccess ? launch_invert_spd(H64, Hinv64, h.n, inv_tmp, c->stream, &residual, ierr) : -1;
     if (nl >= 0) {
       nl += launch_convert_pad(Hinv64, h.n, c->ws + L.type_off[9][t], h.n_pad, c->precision, c->stream);
-      if (c->precision == NPFEM_F32)   // the tensor-core operand: H~^-1 rounded to TF32 to nearest (internal.h, tf32_rn)
+      if (c->precision == NPFEM_F32) {   // the tensor-core operands: W_hi = H~^-1 rounded to TF32 to nearest (internal.h,
+        // tf32_rn) and W_lo = tf32(H~^-1 - W_hi) (split-operator GEMM, 3xTF32 line search)
         nl += launch_round_tf32(reinterpret_cast<const float *>(c->ws + L.type_off[9][t]),
                                 reinterpret_cast<float *>(c->ws + L.type_off[10][t]), size_t(h.n_pad) * h.n_pad, c->stream);
+        nl += launch_ls_split_w(reinterpret_cast<const float *>(c->ws + L.type_off[9][t]),
+                                reinterpret_cast<const float *>(c->ws + L.type_off[10][t]),
+                                reinterpret_cast<float *>(c->ws + L.type_off[18][t]), size_t(h.n_pad) * h.n_pad, c->stream);
+        d.Hinv_lo = c->ws + L.type_off[18][t];
+      }
       e = cudaStreamSynchronize(c->stream);
     }
-    cudaFree(H64);
-    cudaFree(Hinv64);
     if (e != cudaSuccess) return fail(c, NPFEM_ECUDA, std::string("H~ inverse: ") + cudaGetErrorString(e));
-    if (nl < 0) return fail(c, nl == -2 ? NPFEM_ENOMEM : NPFEM_ESTATE, ierr);
+    if (nl < 0) return fail(c, NPFEM_ESTATE, ierr);
     c->launches += nl;
-
-    // bucket
+  }
+  // the create-time arena is free again: buckets, cell tables (they overlay it)
+  for (size_t t = 0; t < nt; ++t) {
+    const HostTypeData &h = c->host_types[t];
+    int rc;
     Bucket &b = c->buckets[t];
     BucketView &bv = c->views[t];
-    for (int f = 0; f < F_COUNT; ++f) bv.field[f] = b.field[f] = c->ws + L.field_off[f][t];
+    for (int f = 0; f < F_COUNT; ++f)
+      bv.field[f] = b.field[f] = (f == F_XL && c->precision != NPFEM_F32) ? nullptr : c->ws + L.field_off[f][t];
     bv.origin = b.origin = reinterpret_cast<double *>(c->ws + L.origin_off[t]);
     bv.cells = b.cells;
     bv.n = h.n;
@@ -391,6 +517,8 @@ int ensure_ready(npfem_ctx *c) {
     refs[cell] = CellRef{c->user_offset_all[cell], c->type_of_cell[cell], c->slot_of_cell[cell]};
   if ((rc = upload_raw(c, L.refs_all_off, refs))) return rc;
   c->ready = true;
+  for (int f = 0; f < FEAT_COUNT; ++f)      // features asked for before the workspace existed
+    if (c->feat[f].wanted && (c->feat[f].base || c->ws_owned) && (rc = materialise_feature(c, f))) return rc;
   return NPFEM_OK;
 }
 
@@ -410,9 +538,18 @@ int resolve_refs(npfem_ctx *c, const int64_t *cell_ids, int64_t n_ids, const Cel
   if (n_ids < 0 || n_ids > c->n_cells) return fail(c, NPFEM_EINVAL, "n_ids out of range");
   std::vector<CellRef> refs(static_cast<size_t>(n_ids));
   int64_t off = 0;
+  // ids must be distinct: a repeated id would make the packed buffer larger than the staging areas and let two
+  // CTAs write the same cell (epoch-stamped table: O(n_ids) per call)
+  if (c->seen_epoch.size() != size_t(c->n_cells)) c->seen_epoch.assign(size_t(c->n_cells), 0);
+  if (++c->epoch == 0) {
+    std::fill(c->seen_epoch.begin(), c->seen_epoch.end(), 0u);
+    c->epoch = 1;
+  }
   for (int64_t i = 0; i < n_ids; ++i) {
     const int64_t id = cell_ids[i];
     if (id < 0 || id >= c->n_cells) return fail(c, NPFEM_EINVAL, "cell id " + std::to_string(id) + " out of range");
+    if (c->seen_epoch[size_t(id)] == c->epoch) return fail(c, NPFEM_EINVAL, "cell id " + std::to_string(id) + " listed twice");
+    c->seen_epoch[size_t(id)] = c->epoch;
     const int t = c->type_of_cell[id];
     refs[i] = CellRef{off, t, c->slot_of_cell[id]};
     off += int64_t(3) * c->host_types[t].n;
@@ -432,6 +569,15 @@ int resolve_refs(npfem_ctx *c, const int64_t *cell_ids, int64_t n_ids, const Cel
   *n_refs = n_ids;
   *n_elems = off;
   return NPFEM_OK;
+}
+
+// Small-batch path: does bucket t take the whole-step kernel?  ONE predicate for npfem_step and
+// npfem_step_host (which must not chunk a bucket that would take it unchunked, nor let a chunk fall into it).
+bool takes_fused_step(const npfem_ctx *c, size_t t) {
+  const bool plain = c->precision == NPFEM_F32 && !c->diagnostics && c->ls_max_halvings == 0 && !c->col_active &&
+                     c->opt_local_impl == 0 && c->opt_global_math == 0;
+  return plain && c->buckets[t].cells > 0 && c->opt_fused_step != 1 && step_fused_supported(c->types[t]) &&
+         (c->opt_fused_step == 2 || 2 * c->buckets[t].cells <= int64_t(3) * c->n_sm);
 }
 
 int common_checks(npfem_ctx *c, int32_t dtype, int32_t where) {
@@ -547,12 +693,52 @@ int npfem_bind_workspace(npfem_ctx *c, void *dev_ptr, size_t bytes) {
   return ensure_ready(c);
 }
 
+size_t npfem_scratch_bytes(const npfem_ctx *c, int32_t features) {
+  if (!c) return 0;
+  size_t total = 0;
+  for (int f = 0; f < FEAT_COUNT; ++f)
+    if (features & (1 << f)) total += feature_bytes(c, f);
+  return total;
+}
+
+int npfem_bind_scratch(npfem_ctx *c, void *dev_ptr, size_t bytes, int32_t features) {
+  if (!c) return NPFEM_EINVAL;
+  if (features <= 0 || features >= (1 << FEAT_COUNT)) return fail(c, NPFEM_EINVAL, "features must be a non-empty mask of NPFEM_FEATURE_*");
+  if (!dev_ptr || (reinterpret_cast<uintptr_t>(dev_ptr) & 255)) return fail(c, NPFEM_EINVAL, "scratch must be a 256-byte aligned device pointer");
+  if (bytes < npfem_scratch_bytes(c, features))
+    return fail(c, NPFEM_ENOMEM, "scratch too small: need " + std::to_string(npfem_scratch_bytes(c, features)) + " bytes");
+  for (int f = 0; f < FEAT_COUNT; ++f)
+    if ((features & (1 << f)) && c->feat[f].base) return fail(c, NPFEM_ESTATE, "scratch of this feature is already bound or allocated");
+  unsigned char *p = static_cast<unsigned char *>(dev_ptr);
+  for (int f = 0; f < FEAT_COUNT; ++f)
+    if (features & (1 << f)) {
+      c->feat[f].base = p;
+      c->feat[f].bytes = feature_bytes(c, f);
+      c->feat[f].owned = false;
+      p += c->feat[f].bytes;
+    }
+  if (c->ready)
+    for (int f = 0; f < FEAT_COUNT; ++f)
+      if ((features & (1 << f)) && c->feat[f].wanted) {
+        const int rc = materialise_feature(c, f);
+        if (rc) return rc;
+      }
+  return NPFEM_OK;
+}
+
 int npfem_set_option(npfem_ctx *c, int32_t option, int64_t value) {
   if (!c) return NPFEM_EINVAL;
   switch (option) {
-    case NPFEM_OPT_DIAGNOSTICS: c->diagnostics = value != 0; return NPFEM_OK;
+    case NPFEM_OPT_DIAGNOSTICS: {
+      if (value != 0) {   // the objective history needs scratch: bound by the caller or allocated here, not in npfem_step
+        const int rc = want_feature(c, FEAT_DIAG);
+        if (rc) return rc;
+      }
+      c->diagnostics = value != 0;
+      return NPFEM_OK;
+    }
     case NPFEM_OPT_GLOBAL_STEP_MATH:
-      if (value < 0 || value > 1) return fail(c, NPFEM_EINVAL, "global-step math must be 0 (TF32) or 1 (FP32)");
+      if (value < 0 || value > 2) return fail(c, NPFEM_EINVAL, "global-step math must be 0 (TF32), 1 (FP32) or 2 (TF32, split operator)");
       c->opt_global_math = value;
       return NPFEM_OK;
     case NPFEM_OPT_LOCAL_STEP_IMPL:
@@ -565,9 +751,8 @@ int npfem_set_option(npfem_ctx *c, int32_t option, int64_t value) {
       if (value < 0 || value > 2) return fail(c, NPFEM_EINVAL, "fused-step option must be 0, 1 or 2");
       c->opt_fused_step = value;
       return NPFEM_OK;
-    case NPFEM_OPT_UPDATE_MODE:
-      if (value < 0 || value > 2) return fail(c, NPFEM_EINVAL, "update mode must be 0, 1 or 2");
-      c->opt_update_mode = value;
+    case NPFEM_OPT_UPDATE_MODE:   // kept for old callers: the product-out mode (2) was measured slower and is gone
+      if (value < 0 || value > 1) return fail(c, NPFEM_EINVAL, "update mode must be 0 or 1 (the GEMM epilogue updates d in place)");
       return NPFEM_OK;
     default: return fail(c, NPFEM_EINVAL, "unknown option");
   }
@@ -658,24 +843,10 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   if (!c->ready || c->n_set != c->n_cells) return fail(c, NPFEM_ESTATE, "step before every cell has been given a state");
   int rc;
   const size_t nb = c->buckets.size();
-  if (c->diagnostics) {
-    const int need = n_iterations + 1;
-    if (need > c->history_cap) {
-      if (c->history_dev) NPFEM_CUDA(c, cudaFree(c->history_dev));
-      c->history_dev = nullptr;
-      c->history_cap = 0;
-      void *p = nullptr;
-      if (cudaMalloc(&p, size_t(need) * size_t(c->n_cells ? c->n_cells : 1) * sizeof(double)) != cudaSuccess) {
-        cudaGetLastError();
-        return fail(c, NPFEM_ENOMEM, "cannot allocate the objective history");
-      }
-      c->history_dev = static_cast<double *>(p);
-      c->history_cap = need;
-    }
-    c->history_entries = need;
-  } else {
-    c->history_entries = 0;
-  }
+  // the objective history lives in the scratch arena (feature DIAGNOSTICS, NPFEM_MAX_ITERATIONS + 1 rows):
+  // nothing is allocated here
+  c->history_entries = c->diagnostics ? n_iterations + 1 : 0;
+  if (c->diagnostics && !c->feat[FEAT_DIAG].live) return fail(c, NPFEM_ESTATE, "diagnostics are on but their scratch is not bound");
   auto diag = [&](int row) -> int {
     for (size_t t = 0; t < nb; ++t) {
       double *out = c->history_dev + size_t(row) * c->n_cells;
@@ -694,10 +865,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   // kernel, one CTA per cell (step_fused.cu); everything else goes through the batched kernels below.
   std::vector<char> whole(nb, 0);
   for (size_t t = 0; t < nb; ++t) {
-    const bool plain = c->precision == NPFEM_F32 && !c->diagnostics && c->ls_max_halvings == 0 && !c->col_active &&
-                       c->opt_local_impl == 0 && c->opt_global_math == 0 && c->opt_update_mode != 2;
-    whole[t] = plain && c->opt_fused_step != 1 && step_fused_supported(c->types[t]) &&
-               (c->opt_fused_step == 2 || 2 * c->buckets[t].cells <= int64_t(3) * c->n_sm);
+    whole[t] = takes_fused_step(c, t);
     if (whole[t] && (rc = timed_launch(c, NPFEM_KIND_FUSED_STEP, int(t), "fused step", [&] {
                        return launch_step_fused(c->types[t], c->views[t], c->n_sm, n_iterations, c->v_max, c->stream); })))
       return rc;
@@ -706,64 +874,18 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
     if (!whole[t] && (rc = timed_launch(c, NPFEM_KIND_PROLOGUE, int(t), "prologue", [&] {
            return launch_prologue(c->types[t], c->views[t], c->precision, c->stream); })))
       return rc;
-  // Product-out mode (NPFEM_OPT_UPDATE_MODE = 2; fp32, scheduled local step + tensor-core global step,
-  // no diagnostics): the global step only writes its product u = -H~^-1 r; the NEXT local step (or
-  // the epilogue) applies d <- (1 - gamma) d + u while it streams d anyway.  Measured slower than
-  // the default (the GEMM epilogue updates d in place from register-prefetched rows): 2.21 vs
-  // 2.15 ms per RBC-642 iteration at 90,000 cells, so auto (0) means mode 1.
   const bool ls_on = c->ls_max_halvings > 0;
-  if (ls_on) {
-    if (c->ls.size() != nb) c->ls.assign(nb, LineSearchDev());
-    for (size_t t = 0; t < nb; ++t) {
-      LineSearchDev &l = c->ls[t];
-      const size_t cells = size_t(c->buckets[t].cells);
-      if (l.obj0 || cells == 0) continue;
-      void *pd = nullptr, *pi = nullptr;
-      if (cudaMalloc(&pd, 4 * cells * sizeof(double)) != cudaSuccess || cudaMalloc(&pi, cells * sizeof(int)) != cudaSuccess) {
-        cudaGetLastError();
-        cudaFree(pd);
-        return fail(c, NPFEM_ENOMEM, "cannot allocate the line-search state");
-      }
-      l.obj0 = static_cast<double *>(pd);
-      l.obj1 = l.obj0 + cells;
-      l.slope = l.obj1 + cells;
-      l.alpha = l.slope + cells;
-      l.done = static_cast<int *>(pi);
-    }
-    // fp32 + tensor-core global step: TF32 rounding of g and H~^-1 (2^-11 per entry) spoils the search direction in
-    // the stiff modes - on the violent case of tests/test_parity_gpu.py every cell ends up rejecting all step
-    // lengths by iteration 11 - so the line search takes its direction from a 3xTF32 product (fp32-grade)
-    for (size_t t = 0; t < nb; ++t) {
-      LineSearchDev &l = c->ls[t];
-      const size_t cells = size_t(c->buckets[t].cells);
-      if (l.g_lo || cells == 0 || c->precision != NPFEM_F32 || c->opt_global_math != 0 || !c->types[t].Hinv_tf32 ||
-          !global_tcgen05_supported(c->types[t]))
-        continue;
-      const size_t nn = size_t(c->types[t].n_pad) * c->types[t].n_pad;
-      void *pg = nullptr, *pw = nullptr;
-      if (cudaMalloc(&pg, cells * 3 * c->types[t].n_pad * sizeof(float)) != cudaSuccess ||
-          cudaMalloc(&pw, nn * sizeof(float)) != cudaSuccess) {
-        cudaGetLastError();
-        cudaFree(pg);
-        return fail(c, NPFEM_ENOMEM, "cannot allocate the line-search operands");
-      }
-      l.g_lo = static_cast<float *>(pg);
-      l.w_lo = static_cast<float *>(pw);
-      if ((rc = check_launch(c, launch_ls_split_w(static_cast<const float *>(c->types[t].Hinv),
-                                                  static_cast<const float *>(c->types[t].Hinv_tf32), l.w_lo, nn, c->stream),
-                             "line search: split of H~^-1")))
-        return rc;
-    }
-  }
-  std::vector<char> fused(nb, 0);
+  if (ls_on && !c->feat[FEAT_LS].live) return fail(c, NPFEM_ESTATE, "the line search is on but its scratch is not bound");
+  // which GEMM a bucket takes is decided HERE, before anything is launched: the tcgen05 kernel when the context is
+  // fp32, the option asks for TF32 and the shape is supported; otherwise the SIMT kernel, reported as its own kind
+  // (NPFEM_KIND_GLOBAL_SIMT).  A tensor-core launch that fails is an error, never a silent fallback.
+  std::vector<char> use_tc(nb, 0);
   for (size_t t = 0; t < nb; ++t)
-    fused[t] = !ls_on && !c->col_active && c->precision == NPFEM_F32 && !c->diagnostics && c->opt_global_math == 0 && c->opt_update_mode == 2 &&
-               (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]) &&
-               global_tcgen05_supported(c->types[t]);
+    use_tc[t] = c->precision == NPFEM_F32 && c->opt_global_math != 1 && global_tcgen05_supported(c->types[t]);
   // g feeds the TF32 tensor-core GEMM: the local step stores it already rounded to nearest (the line search
   // then takes its slope and gradient norm from the rounded gradient: 2^-12 relative per entry, random sign)
   for (size_t t = 0; t < nb; ++t)
-    c->views[t].g_tf32 = !ls_on && c->precision == NPFEM_F32 && c->opt_global_math == 0 && global_tcgen05_supported(c->types[t]);
+    c->views[t].g_tf32 = !ls_on && use_tc[t];
   for (int k = 0; k < n_iterations; ++k) {
     if (c->diagnostics && (rc = diag(k))) return rc;
     for (size_t t = 0; t < nb; ++t) {
@@ -779,7 +901,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
       const double d_scale = reduced && !ls_on ? 1.0 - c->types[t].gamma : 1.0;
       const BucketView &lv = c->views[t];
       if ((rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "local step", [&] {
-             if (sched) return launch_local_sched(c->types[t], lv, c->n_sm, fused[t] && k > 0, d_scale, c->stream);
+             if (sched) return launch_local_sched(c->types[t], lv, c->n_sm, c->stream);
              if (fast) return launch_local_smem(c->types[t], lv, c->n_sm, c->stream);
              if (big) return launch_local_big(c->types[t], lv, c->n_sm, c->stream);
              return launch_local_generic(c->types[t], lv, c->buckets[t].scratch, c->precision, c->n_sm,
@@ -787,7 +909,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
         return rc;
       // 3xTF32 operands of the line search's global step: split by the damping kernel, unless the collision term is
       // still to come or the generic kernel ran (then by launch_ls_split_g just before the GEMMs)
-      const bool split_early = ls_on && reduced && !c->col_active && c->ls[t].g_lo;
+      const bool split_early = ls_on && reduced && !c->col_active && use_tc[t] && c->ls[t].g_lo;
       if (ls_on && reduced && (rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "damping gradient", [&] {
                                  return launch_damping_grad(c->types[t], c->views[t], split_early ? c->ls[t].g_lo : nullptr,
                                                             c->n_sm, c->stream); })))
@@ -806,21 +928,20 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
                  nl += launch_collision_energy(c->views[t], c->col[t], nullptr, c->ls[t].obj0, nullptr, c->precision, c->stream);
                return nl; })))
           return rc;
-        NPFEM_CUDA(c, cudaMemcpyAsync(c->views[t].field[F_U], c->views[t].field[F_D], bytes, cudaMemcpyDeviceToDevice, c->stream));
+        NPFEM_CUDA(c, cudaMemcpyAsync(c->ls[t].d_old, c->views[t].field[F_D], bytes, cudaMemcpyDeviceToDevice, c->stream));
       }
-      if ((rc = timed_launch(c, NPFEM_KIND_GLOBAL, int(t), "global step", [&] {
-             if (ls_on && c->ls[t].g_lo) {     // 3xTF32: d <- d - (g_hi W_hi + g_lo W_hi + g_hi W_lo), one K-concatenated GEMM
+      const bool tc3 = ls_on && use_tc[t] && c->ls[t].g_lo;
+      if ((rc = timed_launch(c, use_tc[t] ? NPFEM_KIND_GLOBAL : NPFEM_KIND_GLOBAL_SIMT, int(t), "global step", [&] {
+             if (tc3) {                         // 3xTF32: d <- d - (g_hi W_hi + g_lo W_hi + g_hi W_lo), one K-concatenated GEMM
                const LineSearchDev &l = c->ls[t];
                const size_t count = size_t(c->buckets[t].cells) * 3 * c->types[t].n_pad;
                int nl = split_early ? 0 : launch_ls_split_g(static_cast<float *>(c->views[t].field[F_G]), l.g_lo, count, c->stream);
-               const int n1 = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, 1.0, nullptr, c->stream, l.g_lo, l.w_lo);
-               return n1 < 0 ? -1 : nl + n1;
+               const int n1 = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, 1.0, c->stream, l.g_lo, c->types[t].Hinv_lo);
+               return n1 < 0 ? n1 : nl + n1;
              }
-             if (c->precision == NPFEM_F32 && c->opt_global_math == 0) {
-               const int n = launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, d_scale,
-                                                   fused[t] ? c->views[t].field[F_U] : nullptr, c->stream);
-               if (n >= 0 || fused[t]) return n;
-             }
+             if (use_tc[t])   // option 2: [g g] . [W_hi; W_lo], the operator to fp32 accuracy at twice the tensor work
+               return launch_global_tcgen05(c->types[t], c->views[t], c->n_sm, d_scale, c->stream, nullptr,
+                                            c->opt_global_math == 2 ? c->types[t].Hinv_lo : nullptr);
              return launch_global_simt(c->types[t], c->views[t], c->precision, d_scale, c->stream); })))
         return rc;
       if (ls_on && c->buckets[t].cells) {
@@ -842,8 +963,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
   if (c->diagnostics && (rc = diag(n_iterations))) return rc;
   for (size_t t = 0; t < nb; ++t)
     if (!whole[t] && (rc = timed_launch(c, NPFEM_KIND_EPILOGUE, int(t), "epilogue", [&] {
-           return launch_epilogue(c->types[t], c->views[t], c->precision, fused[t] != 0, 1.0 - c->types[t].gamma,
-                                  c->v_max, c->stream); })))
+           return launch_epilogue(c->types[t], c->views[t], c->precision, c->v_max, c->stream); })))
       return rc;
   return NPFEM_OK;
 }
@@ -862,17 +982,14 @@ int npfem_step_host(npfem_ctx *c, const void *forces, int32_t n_iterations, void
   if (!c->ready || c->n_set != c->n_cells) return fail(c, NPFEM_ESTATE, "step before every cell has been given a state");
   const size_t es = dtype == NPFEM_F32 ? 4 : 8;
   const int64_t total = c->total_vertices * 3;
-  if (n_chunks == 0) n_chunks = int32_t(std::min<int64_t>(16, std::max<int64_t>(1, int64_t(total * es) / (48 << 20))));
+  if (n_chunks == 0) n_chunks = int32_t(std::min<int64_t>(16, std::max<int64_t>(1, int64_t(total * es) / (48 << 20))));   // auto: <= 16
   n_chunks = int32_t(std::max<int64_t>(1, std::min<int64_t>(n_chunks, c->n_cells)));
   // per-cell reductions over the whole bucket (history rows, line-search state, collision tables) are
   // indexed by bucket slot: those modes take the unchunked sequence
   // the small-batch whole-step kernel is chosen by bucket size: a bucket that would take it unchunked is small
   // enough not to be worth chunking, and no chunk may fall into it when the whole bucket would not
-  bool small_batch = false;
-  if (c->opt_fused_step != 1)
-    for (size_t t = 0; t < c->buckets.size(); ++t)
-      small_batch = small_batch || (c->buckets[t].cells > 0 && step_fused_supported(c->types[t]) &&
-                                    (c->opt_fused_step == 2 || 2 * c->buckets[t].cells <= int64_t(3) * c->n_sm));
+  bool small_batch = false;      // the SAME predicate npfem_step uses (fp64 contexts, option-forced kernels ... never take it)
+  for (size_t t = 0; t < c->buckets.size(); ++t) small_batch = small_batch || takes_fused_step(c, t);
   if (c->diagnostics || c->ls_max_halvings > 0 || c->col_active || c->median_filter || small_batch || n_chunks == 1) {
     if ((rc = npfem_set_forces(c, nullptr, 0, forces, dtype, NPFEM_HOST))) return rc;
     if ((rc = npfem_step(c, n_iterations))) return rc;
@@ -926,7 +1043,8 @@ int npfem_step_host(npfem_ctx *c, const void *forces, int32_t n_iterations, void
     for (size_t t = 0; t < nb; ++t) {
       BucketView bv = full_views[t];
       const size_t shift = size_t(slot0[t]) * 3 * size_t(bv.n_pad) * esize(c->precision);
-      for (int f = 0; f < F_COUNT; ++f) bv.field[f] = static_cast<unsigned char *>(bv.field[f]) + shift;
+      for (int f = 0; f < F_COUNT; ++f)
+        if (bv.field[f]) bv.field[f] = static_cast<unsigned char *>(bv.field[f]) + shift;   // F_XL is null in fp64 contexts
       bv.origin += slot0[t] * 3;
       bv.cells = count[t];
       c->views[t] = bv;
@@ -961,6 +1079,10 @@ int npfem_set_line_search(npfem_ctx *c, int32_t max_halvings, double armijo_c1, 
   if (!c) return NPFEM_EINVAL;
   if (max_halvings < 0 || max_halvings > 30 || !(armijo_c1 >= 0) || !(armijo_c1 < 1) || !(grad_tol >= 0))
     return fail(c, NPFEM_EINVAL, "line search: 0 <= max_halvings <= 30, 0 <= armijo_c1 < 1, grad_tol >= 0");
+  if (max_halvings > 0) {   // per-cell search state, d_old, 3xTF32 operands: scratch, bound by the caller or allocated here
+    const int rc = want_feature(c, FEAT_LS);
+    if (rc) return rc;
+  }
   c->ls_max_halvings = max_halvings;
   c->ls_c1 = armijo_c1;
   c->ls_tol = grad_tol;
@@ -973,28 +1095,7 @@ int npfem_set_collisions(npfem_ctx *c, const int64_t *cell_ids, int64_t n_ids, c
   if (rc) return rc;
   if (!targets || !stiffness) return fail(c, NPFEM_EINVAL, "targets / stiffness is NULL");
   if (!c->ready || c->n_set != c->n_cells) return fail(c, NPFEM_ESTATE, "set_collisions before every cell has been given a state");
-  const size_t nb = c->buckets.size(), es = esize(c->precision);
-  if (c->col.size() != nb) {
-    c->col.assign(nb, CollisionDev());
-    for (size_t t = 0; t < nb; ++t) {
-      const size_t slots = size_t(c->buckets[t].cells) * c->types[t].n_pad;
-      if (!slots) continue;
-      if (cudaMalloc(&c->col[t].targets, 3 * slots * es) != cudaSuccess || cudaMalloc(&c->col[t].stiffness, slots * es) != cudaSuccess) {
-        cudaGetLastError();
-        return fail(c, NPFEM_ENOMEM, "cannot allocate the collision targets");
-      }
-      NPFEM_CUDA(c, cudaMemsetAsync(c->col[t].targets, 0, 3 * slots * es, c->stream));
-      NPFEM_CUDA(c, cudaMemsetAsync(c->col[t].stiffness, 0, slots * es, c->stream));
-    }
-    void *p = nullptr;
-    if (cudaMalloc(&p, nb * sizeof(CollisionDev)) != cudaSuccess) {
-      cudaGetLastError();
-      return fail(c, NPFEM_ENOMEM, "cannot allocate the collision table");
-    }
-    c->col_dev = static_cast<CollisionDev *>(p);
-    NPFEM_CUDA(c, cudaMemcpyAsync(c->col_dev, c->col.data(), nb * sizeof(CollisionDev), cudaMemcpyHostToDevice, c->stream));
-    NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
-  }
+  if ((rc = want_feature(c, FEAT_COL))) return rc;   // tables in the scratch arena (zeroed when first carved)
   PackArgs a{};
   int64_t n_elems = 0;
   if ((rc = resolve_refs(c, cell_ids, n_ids, &a.refs, &a.n_refs, &n_elems, false))) return rc;
@@ -1018,7 +1119,7 @@ int npfem_set_collisions(npfem_ctx *c, const int64_t *cell_ids, int64_t n_ids, c
 int npfem_clear_collisions(npfem_ctx *c) {
   if (!c) return NPFEM_EINVAL;
   if (c->sticky) return fail(c, NPFEM_ECUDA, "context is in a sticky CUDA error state: " + c->err);
-  for (size_t t = 0; t < c->col.size(); ++t) {
+  for (size_t t = 0; t < c->col.size() && c->feat[FEAT_COL].live; ++t) {
     const size_t slots = size_t(c->buckets[t].cells) * c->types[t].n_pad;
     if (slots) NPFEM_CUDA(c, cudaMemsetAsync(c->col[t].stiffness, 0, slots * esize(c->precision), c->stream));
   }
@@ -1187,18 +1288,8 @@ void npfem_destroy(npfem_ctx *c) {
   cudaSetDevice(c->device);
   cudaStreamSynchronize(c->stream);
   if (c->ws_owned && c->ws) cudaFree(c->ws);
-  if (c->history_dev) cudaFree(c->history_dev);
-  for (auto &cl : c->col) {
-    if (cl.targets) cudaFree(cl.targets);
-    if (cl.stiffness) cudaFree(cl.stiffness);
-  }
-  if (c->col_dev) cudaFree(c->col_dev);
-  for (auto &l : c->ls) {
-    if (l.g_lo) cudaFree(l.g_lo);
-    if (l.w_lo) cudaFree(l.w_lo);
-    if (l.obj0) cudaFree(l.obj0);
-    if (l.done) cudaFree(l.done);
-  }
+  for (auto &m : c->feat)
+    if (m.owned && m.base) cudaFree(m.base);
   for (auto &sp : c->spans) {
     cudaEventDestroy(sp.a);
     cudaEventDestroy(sp.b);

@@ -6,7 +6,8 @@
 //   * the vertex-velocity cap (reading R17) lives in the step epilogue (prologue.cu);
 //   * the PIK collision energy sum_i 1/2 k_i |x_i - p_i|^2 over the vertices the collision detection flagged
 //     (reading R19: it enters grad g and the objective, not the constant H~):
-//     npfem_set_collisions stores targets p (cell-local coordinates) and stiffnesses k per vertex, the
+//     npfem_set_collisions stores targets p (GLOBAL coordinates, fp64: the origin of a cell's local frame moves when
+//     the prologue re-centres it or set_state is called again) and stiffnesses k per vertex, the
 //     gradient term is added to the local step's output, the energy to the objective.
 #include "internal.h"
 
@@ -56,7 +57,7 @@ __device__ __forceinline__ double load_user(const void *p, int64_t i) {
   return double(static_cast<const U *>(p)[i]);
 }
 
-// one CTA per listed cell: user targets [n][3] / stiffness [n] -> cell-local SoA
+// one CTA per listed cell: user targets [n][3] / stiffness [n] -> SoA, targets kept in global coordinates (fp64)
 template <typename T, typename U>
 __global__ void __launch_bounds__(256)
 set_collisions_kernel(const BucketView *__restrict__ views, const CellRef *__restrict__ refs, const CollisionDev *cols,
@@ -65,11 +66,10 @@ set_collisions_kernel(const BucketView *__restrict__ views, const CellRef *__res
   const BucketView bv = views[ref.bucket];
   const CollisionDev col = cols[ref.bucket];
   const int n = bv.n, n_pad = bv.n_pad;
-  T *P = static_cast<T *>(col.targets) + size_t(ref.slot) * 3 * n_pad;
+  double *P = col.targets + size_t(ref.slot) * 3 * n_pad;
   T *W = static_cast<T *>(col.stiffness) + size_t(ref.slot) * n_pad;
-  const double *origin = bv.origin + size_t(ref.slot) * 3;
   for (int i = threadIdx.x; i < 3 * n; i += blockDim.x)
-    P[(i % 3) * n_pad + i / 3] = T(load_user<U>(targets, ref.user_offset + i) - origin[i % 3]);
+    P[(i % 3) * n_pad + i / 3] = load_user<U>(targets, ref.user_offset + i);
   for (int i = threadIdx.x; i < n; i += blockDim.x) W[i] = T(load_user<U>(stiffness, ref.user_offset / 3 + i));
 }
 
@@ -79,18 +79,22 @@ __global__ void __launch_bounds__(256)
 collision_grad_kernel(BucketView bv, CollisionDev col) {
   const T *x = static_cast<const T *>(bv.field[F_X]);
   const T *d = static_cast<const T *>(bv.field[F_D]);
+  const T *xl = static_cast<const T *>(bv.field[F_XL]);      // null in fp64 contexts
   T *g = static_cast<T *>(bv.field[F_G]);
-  const T *P = static_cast<const T *>(col.targets), *W = static_cast<const T *>(col.stiffness);
+  const double *P = col.targets;
+  const T *W = static_cast<const T *>(col.stiffness);
   const int n_pad = bv.n_pad;
   const size_t total = size_t(bv.cells) * n_pad;
   for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < total; i += size_t(gridDim.x) * blockDim.x) {
     const T w = W[i];
     if (w > T(0)) {
-      const size_t base = (i / n_pad) * 3 * size_t(n_pad) + i % n_pad;
+      const size_t cell = i / n_pad, base = cell * 3 * size_t(n_pad) + i % n_pad;
 #pragma unroll
       for (int k = 0; k < 3; ++k) {
         const size_t o = base + size_t(k) * n_pad;
-        g[o] += w * (x[o] + d[o] - P[o]);
+        // the target in the cell's CURRENT local frame (fp64 difference of two global coordinates)
+        const double local = (double(x[o]) + (xl ? double(xl[o]) : 0.0) + double(d[o])) - (P[o] - bv.origin[cell * 3 + k]);
+        g[o] += w * T(local);
       }
     }
   }
@@ -109,7 +113,9 @@ collision_energy_kernel(BucketView bv, CollisionDev col, const int64_t *__restri
     if (skip && skip[cell]) continue;
     const size_t base = size_t(cell) * 3 * n_pad;
     const T *x = static_cast<const T *>(bv.field[F_X]) + base, *d = static_cast<const T *>(bv.field[F_D]) + base;
-    const T *P = static_cast<const T *>(col.targets) + base;
+    const T *xl = bv.field[F_XL] ? static_cast<const T *>(bv.field[F_XL]) + base : nullptr;
+    const double *P = col.targets + base;
+    const double *origin = bv.origin + size_t(cell) * 3;
     const T *W = static_cast<const T *>(col.stiffness) + size_t(cell) * n_pad;
     double e = 0.0;
     for (int i = lane; i < n; i += 32) {
@@ -117,7 +123,8 @@ collision_energy_kernel(BucketView bv, CollisionDev col, const int64_t *__restri
       if (w > 0.0) {
         double r2 = 0.0;
         for (int k = 0; k < 3; ++k) {
-          const double r = double(x[k * n_pad + i]) + double(d[k * n_pad + i]) - double(P[k * n_pad + i]);
+          const double r = (double(x[k * n_pad + i]) + (xl ? double(xl[k * n_pad + i]) : 0.0) + double(d[k * n_pad + i])) -
+                           (P[k * n_pad + i] - origin[k]);
           r2 += r * r;
         }
         e += 0.5 * w * r2;
@@ -171,13 +178,13 @@ int launch_median_filter(const BucketView *views_dev, const CellRef *refs_dev, i
   const size_t smem = size_t(3) * td.n * es;
   if (smem > 200 * 1024 || td.valence_max > 32) return -1;
   if (precision == NPFEM_F32) {
-    if (smem > 48 * 1024 &&
-        cudaFuncSetAttribute(median_filter_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess)
+    if (smem > 48 * 1024 &&   // off the hot path (once per set_forces): set every time, the attribute is per device
+        cudaFuncSetAttribute(median_filter_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess)
       return -1;
     median_filter_kernel<float><<<unsigned(n_refs), 256, smem, s>>>(views_dev, refs_dev, bucket, td.vtx_nbr, td.valence_max);
   } else {
     if (smem > 48 * 1024 &&
-        cudaFuncSetAttribute(median_filter_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess)
+        cudaFuncSetAttribute(median_filter_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess)
       return -1;
     median_filter_kernel<double><<<unsigned(n_refs), 256, smem, s>>>(views_dev, refs_dev, bucket, td.vtx_nbr, td.valence_max);
   }

@@ -18,7 +18,9 @@
 //                           d_scale d + acc in place (row per lane, conflict-free) -> TMA store
 // Work item of a cluster = (CL consecutive M tiles, N pass); the passes of one group are adjacent items
 // (neighbouring clusters at about the same time), so the repeated G reads are L2 hits.
-// Line-search mode (k_segs = 3): the 3xTF32 product [g_hi g_lo g_hi] . [W_hi; W_hi; W_lo] as one GEMM with K = 3 n_pad;
+// Split-operator mode (k_segs = 2, NPFEM_OPT_GLOBAL_STEP_MATH = 2): [g g] . [W_hi; W_lo], the operator to ~fp32 accuracy
+// (the reduced-gradient identity is exact only for the exact H~^-1; TF32 rounding of W biases the
+// fixed point).  Line-search mode (k_segs = 3): the 3xTF32 product [g_hi g_lo g_hi] . [W_hi; W_hi; W_lo] as one GEMM with K = 3 n_pad;
 // the producer switches tensor maps per K segment, nothing else changes.
 #include <cuda.h>
 
@@ -128,14 +130,14 @@ __device__ __forceinline__ void umma_commit_mc(uint64_t *bar, uint16_t mask) {
 }
 
 struct GemmParams {
-  float *D;            // [rows][n_pad], updated in place (U == nullptr)
-  float *U;            // [rows][n_pad] or nullptr: write the raw product -G W here instead of updating D
+  float *D;            // [rows][n_pad], updated in place
   int64_t rows;
   int n_pad;
   int n_pass;          // accumulator columns per pass = N of the MMA (multiple of 16, <= MAX_NPASS)
   int passes;          // ceil(n_pad / n_pass)
   int k_chunks;        // ceil(n_pad / BK)
-  int k_segs;          // 1, or 3: K-concatenated 3xTF32 product [g_hi g_lo g_hi] . [W_hi; W_hi; W_lo] (line search)
+  int k_segs;          // 1; 2: [g g] . [W_hi; W_lo]; 3: K-concatenated 3xTF32 product [g_hi g_lo g_hi] . [W_hi; W_hi; W_lo]
+  int seg_g2, seg_w2;  // bit s set: K segment s reads the second G map (g_lo) / the second W map (W_lo)
   int64_t m_tiles;
   float d_scale;       // d <- d_scale * d + acc
   int stages;          // depth of the operand ring (<= MAX_STAGES)
@@ -198,8 +200,8 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
       const int w_rows = p.n_pass / CL;                     // this CTA's slice of the W tile (multiple of 8 rows)
       for (int64_t item = first_item; item < n_items; item += item_step) {
         const int row0 = int(((item / p.passes) * CL + rank) * BM), col0 = int(item % p.passes) * p.n_pass;
-        for (int seg = 0; seg < p.k_segs; ++seg) {          // segment 1 reads g_lo, segment 2 reads W_lo
-          const CUtensorMap *mg = seg == 1 ? &map_g2 : &map_g, *mw = seg == 2 ? &map_w2 : &map_w;
+        for (int seg = 0; seg < p.k_segs; ++seg) {
+          const CUtensorMap *mg = (p.seg_g2 >> seg) & 1 ? &map_g2 : &map_g, *mw = (p.seg_w2 >> seg) & 1 ? &map_w2 : &map_w;
           for (int kc = 0; kc < p.k_chunks; ++kc) {
             mbar_wait(&empty_bar[stage], phase ^ 1);        // this slot is free in EVERY CTA of the cluster
             unsigned char *sa = smem + stage * p.stage_bytes, *sb = sa + A_BYTES;
@@ -239,7 +241,7 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
     }
   } else {
     // ===== epilogue: warps 2..5 own TMEM lanes 32*(warp%4) .. +31; overlaps the next item's MMAs =====
-    // d <- d_scale d + acc (or u <- acc) in tiles of [32 rows x 32 columns], each warp on its own ring of
+    // d <- d_scale d + acc in tiles of [32 rows x 32 columns], each warp on its own ring of
     // EBUF staging tiles: TMA load (128B swizzle) -> every lane updates ITS row in shared memory
     // (conflict-free thanks to the swizzle) -> TMA store.  All global traffic of the epilogue is
     // full 128-byte rows moved by the TMA unit; a row-per-lane LDG/STG pattern (32 lines per warp
@@ -247,7 +249,6 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
     const int lane_base = (warp & 3) * 32;
     unsigned char *ebuf = smem + p.stages * p.stage_bytes + (warp & 3) * (EBUF * 4096);
     uint64_t *efull = &epi_full[(warp & 3) * EBUF];
-    const bool rmw = p.U == nullptr;
     const int n_chunks = (p.n_pass + 31) / 32;
     uint32_t g = 0;                                         // tiles this warp has processed (ring position)
     uint32_t li = 0;
@@ -262,12 +263,12 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
         mbar_expect_tx(&efull[b], 4096);
         tma_load_2d(ebuf + b * 4096, &map_d, col0 + 32 * c, row0w, &efull[b]);
       };
-      if (rmw && lane == 0) issue_load(0, g);               // requested before the accumulator is awaited
+      if (lane == 0) issue_load(0, g);                      // requested before the accumulator is awaited
       mbar_wait(&tmem_full_bar[acc], acc_phase);
       asm volatile("tcgen05.fence::after_thread_sync;");
       for (int c = 0; c < n_chunks; ++c) {
         const uint32_t gc = g + uint32_t(c), b = gc % EBUF;
-        if (rmw && lane == 0 && c + 1 < n_chunks) issue_load(c + 1, gc + 1);   // tile gc-2's store may still run
+        if (lane == 0 && c + 1 < n_chunks) issue_load(c + 1, gc + 1);   // tile gc-2's store may still run
         uint32_t r[32];
         {
           uint32_t r0[16], r1[16];
@@ -277,17 +278,12 @@ global_tcgen05_kernel(const __grid_constant__ CUtensorMap map_g, const __grid_co
 #pragma unroll
           for (int q = 0; q < 16; ++q) { r[q] = r0[q]; r[16 + q] = r1[q]; }
         }
-        if (rmw) {
-          mbar_wait(&efull[b], (gc / EBUF) & 1u);
-        } else {
-          if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 2;" ::: "memory");
-          __syncwarp();
-        }
+        mbar_wait(&efull[b], (gc / EBUF) & 1u);
         float4 *rowp = reinterpret_cast<float4 *>(ebuf + b * 4096 + lane * 128);
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
           float4 *slot = rowp + (q ^ (lane & 7));           // 128B swizzle: 16-byte chunk q of row r sits at q ^ (r % 8)
-          float4 v = rmw ? *slot : make_float4(0.f, 0.f, 0.f, 0.f);
+          float4 v = *slot;
           v.x = fmaf(p.d_scale, v.x, __uint_as_float(r[4 * q]));
           v.y = fmaf(p.d_scale, v.y, __uint_as_float(r[4 * q + 1]));
           v.z = fmaf(p.d_scale, v.z, __uint_as_float(r[4 * q + 2]));
@@ -356,7 +352,10 @@ static bool gemm_shape(const TypeDev &td, GemmParams &p) {
   p.n_pass = ((td.n_pad + p.passes - 1) / p.passes + gran - 1) / gran * gran;
   if (p.n_pass > MAX_NPASS || p.n_pass < 16 || (p.n_pass / CL) % 8 != 0 || td.Hinv == nullptr) return false;
   p.k_chunks = (td.n_pad + BK - 1) / BK;
-  return true;
+  p.stage_bytes = A_BYTES + (p.n_pass * BK * 4 + 1023) / 1024 * 1024;
+  p.stages = (SMEM_LIMIT - 1024 - EPI_BYTES) / p.stage_bytes;
+  if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;
+  return p.stages >= 2;
 }
 
 bool global_tcgen05_supported(const TypeDev &td) {
@@ -364,44 +363,46 @@ bool global_tcgen05_supported(const TypeDev &td) {
   return gemm_shape(td, p) && get_encode() != nullptr;
 }
 
-// d <- d_scale d - g Hinv (u_out == nullptr) or u_out <- -g Hinv.  Returns #launches, or -1 if the
-// configuration is unsupported (caller falls back to the SIMT GEMM).
-// g_lo / w_lo (both or neither): the line search's 3xTF32 product d <- d_scale d - (g W + g_lo W + g W_lo) as ONE
+// d <- d_scale d - g Hinv.  Returns #launches, -1 if the shape is unsupported (npfem_step decides BEFORE launching
+// which GEMM a bucket takes: global_tcgen05_supported), -2 if the launch itself failed (an NPFEM_ECUDA for the
+// caller, never a silent fall back to the SIMT GEMM).
+// w_lo alone: d <- d_scale d - (g W + g W_lo) (split operator).  g_lo and w_lo: the line search's 3xTF32 product d <- d_scale d - (g W + g_lo W + g W_lo) as ONE
 // GEMM with the three products concatenated along K (g = bv.field[F_G] holds the TF32 high part, W = Hinv_tf32).
-int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, double d_scale, void *u_out,
+int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, double d_scale,
                           cudaStream_t s, const void *g_lo, const void *w_lo) {
   if (bv.cells == 0) return 0;
   GemmParams p{};
   if (!gemm_shape(td, p)) return -1;
   p.D = static_cast<float *>(bv.field[F_D]);
-  p.U = static_cast<float *>(u_out);
   p.rows = bv.cells * 3;
   p.m_tiles = (p.rows + BM - 1) / BM;
   p.d_scale = float(d_scale);
   CUtensorMap map_g, map_w, map_d;
-  if (!make_map(&map_g, bv.field[F_G], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), BM)) return -1;
+  if (!make_map(&map_g, bv.field[F_G], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), BM)) return -2;
   if (!make_map(&map_w, td.Hinv_tf32 ? td.Hinv_tf32 : td.Hinv, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n_pass / CL)))
-    return -1;
+    return -2;
   CUtensorMap map_g2 = map_g, map_w2 = map_w;
   p.k_segs = 1;
-  if (g_lo && w_lo) {
-    if (!make_map(&map_g2, g_lo, uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), BM)) return -1;
-    if (!make_map(&map_w2, w_lo, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n_pass / CL))) return -1;
-    p.k_segs = 3;
+  p.seg_g2 = p.seg_w2 = 0;
+  if (w_lo) {
+    if (!make_map(&map_w2, w_lo, uint64_t(td.n_pad), uint64_t(td.n_pad), uint64_t(td.n_pad), uint32_t(p.n_pass / CL))) return -2;
+    if (g_lo) {          // (g_hi, W_hi), (g_lo, W_hi), (g_hi, W_lo)
+      if (!make_map(&map_g2, g_lo, uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), BM)) return -2;
+      p.k_segs = 3;
+      p.seg_g2 = 0b010;
+      p.seg_w2 = 0b100;
+    } else {             // (g, W_hi), (g, W_lo)
+      p.k_segs = 2;
+      p.seg_w2 = 0b010;
+    }
   }
-  // epilogue tiles: [32 rows][32 columns] of D (in-place update) or of U (product out)
-  if (!make_map(&map_d, u_out ? u_out : bv.field[F_D], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), 32))
-    return -1;
-  p.stage_bytes = A_BYTES + (p.n_pass * BK * 4 + 1023) / 1024 * 1024;
-  p.stages = (SMEM_LIMIT - 1024 - EPI_BYTES) / p.stage_bytes;
-  if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;
-  if (p.stages < 2) return -1;
+  // epilogue tiles: [32 rows][32 columns] of D (in-place update)
+  if (!make_map(&map_d, bv.field[F_D], uint64_t(p.rows), uint64_t(td.n_pad), uint64_t(td.n_pad), 32))
+    return -2;
   const int smem_bytes = p.stages * p.stage_bytes + EPI_BYTES + 1024;
-  static int smem_set = 0;
-  if (smem_bytes > smem_set) {
-    if (cudaFuncSetAttribute(global_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes) != cudaSuccess)
-      return -1;
-    smem_set = smem_bytes;
+  if (td.cache.tc_smem == 0) {   // per context and type: the attribute is per device (always the architectural maximum)
+    if (opt_in_max_dynamic_smem(global_tcgen05_kernel) != cudaSuccess) return -2;
+    td.cache.tc_smem = smem_bytes;
   }
   // the passes of one group of M tiles are adjacent items: they run on neighbouring clusters at about
   // the same time, so the repeated reads of the G tiles are L2 hits
@@ -419,7 +420,7 @@ int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, dou
   attrs[0].val.clusterDim.z = 1;
   cfg.attrs = attrs;
   cfg.numAttrs = 1;
-  if (cudaLaunchKernelEx(&cfg, global_tcgen05_kernel, map_g, map_w, map_d, map_g2, map_w2, p) != cudaSuccess) return -1;
+  if (cudaLaunchKernelEx(&cfg, global_tcgen05_kernel, map_g, map_w, map_d, map_g2, map_w2, p) != cudaSuccess) return -2;
   return 1;
 }
 

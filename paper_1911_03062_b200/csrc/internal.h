@@ -13,7 +13,11 @@
 namespace npfem {
 
 // Number of state fields kept per bucket, each [cells][3][n_pad] of the compute type.
-enum Field { F_X = 0, F_V, F_F, F_B, F_D, F_G, F_U, F_COUNT };   // F_U: raw product of the last global step
+// F_XL: fp32 contexts only (null in fp64 contexts): low part of the positions.  The cell-local position of a vertex
+//       is the unevaluated sum x + xl with |xl| <= ulp(x)/2 (two-float storage): the epilogue
+//       adds d to it with a compensated sum, so the rounding of x_{n+1} = x_n + d to fp32 does not accumulate in the
+//       state over the steps, and the local step evaluates grad E at x + (xl + d)
+enum Field { F_X = 0, F_V, F_F, F_B, F_D, F_G, F_XL, F_COUNT };
 
 // Device tables of the scheduled fp32 local step (local_schedule.hpp / local_sched.cu).
 struct SchedDev {
@@ -24,6 +28,28 @@ struct SchedDev {
   const uint32_t *vtx_words = nullptr;
   const float *vtx_coef = nullptr;
   double vol_lane_bound = 0;   // max over threads of sum_j |x0| 2A_t of the rest shape (6V partial per lane)
+};
+
+// Per-context launch state of the kernels that opt in to more than 48 KB of dynamic shared memory: the attribute
+// is per device and function, the occupancy depends on it, so both are cached per context and cell type (a
+// process-wide static would be wrong for two devices in one process).
+// Opt a kernel in to the largest dynamic shared-memory size the SM allows next to its static shared memory
+// (227 KB per CTA in all).  Always the maximum, never the size of the launch at hand: the attribute belongs to the
+// function on the device, and two cell types (or two contexts) sharing a kernel must not lower each other's limit.
+template <typename K>
+inline cudaError_t opt_in_max_dynamic_smem(K kernel) {
+  cudaFuncAttributes fa;
+  cudaError_t e = cudaFuncGetAttributes(&fa, kernel);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - int(fa.sharedSizeBytes));
+}
+
+struct KernelCache {
+  size_t sched_smem = 0;
+  int sched_per_sm = 0;
+  int tc_smem = 0;
+  bool generic_attr[2] = {false, false}, smem_attr = false, big_attr = false, fused_attr = false, objective_attr = false,
+       damping_attr = false;
 };
 
 // Device view of one cell type (pointers into the workspace; element type = compute type).
@@ -39,7 +65,8 @@ struct TypeDev {
   const void *vtx_mass = nullptr;    // [n]  m_v
   const void *vtx_inv_area = nullptr;// [n]  1/A_v
   const void *Hinv = nullptr;        // [n_pad][n_pad] dense inverse of H~ (compute type)
-  const void *Hinv_tf32 = nullptr;
+  const void *Hinv_tf32 = nullptr;   // fp32 contexts: H~^-1 rounded to TF32 to nearest (the tensor-core operand W_hi)
+  const void *Hinv_lo = nullptr;     // fp32 contexts: W_lo = tf32(H~^-1 - W_hi), the second term of the split operator
   // fp32 shared-memory local step (local_smem.cu)
   const void *tri_pack = nullptr;    // [T] uint4: v0|v1<<16, v2|n0<<16, n1|n2<<16, 0
   const void *vtx_pack = nullptr;    // [n] uint4: 8 x u16 corner ids (3T = none)
@@ -50,6 +77,7 @@ struct TypeDev {
   double inertia_coef = 0;           // (1 + h alpha) / h^2, multiplies m_v
   double kappa = 0;
   SchedDev sched;                    // fp32 contexts: scheduled local step (may be invalid)
+  mutable KernelCache cache;
 };
 
 // One bucket = all cells of one type, contiguous slots.
@@ -70,7 +98,9 @@ struct CellRef {
 };
 
 // ---- launchers (each enqueues on `stream`, returns the number of kernels launched or <0) -------
-int launch_invert_spd(const double *H_dev, double *Hinv_dev, int n, cudaStream_t stream,
+// tmp: device scratch of invert_spd_tmp_doubles(n) doubles (from the workspace: the library allocates nothing here)
+size_t invert_spd_tmp_doubles(int n);
+int launch_invert_spd(const double *H_dev, double *Hinv_dev, int n, double *tmp, cudaStream_t stream,
                       double *residual_out, std::string &err);
 
 int launch_convert_pad(const double *X, int n, void *out, int n_pad, int precision, cudaStream_t s);
@@ -111,14 +141,14 @@ int launch_set_forces(const BucketView *views_dev, const PackArgs &a, int precis
 int launch_get_state(const BucketView *views_dev, const PackArgs &a, int precision, cudaStream_t s);
 
 int launch_prologue(const TypeDev &td, const BucketView &bv, int precision, cudaStream_t s);
-// pending: d <- d_scale d + u still has to be applied (fused-update mode, see npfem_step)
-int launch_epilogue(const TypeDev &td, const BucketView &bv, int precision, bool pending, double d_scale,
-                    double v_max, cudaStream_t s);
+int launch_epilogue(const TypeDev &td, const BucketView &bv, int precision, double v_max, cudaStream_t s);
 
-// PIK collision term (coupling.cu): per bucket, targets [cells][3][n_pad] in cell-local coordinates and
-// stiffness [cells][n_pad] (0 = vertex not in contact), compute type
+// PIK collision term (coupling.cu): per bucket, targets [cells][3][n_pad] in GLOBAL coordinates, fp64 (the origin of
+// a cell's local frame moves when the prologue re-centres it or set_state is called again; global targets stay
+// valid), and stiffness [cells][n_pad] (0 = vertex not in contact), compute type
 struct CollisionDev {
-  void *targets = nullptr, *stiffness = nullptr;
+  double *targets = nullptr;
+  void *stiffness = nullptr;
 };
 int launch_set_collisions(const BucketView *views_dev, const CollisionDev *cols_dev, const PackArgs &a, int precision,
                           cudaStream_t s);   // a.src_a = targets, a.src_b = stiffness
@@ -142,10 +172,10 @@ int launch_objective(const TypeDev &td, const BucketView &bv, const int64_t *cel
 struct LineSearchDev {
   double *obj0 = nullptr, *obj1 = nullptr, *slope = nullptr, *alpha = nullptr;   // [cells]
   int *done = nullptr;                                                            // [cells]
+  void *d_old = nullptr;                                                          // [cells][3][n_pad] d before the global step
   // fp32 contexts whose global step runs on the TF32 tensor cores: the search direction comes from a 3xTF32
   // product (g = g_hi + g_lo, H~^-1 = W_hi + W_lo, the lo x lo term dropped), see launch_ls_split_g
   float *g_lo = nullptr;                                                          // [cells][3][n_pad]
-  float *w_lo = nullptr;                                                          // [n_pad][n_pad]
 };
 // g <- tf32(g), g_lo <- tf32(g - tf32(g)) over count elements; w_lo <- tf32(w - w_hi)
 int launch_ls_split_g(float *g, float *g_lo, size_t count, cudaStream_t s);
@@ -164,8 +194,9 @@ int launch_ls_accept(const BucketView &bv, const LineSearchDev &ls, double c1, b
 int launch_global_simt(const TypeDev &td, const BucketView &bv, int precision, double d_scale, cudaStream_t s);
 // fp32 contexts, TF32 tensor cores (tcgen05); returns -1 when the shape is unsupported
 bool global_tcgen05_supported(const TypeDev &td);
-// u_out == nullptr: d <- d_scale d - g Hinv;  else u_out <- -g Hinv (the next local step / the epilogue applies it)
-int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, double d_scale, void *u_out,
+// d <- d_scale d - g Hinv.  Returns -1 for an unsupported shape, -2 when the launch itself failed (the CUDA error
+// is left for the caller's cudaGetLastError: a failed tensor-core launch is an error, never a silent SIMT fallback)
+int launch_global_tcgen05(const TypeDev &td, const BucketView &bv, int n_sm, double d_scale,
                           cudaStream_t s, const void *g_lo = nullptr, const void *w_lo = nullptr);
 
 // fp32 fast local step; writes the reduced gradient (global step must then use d_scale = 1 - gamma)
@@ -175,9 +206,7 @@ int launch_local_smem(const TypeDev &td, const BucketView &bv, int n_sm, cudaStr
 // fp32 scheduled local step (register-resident topology, conflict-free shared-memory slots); same
 // reduced-gradient convention as launch_local_smem
 bool local_sched_supported(const TypeDev &td);
-// apply_u: first d <- d_scale d + u (pending update of the previous global step), stored back to d
-int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, bool apply_u, double d_scale,
-                       cudaStream_t s);
+int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
 
 // fp32 reduced-gradient local step for types too large for the scheduled kernel (chunked corner forces)
 bool local_big_supported(const TypeDev &td);

@@ -119,8 +119,11 @@ int launch_convert_pad(const double *X, int n, void *out, int n_pad, int precisi
   return 1;
 }
 
-// H_dev, Hinv_dev: device [n][n] fp64.  Synchronises the stream (setup path, called once per type).
-int launch_invert_spd(const double *H_dev, double *Hinv_dev, int n, cudaStream_t stream,
+// H_dev, Hinv_dev: device [n][n] fp64; tmp: invert_spd_tmp_doubles(n) doubles of device scratch.
+// Synchronises the stream (setup path, called once per type).
+size_t invert_spd_tmp_doubles(int n) { return size_t(3) * n * n + 32; }
+
+int launch_invert_spd(const double *H_dev, double *Hinv_dev, int n, double *tmp, cudaStream_t stream,
                       double *residual_out, std::string &err) {
   int launches = 0;
   const size_t bytes = size_t(n) * n * sizeof(double);
@@ -141,12 +144,11 @@ int launch_invert_spd(const double *H_dev, double *Hinv_dev, int n, cudaStream_t
       return -1;
     }
   }
-  if (cudaMalloc(&X, bytes) != cudaSuccess || cudaMalloc(&P, bytes) != cudaSuccess ||
-      cudaMalloc(&Y, bytes) != cudaSuccess || cudaMalloc(&res_dev, sizeof(double)) != cudaSuccess) {
-    cudaFree(X); cudaFree(P); cudaFree(Y); cudaFree(res_dev);
-    err = "inverse: out of device memory for the Newton-Schulz temporaries";
-    return -2;
-  }
+  // Newton-Schulz temporaries from the caller's scratch (workspace): no allocation here
+  X = tmp;
+  P = X + size_t(n) * n;
+  Y = P + size_t(n) * n;
+  res_dev = Y + size_t(n) * n;
   const dim3 grid((n + BN - 1) / BN, (n + BM - 1) / BM);
   const int eb = 256, eg = int((size_t(n) * n + eb - 1) / eb);
   init_scaled_identity_kernel<<<eg, eb, 0, stream>>>(X, n, 1.0 / norm_inf);
@@ -177,7 +179,6 @@ int launch_invert_spd(const double *H_dev, double *Hinv_dev, int n, cudaStream_t
     ++launches;
   }
   const cudaError_t e = cudaStreamSynchronize(stream);
-  cudaFree(X); cudaFree(P); cudaFree(Y); cudaFree(res_dev);
   if (residual_out) *residual_out = res;
   if (e != cudaSuccess) {
     err = std::string("inverse: CUDA failure: ") + cudaGetErrorString(e);

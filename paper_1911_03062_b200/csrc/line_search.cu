@@ -38,7 +38,7 @@ ls_init_kernel(BucketView bv, LineSearchDev ls, double grad_tol) {
     const size_t base = size_t(cell) * 3 * bv.n_pad;
     V *g = reinterpret_cast<V *>(static_cast<T *>(bv.field[F_G]) + base);
     V *d = reinterpret_cast<V *>(static_cast<T *>(bv.field[F_D]) + base);
-    const V *d_old = reinterpret_cast<const V *>(static_cast<const T *>(bv.field[F_U]) + base);
+    const V *d_old = reinterpret_cast<const V *>(static_cast<const T *>(ls.d_old) + base);
     const V *b = reinterpret_cast<const V *>(static_cast<const T *>(bv.field[F_B]) + base);
     const float4 *g_lo = ls.g_lo ? reinterpret_cast<const float4 *>(ls.g_lo + base) : nullptr;   // 3xTF32 mode: gradient = g + g_lo
     double slope = 0.0, gg = 0.0, bb = 0.0;
@@ -99,7 +99,7 @@ ls_accept_kernel(BucketView bv, LineSearchDev ls, double c1, int last) {
     const size_t base = size_t(cell) * 3 * n_pad;
     const T *p = static_cast<const T *>(bv.field[F_G]) + base;
     T *d = static_cast<T *>(bv.field[F_D]) + base;
-    const T *d_old = static_cast<const T *>(bv.field[F_U]) + base;
+    const T *d_old = static_cast<const T *>(ls.d_old) + base;
     for (int k = 0; k < 3; ++k)
       for (int i = lane; i < n; i += 32) {
         const int o = k * n_pad + i;
@@ -211,7 +211,8 @@ int launch_damping_grad(const TypeDev &td, const BucketView &bv, float *g_lo, in
   p.cells = bv.cells;
   const size_t smem = sizeof(float) * 6 * size_t(td.n);
   if (smem > 200 * 1024) return -1;
-  cudaFuncSetAttribute(damping_grad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (!td.cache.damping_attr) cudaFuncSetAttribute(damping_grad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  td.cache.damping_attr = true;
   const int64_t cap = int64_t(n_sm) * 8 * 2;
   damping_grad_kernel<<<unsigned(bv.cells < cap ? bv.cells : cap), 256, smem, s>>>(p);
   return 1;

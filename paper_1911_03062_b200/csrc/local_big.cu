@@ -29,7 +29,7 @@ struct BigParams {
   const float *vtx_coef;      // [n]  (1 - gamma)(1 + h alpha) m_v / h^2
   float B4, C4, k_b;
   double kv_over_V0, V0;
-  const float *x, *d, *b;     // [cells][3][n_pad]
+  const float *x, *xl, *d, *b;   // [cells][3][n_pad]; positions are the two-float sum x + xl (internal.h F_XL)
   float *g;
   int g_tf32;
   int64_t cells;
@@ -52,19 +52,20 @@ __global__ void __launch_bounds__(THREADS, 1) local_big_kernel(const BigParams p
 
   for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x) {
     const size_t base = size_t(cell) * 3 * n_pad;
-    const float *xg = p.x + base, *dg = p.d + base, *bg = p.b + base;
+    const float *xg = p.x + base, *lg = p.xl + base, *dg = p.d + base, *bg = p.b + base;
     {   // pull the NEXT cell's x, d, b towards L2 while this one is computed (one 128-byte line per thread)
       const int64_t nxt = cell + gridDim.x;
       const int lines = (3 * n_pad * 4 + 127) / 128;
       if (nxt < p.cells)
-        for (int l = tid; l < 3 * lines; l += THREADS) {
-          const float *f = (l < lines ? p.x : (l < 2 * lines ? p.d : p.b)) + size_t(nxt) * 3 * n_pad;
+        for (int l = tid; l < 4 * lines; l += THREADS) {
+          const float *f = (l < lines ? p.x : (l < 2 * lines ? p.d : (l < 3 * lines ? p.b : p.xl))) + size_t(nxt) * 3 * n_pad;
           asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(f) + size_t(l % lines) * 128));
         }
     }
     // ---- phase 0 ----------------------------------------------------------------------------
     for (int i = tid; i < n; i += THREADS)
-      sx[i] = make_float4(xg[i] + dg[i], xg[n_pad + i] + dg[n_pad + i], xg[2 * n_pad + i] + dg[2 * n_pad + i], 0.f);
+      sx[i] = make_float4(xg[i] + (lg[i] + dg[i]), xg[n_pad + i] + (lg[n_pad + i] + dg[n_pad + i]),
+                          xg[2 * n_pad + i] + (lg[2 * n_pad + i] + dg[2 * n_pad + i]), 0.f);   // two-float x_n (F_XL)
     __syncthreads();
     // ---- phase A: unit normals, volume --------------------------------------------------------
     float vol = 0.f;
@@ -233,16 +234,16 @@ int launch_local_big(const TypeDev &td, const BucketView &bv, int n_sm, cudaStre
   p.B4 = float(td.B4); p.C4 = float(td.C4); p.k_b = float(td.k_b);
   p.kv_over_V0 = td.kv_over_V0; p.V0 = td.V0;
   p.x = static_cast<const float *>(bv.field[F_X]);
+  p.xl = static_cast<const float *>(bv.field[F_XL]);
   p.d = static_cast<const float *>(bv.field[F_D]);
   p.b = static_cast<const float *>(bv.field[F_B]);
   p.g = static_cast<float *>(bv.field[F_G]);
   p.g_tf32 = bv.g_tf32;
   p.cells = bv.cells;
   const size_t smem = size_t(td.n) * 16 + size_t(td.T) * 16 + size_t(3) * p.tc * 16;
-  static size_t smem_set = 0;
-  if (smem > smem_set) {
-    if (cudaFuncSetAttribute(local_big_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) return -1;
-    smem_set = smem;
+  if (!td.cache.big_attr) {   // per context (the attribute is per device): always the architectural maximum
+    if (opt_in_max_dynamic_smem(local_big_kernel) != cudaSuccess) return -1;
+    td.cache.big_attr = true;
   }
   const int64_t grid = bv.cells < n_sm ? bv.cells : n_sm;
   local_big_kernel<<<unsigned(grid), THREADS, smem, s>>>(p);

@@ -28,7 +28,7 @@ struct LocalParams {
   const int *vtx_corner, *vtx_nbr;
   const T *vtx_w, *vtx_mass, *vtx_inv_area;
   T B4, C4, k_b, kv_over_V0, V0, k_mem, beta_over_h, inertia_coef;
-  const T *x, *d, *b;
+  const T *x, *xl, *d, *b;   // xl: low part of the two-float positions of fp32 contexts (internal.h F_XL), else null
   T *g;
   int64_t cells;
   T *scratch;          // global scratch per CTA when the working set does not fit in shared memory:
@@ -79,7 +79,7 @@ local_generic_kernel(const LocalParams<T> p) {
     for (int k = 0; k < 3; ++k)
       for (int i = threadIdx.x; i < n; i += blockDim.x) {
         const T dd = p.d[base + k * n_pad + i];
-        sx[k * n + i] = p.x[base + k * n_pad + i] + dd;
+        sx[k * n + i] = p.x[base + k * n_pad + i] + (p.xl ? p.xl[base + k * n_pad + i] + dd : dd);
         sd[k * n + i] = dd;
       }
     __syncthreads();
@@ -229,7 +229,9 @@ objective_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_id, do
   for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x) {
     if (skip && skip[cell]) continue;
     const size_t base = size_t(cell) * 3 * n_pad;
-    auto pos = [&](int v, int k) { return double(p.x[base + k * n_pad + v]) + double(p.d[base + k * n_pad + v]); };
+    auto pos = [&](int v, int k) {
+      return double(p.x[base + k * n_pad + v]) + ((p.xl ? double(p.xl[base + k * n_pad + v]) : 0.0) + double(p.d[base + k * n_pad + v]));
+    };
     double acc = 0.0, vol = 0.0;
     for (int t = threadIdx.x; t < nt; t += blockDim.x) {
       const int4 tv = p.tri[t];
@@ -335,7 +337,8 @@ objective_smem_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_i
     const size_t base = size_t(cell) * 3 * n_pad;
     for (int k = 0; k < 3; ++k)
       for (int i = threadIdx.x; i < n; i += NT)
-        sp[k * n + i] = double(p.x[base + k * n_pad + i]) + double(p.d[base + k * n_pad + i]);
+        sp[k * n + i] = double(p.x[base + k * n_pad + i]) +
+                        ((p.xl ? double(p.xl[base + k * n_pad + i]) : 0.0) + double(p.d[base + k * n_pad + i]));
     __syncthreads();
     double acc = 0.0, vol = 0.0;
     for (int t = threadIdx.x; t < nt; t += NT) {
@@ -429,6 +432,7 @@ LocalParams<T> make_params(const TypeDev &td, const BucketView &bv) {
   p.B4 = T(td.B4); p.C4 = T(td.C4); p.k_b = T(td.k_b); p.kv_over_V0 = T(td.kv_over_V0); p.V0 = T(td.V0);
   p.k_mem = T(td.k_mem); p.beta_over_h = T(td.beta_over_h); p.inertia_coef = T(td.inertia_coef);
   p.x = static_cast<const T *>(bv.field[F_X]);
+  p.xl = static_cast<const T *>(bv.field[F_XL]);
   p.d = static_cast<const T *>(bv.field[F_D]);
   p.b = static_cast<const T *>(bv.field[F_B]);
   p.g = static_cast<T *>(bv.field[F_G]);
@@ -459,11 +463,11 @@ int launch_local_T(const TypeDev &td, const BucketView &bv, void *scratch, int n
       p.scratch_in_smem = -1;
     }
   }
-  static bool attr_set[2] = {false, false};
-  if (!attr_set[sizeof(T) == 8]) {
-    cudaFuncSetAttribute(local_generic_kernel<T, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kMaxSmem));
-    cudaFuncSetAttribute(local_generic_kernel<T, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kMaxSmem));
-    attr_set[sizeof(T) == 8] = true;
+  if (!td.cache.generic_attr[sizeof(T) == 8]) {   // per context and type (the attribute is per device)
+    if (cudaFuncSetAttribute(local_generic_kernel<T, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kMaxSmem)) != cudaSuccess ||
+        cudaFuncSetAttribute(local_generic_kernel<T, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kMaxSmem)) != cudaSuccess)
+      return -1;
+    td.cache.generic_attr[sizeof(T) == 8] = true;
   }
   const int per_sm = smem * 2 + 4096 <= 227 * 1024 ? 2 : 1;
   int64_t grid = int64_t(n_sm) * per_sm;
@@ -499,11 +503,13 @@ int launch_objective_T(const TypeDev &td, const BucketView &bv, const int64_t *c
   const LocalParams<T> p = make_params<T>(td, bv);
   const size_t smem = sizeof(double) * (size_t(3) * td.n + size_t(3) * td.T);
   if (smem <= 56 * 1024) {                    // 4 CTAs of 256 threads per SM (RBC-642: 46 KB each)
-    cudaFuncSetAttribute(objective_smem_kernel<T, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 56 * 1024);
+    if (!td.cache.objective_attr) cudaFuncSetAttribute(objective_smem_kernel<T, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 56 * 1024);
+    td.cache.objective_attr = true;
     const int64_t cap = int64_t(n_sm) * 4 * 4;
     objective_smem_kernel<T, 256><<<unsigned(bv.cells < cap ? bv.cells : cap), 256, smem, s>>>(p, cell_id_dev, objective_row, skip_dev);
   } else if (smem <= kMaxSmem) {              // one CTA of 1024 threads per SM (RBC-2562: 184 KB)
-    cudaFuncSetAttribute(objective_smem_kernel<T, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kMaxSmem));
+    if (!td.cache.objective_attr) cudaFuncSetAttribute(objective_smem_kernel<T, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kMaxSmem));
+    td.cache.objective_attr = true;
     const int64_t cap = int64_t(n_sm) * 4;
     objective_smem_kernel<T, 1024><<<unsigned(bv.cells < cap ? bv.cells : cap), 1024, smem, s>>>(p, cell_id_dev, objective_row, skip_dev);
   } else {

@@ -43,12 +43,9 @@ struct SchedParams {
   float fx_scale;              // per-lane 6V partials are reduced as integers in units of 1 / fx_scale
   long long fx_rest;           // round(6 V0 fx_scale)
   float vc_scale;              // k_v / (36 V0) / fx_scale:  vc = vc_scale (6V - 6V0)_fixed = k_v (V - V0)/V0 / 6
-  const float *x, *b, *u;      // [cells][3][n_pad]
-  float *d;                    // read; written back when apply_u
+  const float *x, *xl, *d, *b; // [cells][3][n_pad]; the position of a vertex is x + xl (two-float, internal.h F_XL)
   float *g;
   int g_tf32;                  // round g to TF32 (its consumer is the tensor-core GEMM)
-  int apply_u;                 // first d <- d_scale d + u (pending update of the last global step)
-  float d_scale;
   int64_t cells;
 };
 
@@ -86,7 +83,7 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
   unsigned char *sx = smem;
   unsigned char *sN = sx + p.sx_bytes;
   unsigned char *sC = sN + p.sN_bytes;
-  float *stage = reinterpret_cast<float *>(sC + p.sC_bytes);            // [NSTAGE][4 fields x, d, b, u][3][n_pad]
+  float *stage = reinterpret_cast<float *>(sC + p.sC_bytes);            // [NSTAGE][4 fields x, d, b, xl][3][n_pad]
   int *vacc = reinterpret_cast<int *>(stage + NSTAGE * 12 * n_pad);   // [2 cells][hi, lo] base-2^12 digits of 6V (fixed point)
   uint64_t *mbar = reinterpret_cast<uint64_t *>(vacc + 4);   // [NSTAGE] TMA ring
   uint64_t *bars = mbar + NSTAGE;                              // [4] split block barriers B1, B2, B3, BV
@@ -121,17 +118,16 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
   const int v2c = tid + 64;
   const bool vact2c = tid >= nthreads - 64 && tid < nthreads - 32 && v2c < n;
 
-  auto prefetch = [&](int64_t cell, int st) {   // one thread: arm the barrier, start 3 bulk copies
+  auto prefetch = [&](int64_t cell, int st) {   // one thread: arm the barrier, start 4 bulk copies
     const size_t base = size_t(cell) * 3 * n_pad;
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar + st)),
-                 "r"((p.apply_u ? 4u : 3u) * field_bytes) : "memory");
-    const float *src[4] = {p.x + base, p.d + base, p.b + base, p.u + base};
+                 "r"(4u * field_bytes) : "memory");
+    const float *src[4] = {p.x + base, p.d + base, p.b + base, p.xl + base};
 #pragma unroll
     for (int f = 0; f < 4; ++f)
-      if (f < 3 || p.apply_u)
-        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                     ::"r"(smem_u32(stage + (st * 12 + f * 3) * n_pad)), "l"(src[f]), "r"(field_bytes),
-                       "r"(smem_u32(mbar + st)) : "memory");
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                   ::"r"(smem_u32(stage + (st * 12 + f * 3) * n_pad)), "l"(src[f]), "r"(field_bytes),
+                     "r"(smem_u32(mbar + st)) : "memory");
   };
 
   if (tid == 0) {
@@ -167,26 +163,16 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
           : "=r"(done) : "r"(smem_u32(bars + which)), "r"(parity) : "memory");
     } while (!done);
   };
-  // phase 0 of this CTA's it0-th cell (ring slot it0 % NSTAGE): apply the pending update
-  // d <- d_scale d + u (kept in the ring slot for phase C, written back to global d), then
-  // sx[slot(v)] = (x_n + d, 0)
-  auto phase0_vertex = [&](float *sg, float *dglob, int v, uint32_t slot_off) {
-    float dv[3];
-#pragma unroll
-    for (int k = 0; k < 3; ++k) dv[k] = sg[(3 + k) * n_pad + v];
-    if (p.apply_u) {
-#pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        dv[k] = fmaf(p.d_scale, dv[k], sg[(9 + k) * n_pad + v]);
-        sg[(3 + k) * n_pad + v] = dv[k];
-        dglob[k * n_pad + v] = dv[k];
-      }
-    }
-    sts4(sx, slot_off, sg[v] + dv[0], sg[n_pad + v] + dv[1], sg[2 * n_pad + v] + dv[2], 0.f);
+  // phase 0 of this CTA's it0-th cell (ring slot it0 % NSTAGE): sx[slot(v)] = (x + (xl + d), 0), the current
+  // position from the two-float x_n = x + xl
+  auto phase0_vertex = [&](const float *sg, int v, uint32_t slot_off) {
+    sts4(sx, slot_off, sg[v] + (sg[9 * n_pad + v] + sg[3 * n_pad + v]),
+         sg[n_pad + v] + (sg[10 * n_pad + v] + sg[4 * n_pad + v]),
+         sg[2 * n_pad + v] + (sg[11 * n_pad + v] + sg[5 * n_pad + v]), 0.f);
   };
-  auto phase0 = [&](int it0, int64_t cell0) {
+  auto phase0 = [&](int it0) {
     const int st = it0 % NSTAGE;
-    float *sg = stage + st * 12 * n_pad;
+    const float *sg = stage + st * 12 * n_pad;
     const uint32_t parity = uint32_t(it0 / NSTAGE) & 1u;
     uint32_t done;
     do {
@@ -194,9 +180,45 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
           "{\n.reg .pred q;\nmbarrier.try_wait.parity.shared::cta.b64 q, [%1], %2;\nselp.u32 %0, 1, 0, q;\n}\n"
           : "=r"(done) : "r"(smem_u32(mbar + st)), "r"(parity) : "memory");
     } while (!done);
-    float *dglob = p.d + size_t(cell0) * 3 * n_pad;
-    if (vact) phase0_vertex(sg, dglob, tid, lo16(vw[0]));
-    if (vact2) phase0_vertex(sg, dglob, v2, p.vtx_words[v2] & 0xffffu);
+    if (vact) phase0_vertex(sg, tid, lo16(vw[0]));
+    if (vact2) phase0_vertex(sg, v2, p.vtx_words[v2] & 0xffffu);
+  };
+
+  // ---- phase C of one cell: r = coef d - b + sum of the vertex's corner forces -> global ---------------
+  auto phaseC = [&](int64_t cell, const float *sg) {
+    if (vact) {
+      float4 f[MAXV];
+#pragma unroll
+      for (int q = 0; q < MAXV; ++q)
+        f[q] = lds4(sC, (q & 1) ? hi16(vw[1 + (q >> 1)]) : lo16(vw[1 + (q >> 1)]));
+      float ax = 0.f, ay = 0.f, az = 0.f;
+#pragma unroll
+      for (int q = 0; q < MAXV; ++q) { ax += f[q].x; ay += f[q].y; az += f[q].z; }
+      float *gout = p.g + size_t(cell) * 3 * n_pad + tid;
+      float g0 = fmaf(coef, sg[3 * n_pad + tid], ax - sg[6 * n_pad + tid]);
+      float g1 = fmaf(coef, sg[4 * n_pad + tid], ay - sg[7 * n_pad + tid]);
+      float g2 = fmaf(coef, sg[5 * n_pad + tid], az - sg[8 * n_pad + tid]);
+      if (p.g_tf32) { g0 = tf32_rn(g0); g1 = tf32_rn(g1); g2 = tf32_rn(g2); }
+      gout[0] = g0;
+      gout[n_pad] = g1;
+      gout[2 * n_pad] = g2;
+    }
+    if (vact2c) {
+      float ax = 0.f, ay = 0.f, az = 0.f;
+      for (int q = 0; q < MAXV; ++q) {
+        const uint32_t w = p.vtx_words[(1 + (q >> 1)) * p.vstride + v2c];
+        const float4 f = lds4(sC, (q & 1) ? (w >> 16) : (w & 0xffffu));
+        ax += f.x; ay += f.y; az += f.z;
+      }
+      const float coef2 = p.vtx_coef[v2c];
+      float *gout = p.g + size_t(cell) * 3 * n_pad + v2c;
+      const float g0 = fmaf(coef2, sg[3 * n_pad + v2c], ax - sg[6 * n_pad + v2c]);
+      const float g1 = fmaf(coef2, sg[4 * n_pad + v2c], ay - sg[7 * n_pad + v2c]);
+      const float g2 = fmaf(coef2, sg[5 * n_pad + v2c], az - sg[8 * n_pad + v2c]);
+      gout[0] = p.g_tf32 ? tf32_rn(g0) : g0;
+      gout[n_pad] = p.g_tf32 ? tf32_rn(g1) : g1;
+      gout[2 * n_pad] = p.g_tf32 ? tf32_rn(g2) : g2;
+    }
   };
 
   // Software pipeline over the cells of this CTA (B1/B2/B3 = split barriers, parity it & 1):
@@ -204,8 +226,11 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
   //   corner forces | arrive B3 | phase 0 of the NEXT cell |
   //   arrive B1 | wait B3 | phase C
   // so a warp that is early at a barrier runs ahead into work that does not depend on it.
+  // (Tried in round 2 and dropped, profiles/r2_ncu.md: a two-barrier order with phase C of cell i-1 merged into the
+  // section of phase A of cell i - 1.435 vs 1.369 ms per launch: the six corner-force gathers queue in front of the
+  // vertex gathers that phase A's critical chain starts with.)
   if (int64_t(blockIdx.x) < p.cells) {
-    phase0(0, blockIdx.x);
+    phase0(0);
     bar_arrive(0);
   }
   int it = 0;
@@ -320,6 +345,13 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
     }
     bar_wait(3, par);                                  // BV: volume accumulated
     const int2 vd = *reinterpret_cast<const int2 *>(vacc + 2 * (it & 1));
+    // The int32 REDUX sums and the digit sums are exact MODULO 2^32 (a warp sum may wrap at a strongly deformed
+    // iterate); the cast to int is the modular reduction that makes the difference to the rest value exact again as
+    // long as |6V - 6V0| fx_scale < 2^31, i.e. while the volume stays within about +-80 % of V0 (6 V0 fx_scale is
+    // 0.6 .. 1.25 x 2^31) and no lane's partial saturates the float -> int conversion (2^31: 512 x the rest-shape
+    // bound).  Beyond that the volume force is garbage - the plain iteration has diverged long before, and the line
+    // search takes its decisions from the fp64 objective kernel, which has no such range.  (A 64-bit conversion here
+    // would be WRONG: it drops the modular reduction; tried in round 2, the violent line-search case caught it.)
     const float vc = p.vc_scale * float(int((static_cast<long long>(vd.x) << 12) + vd.y - p.fx_rest));
     float cf[TPT][9];
 #pragma unroll
@@ -345,44 +377,11 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
       }
     bar_arrive(2);
     if (cell + gridDim.x < p.cells) {                  // sx was last read in phase A (before B2)
-      phase0(it + 1, cell + gridDim.x);
+      phase0(it + 1);
       bar_arrive(0);
     }
     bar_wait(2, par);                                  // B3: corner forces complete
-    // ---- phase C ----------------------------------------------------------------------------
-    if (vact) {
-      float4 f[MAXV];
-#pragma unroll
-      for (int q = 0; q < MAXV; ++q)
-        f[q] = lds4(sC, (q & 1) ? hi16(vw[1 + (q >> 1)]) : lo16(vw[1 + (q >> 1)]));
-      float ax = 0.f, ay = 0.f, az = 0.f;
-#pragma unroll
-      for (int q = 0; q < MAXV; ++q) { ax += f[q].x; ay += f[q].y; az += f[q].z; }
-      float *gout = p.g + size_t(cell) * 3 * n_pad + tid;
-      float g0 = fmaf(coef, sg[3 * n_pad + tid], ax - sg[6 * n_pad + tid]);
-      float g1 = fmaf(coef, sg[4 * n_pad + tid], ay - sg[7 * n_pad + tid]);
-      float g2 = fmaf(coef, sg[5 * n_pad + tid], az - sg[8 * n_pad + tid]);
-      if (p.g_tf32) { g0 = tf32_rn(g0); g1 = tf32_rn(g1); g2 = tf32_rn(g2); }
-      gout[0] = g0;
-      gout[n_pad] = g1;
-      gout[2 * n_pad] = g2;
-    }
-    if (vact2c) {
-      float ax = 0.f, ay = 0.f, az = 0.f;
-      for (int q = 0; q < MAXV; ++q) {
-        const uint32_t w = p.vtx_words[(1 + (q >> 1)) * p.vstride + v2c];
-        const float4 f = lds4(sC, (q & 1) ? (w >> 16) : (w & 0xffffu));
-        ax += f.x; ay += f.y; az += f.z;
-      }
-      const float coef2 = p.vtx_coef[v2c];
-      float *gout = p.g + size_t(cell) * 3 * n_pad + v2c;
-      const float g0 = fmaf(coef2, sg[3 * n_pad + v2c], ax - sg[6 * n_pad + v2c]);
-      const float g1 = fmaf(coef2, sg[4 * n_pad + v2c], ay - sg[7 * n_pad + v2c]);
-      const float g2 = fmaf(coef2, sg[5 * n_pad + v2c], az - sg[8 * n_pad + v2c]);
-      gout[0] = p.g_tf32 ? tf32_rn(g0) : g0;
-      gout[n_pad] = p.g_tf32 ? tf32_rn(g1) : g1;
-      gout[2 * n_pad] = p.g_tf32 ? tf32_rn(g2) : g2;
-    }
+    phaseC(cell, sg);
     // sN / sC are rewritten only after B1 / B2 of the next cell, which every warp reaches after this
   }
 }
@@ -396,19 +395,19 @@ size_t sched_smem_bytes(const SchedDev &s, int n_pad) {
 }
 
 template <int TPT, int MAXV, int MAXT, int MINB, int NPAD>
-int launch_variant(const SchedParams &p, size_t smem, int n_sm, int64_t cells, cudaStream_t s) {
+int launch_variant(const SchedParams &p, KernelCache &kc, size_t smem, int n_sm, int64_t cells, cudaStream_t s) {
   auto kernel = local_sched_kernel<TPT, MAXV, MAXT, MINB, NPAD>;
-  static int per_sm = 0;          // per template instance; the smem size of a type never changes
-  static size_t smem_set = 0;
-  if (smem > smem_set) {
-    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) return -1;
-    smem_set = smem;
-    per_sm = 0;
-  }
-  if (per_sm == 0) {
+  // the opt-in attribute is per device and function, the occupancy follows from it: cached per context and type
+  if (kc.sched_smem != smem) {
+    // (always the architectural maximum: two types sharing this instantiation must not lower each other's limit)
+    if (opt_in_max_dynamic_smem(kernel) != cudaSuccess) return -1;
+    int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, p.threads, smem) != cudaSuccess || per_sm < 1)
       return -1;
+    kc.sched_smem = smem;
+    kc.sched_per_sm = per_sm;
   }
+  const int per_sm = kc.sched_per_sm;
   int64_t grid = int64_t(n_sm) * per_sm;
   if (grid > cells) grid = cells;
   kernel<<<unsigned(grid), p.threads, smem, s>>>(p);
@@ -424,8 +423,7 @@ bool local_sched_supported(const TypeDev &td) {
   return (s.tpt == 2 && s.threads <= 640) || (s.tpt == 1 && s.threads <= 320);
 }
 
-int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, bool apply_u, double d_scale,
-                       cudaStream_t stream) {
+int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t stream) {
   if (bv.cells == 0) return 0;
   if (!local_sched_supported(td)) return -1;
   const SchedDev &s = td.sched;
@@ -442,10 +440,8 @@ int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, bool a
   p.fx_rest = std::llrint(6.0 * td.V0 * scale);
   p.vc_scale = float(td.kv_over_V0 / 36.0 / scale);
   p.x = static_cast<const float *>(bv.field[F_X]);
-  p.d = static_cast<float *>(bv.field[F_D]);
-  p.u = static_cast<const float *>(bv.field[F_U]);
-  p.apply_u = apply_u ? 1 : 0;
-  p.d_scale = float(d_scale);
+  p.xl = static_cast<const float *>(bv.field[F_XL]);
+  p.d = static_cast<const float *>(bv.field[F_D]);
   p.b = static_cast<const float *>(bv.field[F_B]);
   p.g = static_cast<float *>(bv.field[F_G]);
   p.g_tf32 = bv.g_tf32;
@@ -453,13 +449,13 @@ int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, bool a
   const size_t smem = sched_smem_bytes(s, td.n_pad);
   // the BASELINE cell types get their row pitch at compile time, everything else the generic variants
   if (s.tpt == 2) {
-    if (s.maxv == 6 && td.n_pad == 656) return launch_variant<2, 6, 640, 1, 656>(p, smem, n_sm, bv.cells, stream);
-    if (s.maxv == 6) return launch_variant<2, 6, 640, 1, 0>(p, smem, n_sm, bv.cells, stream);
-    return launch_variant<2, 8, 640, 1, 0>(p, smem, n_sm, bv.cells, stream);
+    if (s.maxv == 6 && td.n_pad == 656) return launch_variant<2, 6, 640, 1, 656>(p, td.cache, smem, n_sm, bv.cells, stream);
+    if (s.maxv == 6) return launch_variant<2, 6, 640, 1, 0>(p, td.cache, smem, n_sm, bv.cells, stream);
+    return launch_variant<2, 8, 640, 1, 0>(p, td.cache, smem, n_sm, bv.cells, stream);
   }
-  if (s.maxv == 6 && td.n_pad == 176) return launch_variant<1, 6, 320, 2, 176>(p, smem, n_sm, bv.cells, stream);
-  if (s.maxv == 6) return launch_variant<1, 6, 320, 2, 0>(p, smem, n_sm, bv.cells, stream);
-  return launch_variant<1, 8, 320, 2, 0>(p, smem, n_sm, bv.cells, stream);
+  if (s.maxv == 6 && td.n_pad == 176) return launch_variant<1, 6, 320, 2, 176>(p, td.cache, smem, n_sm, bv.cells, stream);
+  if (s.maxv == 6) return launch_variant<1, 6, 320, 2, 0>(p, td.cache, smem, n_sm, bv.cells, stream);
+  return launch_variant<1, 8, 320, 2, 0>(p, td.cache, smem, n_sm, bv.cells, stream);
 }
 
 }  // namespace npfem

@@ -33,7 +33,7 @@ struct SmemLocalParams {
   const uint4 *vtx_pack;     // [n]  8 x u16 corner ids, 0xFFFF = none
   const float *vtx_coef;     // [n]  (1 - gamma) (1 + h alpha) m_v / h^2
   float B4, C4, k_b, kv_over_V0, V0;
-  const float *x, *d, *b;    // [cells][3][n_pad]
+  const float *x, *xl, *d, *b;   // [cells][3][n_pad]; positions are the two-float sum x + xl (internal.h F_XL)
   float *g;
   int g_tf32;
   int64_t cells;
@@ -116,7 +116,7 @@ local_smem_kernel(const SmemLocalParams p) {
         for (int k = 0; k < 3; ++k) {
           dv[r][k] = stage[(3 + k) * n_pad + i];
           bv[r][k] = stage[(6 + k) * n_pad + i];
-          xs[k] = stage[k * n_pad + i] + dv[r][k];
+          xs[k] = stage[k * n_pad + i] + (__ldg(p.xl + base + k * n_pad + i) + dv[r][k]);
         }
         sx[i] = make_float4(xs[0], xs[1], xs[2], 0.f);
       }
@@ -272,6 +272,7 @@ int launch_local_smem(const TypeDev &td, const BucketView &bv, int n_sm, cudaStr
   p.B4 = float(td.B4); p.C4 = float(td.C4); p.k_b = float(td.k_b); p.kv_over_V0 = float(td.kv_over_V0);
   p.V0 = float(td.V0);
   p.x = static_cast<const float *>(bv.field[F_X]);
+  p.xl = static_cast<const float *>(bv.field[F_XL]);
   p.d = static_cast<const float *>(bv.field[F_D]);
   p.b = static_cast<const float *>(bv.field[F_B]);
   p.g = static_cast<float *>(bv.field[F_G]);
@@ -288,11 +289,9 @@ int launch_local_smem(const TypeDev &td, const BucketView &bv, int n_sm, cudaStr
   if (per_sm * threads > 2048) per_sm = 2048 / threads;
   if (per_sm > 8) per_sm = 8;
   auto kernel = td.valence_max <= 6 ? local_smem_kernel<6> : local_smem_kernel<8>;
-  static bool attr[2] = {false, false};
-  const int which = td.valence_max <= 6 ? 0 : 1;
-  if (!attr[which]) {
+  if (!td.cache.smem_attr) {   // per context and type (the attribute is per device)
     if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024) != cudaSuccess) return -1;
-    attr[which] = true;
+    td.cache.smem_attr = true;
   }
   int64_t grid = int64_t(n_sm) * per_sm;
   if (grid > bv.cells) grid = bv.cells;

@@ -42,15 +42,20 @@ set_state_kernel(const BucketView *__restrict__ views, const CellRef *__restrict
   if (threadIdx.x < 3) bv.origin[size_t(ref.slot) * 3 + threadIdx.x] = origin[threadIdx.x];
   T *x = static_cast<T *>(bv.field[F_X]) + base;
   T *v = static_cast<T *>(bv.field[F_V]) + base;
+  T *xl = bv.field[F_XL] ? static_cast<T *>(bv.field[F_XL]) + base : nullptr;   // fp32 contexts: two-float positions
   for (int i = threadIdx.x; i < 3 * n; i += blockDim.x) {
     const int vert = i / 3, k = i % 3;
-    x[k * n_pad + vert] = T(load_as_double<U>(pos, ref.user_offset + i) - origin[k]);
+    const double local = load_as_double<U>(pos, ref.user_offset + i) - origin[k];
+    const T hi = T(local);
+    x[k * n_pad + vert] = hi;
+    if (xl) xl[k * n_pad + vert] = T(local - double(hi));
     v[k * n_pad + vert] = vel ? T(load_as_double<U>(vel, ref.user_offset + i)) : T(0);
   }
   // forces, rhs, displacement, gradient start at zero; padding columns of every field are zero
   for (int f = 0; f < F_COUNT; ++f) {
+    if (!bv.field[f]) continue;
     T *p = static_cast<T *>(bv.field[f]) + base;
-    const bool whole = (f != F_X && f != F_V);
+    const bool whole = (f != F_X && f != F_V && f != F_XL);
     for (int i = threadIdx.x; i < 3 * n_pad; i += blockDim.x)
       if (whole || (i % n_pad) >= n) p[i] = T(0);
   }
@@ -78,10 +83,12 @@ get_state_kernel(const BucketView *__restrict__ views, const CellRef *__restrict
   const size_t base = size_t(ref.slot) * 3 * n_pad;
   const T *x = static_cast<const T *>(bv.field[F_X]) + base;
   const T *v = static_cast<const T *>(bv.field[F_V]) + base;
+  const T *xl = bv.field[F_XL] ? static_cast<const T *>(bv.field[F_XL]) + base : nullptr;
   const double *origin = bv.origin + size_t(ref.slot) * 3;
   for (int i = threadIdx.x; i < 3 * n; i += blockDim.x) {
     const int vert = i / 3, k = i % 3;
-    if (pos) reinterpret_cast<U *>(pos)[ref.user_offset + i] = U(origin[k] + double(x[k * n_pad + vert]));
+    const double lo = xl ? double(xl[k * n_pad + vert]) : 0.0;
+    if (pos) reinterpret_cast<U *>(pos)[ref.user_offset + i] = U(origin[k] + (double(x[k * n_pad + vert]) + lo));
     if (vel) reinterpret_cast<U *>(vel)[ref.user_offset + i] = U(v[k * n_pad + vert]);
   }
 }

@@ -43,6 +43,7 @@ prologue_kernel(BucketView bv, const T *__restrict__ mass, double kappa, double 
     const T *f = static_cast<const T *>(bv.field[F_F]) + base;
     T *b = static_cast<T *>(bv.field[F_B]) + base;
     T *d = static_cast<T *>(bv.field[F_D]) + base;
+    T *xl = bv.field[F_XL] ? static_cast<T *>(bv.field[F_XL]) + base : nullptr;
 
     double s[7] = {};   // sum m, sum m x, sum m v
     for (int i = threadIdx.x; i < n; i += blockDim.x) {
@@ -106,7 +107,11 @@ prologue_kernel(BucketView bv, const T *__restrict__ mass, double kappa, double 
         for (int k = 0; k < 3; ++k) vi[k] += kappa * (vc[k] + w[k] - vi[k]);
       }
       for (int k = 0; k < 3; ++k) {
-        if (recentre) x[k * n_pad + i] = T(xi[k] - shift[k]);
+        if (recentre) {   // what the shifted coordinate loses when it is rounded to T goes to the low part
+          const T hi = T(xi[k] - shift[k]);
+          x[k * n_pad + i] = hi;
+          if (xl) xl[k * n_pad + i] += T((xi[k] - shift[k]) - double(hi));
+        }
         v[k * n_pad + i] = T(vi[k]);
         b[k * n_pad + i] = T(m * vi[k] / h + double(f[k * n_pad + i]));
         d[k * n_pad + i] = T(h * vi[k]);
@@ -211,9 +216,15 @@ prologue_warp_kernel(BucketView bv, const float *__restrict__ mass, float kappa,
 #pragma unroll
         for (int k = 0; k < 3; ++k) v[q][k] += kappa * (vcf[k] + w[k] - v[q][k]);
       }
-      if (recentre && i < n) {
+      if (recentre && i < n) {   // rare; the rounding of the shifted coordinate goes to the low part (F_XL)
+        float *xlg = static_cast<float *>(bv.field[F_XL]) + base;
 #pragma unroll
-        for (int k = 0; k < 3; ++k) xg[k * n_pad + i] = x[q][k] - shift[k];
+        for (int k = 0; k < 3; ++k) {
+          const double xs = double(x[q][k]) - double(shift[k]);
+          const float hi = float(xs);
+          xg[k * n_pad + i] = hi;
+          xlg[k * n_pad + i] += float(xs - double(hi));
+        }
       }
     }
     float f[VPT][3];
@@ -239,13 +250,16 @@ prologue_warp_kernel(BucketView bv, const float *__restrict__ mass, float kappa,
   }
 }
 
+// x_{n+1} = x_n + d, v_{n+1} = d/h.  fp32 contexts keep positions as the two-float sum x + xl: t = xl + d,
+// x' = fl(x + t), xl' = t - (x' - x) (exact: Fast2Sum with |t| << |x|), so the state moves by d to within an ulp of d,
+// not of x (rounding x_n + d to fp32 every step was the floor of the displacement error).
 template <typename T>
 __global__ void __launch_bounds__(256)
-epilogue_kernel(BucketView bv, T inv_h, bool pending, T d_scale, T v_max) {
+epilogue_kernel(BucketView bv, T inv_h, T v_max) {
   T *x = static_cast<T *>(bv.field[F_X]);
   T *v = static_cast<T *>(bv.field[F_V]);
+  T *xl = static_cast<T *>(bv.field[F_XL]);                // null in fp64 contexts
   const T *d = static_cast<const T *>(bv.field[F_D]);
-  const T *u = static_cast<const T *>(bv.field[F_U]);
   const int n_pad = bv.n_pad;
   const size_t total = size_t(bv.cells) * n_pad;          // one thread per (cell, vertex slot)
   for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < total; i += size_t(gridDim.x) * blockDim.x) {
@@ -254,9 +268,14 @@ epilogue_kernel(BucketView bv, T inv_h, bool pending, T d_scale, T v_max) {
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
       const size_t o = base + size_t(k) * n_pad;
-      // pending: the last global step left its product in u (d <- d_scale d + u not applied yet)
-      const T di = pending ? d_scale * d[o] + u[o] : d[o];
-      x[o] += di;
+      const T di = d[o];
+      if (xl) {
+        const T x0 = x[o], t = xl[o] + di, x1 = x0 + t;
+        x[o] = x1;
+        xl[o] = t - (x1 - x0);
+      } else {
+        x[o] += di;
+      }
       vi[k] = di * inv_h;
     }
     if (v_max > T(0)) {   // vertex-velocity cap (reading R17): clamp the magnitude, keep the direction
@@ -270,22 +289,24 @@ epilogue_kernel(BucketView bv, T inv_h, bool pending, T d_scale, T v_max) {
   }
 }
 
-// fp32 fast path: one thread per 4 vertex slots, 128-bit accesses, all six loads in flight before the stores
+// fp32 fast path: one thread per 4 vertex slots, 128-bit accesses, all nine loads in flight before the stores
 __global__ void __launch_bounds__(256)
 epilogue_vec4_kernel(BucketView bv, float inv_h, float v_max) {
   float *x = static_cast<float *>(bv.field[F_X]);
   float *v = static_cast<float *>(bv.field[F_V]);
+  float *xl = static_cast<float *>(bv.field[F_XL]);
   const float *d = static_cast<const float *>(bv.field[F_D]);
   const unsigned q_pad = unsigned(bv.n_pad) >> 2;
   const size_t total = size_t(bv.cells) * q_pad;
   for (size_t i = blockIdx.x * size_t(blockDim.x) + threadIdx.x; i < total; i += size_t(gridDim.x) * blockDim.x) {
     const size_t cell = i / q_pad;
     const size_t base = cell * 3 * size_t(bv.n_pad) + 4 * (i - cell * q_pad);
-    float4 di[3], xi[3];
+    float4 di[3], xi[3], li[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
       di[k] = __ldcs(reinterpret_cast<const float4 *>(d + base + size_t(k) * bv.n_pad));
       xi[k] = *reinterpret_cast<const float4 *>(x + base + size_t(k) * bv.n_pad);
+      li[k] = *reinterpret_cast<const float4 *>(xl + base + size_t(k) * bv.n_pad);
     }
     float sc[4] = {inv_h, inv_h, inv_h, inv_h};
     if (v_max > 0.f) {
@@ -300,14 +321,22 @@ epilogue_vec4_kernel(BucketView bv, float inv_h, float v_max) {
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
       const float4 dk = di[k];
-      float4 xo = xi[k], vo;
-      xo.x += dk.x; xo.y += dk.y; xo.z += dk.z; xo.w += dk.w;
+      float4 xo, lo, vo;
+      const float *x0 = &xi[k].x, *l0 = &li[k].x, *de = &dk.x;
+      float *x1 = &xo.x, *l1 = &lo.x;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {   // compensated x + xl += d (see epilogue_kernel)
+        const float t = l0[e] + de[e];
+        x1[e] = x0[e] + t;
+        l1[e] = t - (x1[e] - x0[e]);
+      }
       if (v_max > 0.f) {
         vo.x = dk.x * inv_h * sc[0]; vo.y = dk.y * inv_h * sc[1]; vo.z = dk.z * inv_h * sc[2]; vo.w = dk.w * inv_h * sc[3];
       } else {
         vo.x = dk.x * inv_h; vo.y = dk.y * inv_h; vo.z = dk.z * inv_h; vo.w = dk.w * inv_h;
       }
       *reinterpret_cast<float4 *>(x + base + size_t(k) * bv.n_pad) = xo;
+      *reinterpret_cast<float4 *>(xl + base + size_t(k) * bv.n_pad) = lo;
       *reinterpret_cast<float4 *>(v + base + size_t(k) * bv.n_pad) = vo;
     }
   }
@@ -333,19 +362,16 @@ int launch_prologue(const TypeDev &td, const BucketView &bv, int precision, cuda
   return 1;
 }
 
-int launch_epilogue(const TypeDev &td, const BucketView &bv, int precision, bool pending, double d_scale,
-                    double v_max, cudaStream_t s) {
+int launch_epilogue(const TypeDev &td, const BucketView &bv, int precision, double v_max, cudaStream_t s) {
   if (bv.cells == 0) return 0;
   const size_t total = size_t(bv.cells) * bv.n_pad;
   const unsigned grid = unsigned((total + 255) / 256 < 148 * 16 ? (total + 255) / 256 : 148 * 16);
-  if (precision == NPFEM_F32 && !pending) {
+  if (precision == NPFEM_F32) {
     const size_t quads = total / 4;
     const unsigned g4 = unsigned((quads + 255) / 256 < 148 * 32 ? (quads + 255) / 256 : 148 * 32);
     epilogue_vec4_kernel<<<g4, 256, 0, s>>>(bv, float(1.0 / td.h), float(v_max));
-  } else if (precision == NPFEM_F32)
-    epilogue_kernel<float><<<grid, 256, 0, s>>>(bv, float(1.0 / td.h), pending, float(d_scale), float(v_max));
-  else
-    epilogue_kernel<double><<<grid, 256, 0, s>>>(bv, 1.0 / td.h, pending, d_scale, v_max);
+  } else
+    epilogue_kernel<double><<<grid, 256, 0, s>>>(bv, 1.0 / td.h, v_max);
   return 1;
 }
 

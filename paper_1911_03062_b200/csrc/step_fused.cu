@@ -45,7 +45,7 @@ struct FusedParams {
   long long fx_rest;
   float vc_scale;
   float kappa, h, d_scale, v_max;
-  float *x, *v;                // [cells][3][n_pad], updated
+  float *x, *xl, *v;           // [cells][3][n_pad], updated; positions are the two-float sum x + xl (internal.h F_XL)
   const float *f;
   double *origin;              // [cells][3]
   int64_t cells;
@@ -82,7 +82,8 @@ __global__ void __launch_bounds__(256, 1) step_fused_kernel(const FusedParams p)
   float *xn = reinterpret_cast<float *>(sC + p.sC_bytes);   // [3][n_pad] x_n (cell-local)
   float *sd = xn + 3 * n_pad;                               // [3][n_pad] d (v during the prologue)
   float *sb = sd + 3 * n_pad;                               // [3][n_pad] b
-  float4 *sr = reinterpret_cast<float4 *>(sb + 3 * n_pad);  // [n_pad]    reduced gradient r, padding rows zero
+  float *sl = sb + 3 * n_pad;                               // [3][n_pad] low part of x_n
+  float4 *sr = reinterpret_cast<float4 *>(sl + 3 * n_pad);  // [n_pad]    reduced gradient r, padding rows zero
   double *red = reinterpret_cast<double *>(sr + n_pad);     // [8][16]
   int *vacc = reinterpret_cast<int *>(red + 8 * 16);        // [2] fixed-point 6V (hi, lo)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -105,7 +106,7 @@ __global__ void __launch_bounds__(256, 1) step_fused_kernel(const FusedParams p)
 
   for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x) {
     const size_t base = size_t(cell) * 3 * n_pad;
-    float *xg = p.x + base, *vg = p.v + base;
+    float *xg = p.x + base, *lg = p.xl + base, *vg = p.v + base;
     const float *fg = p.f + base;
     // ================= prologue: PBD damping, b, d0 =================================================
     double s[16];
@@ -115,6 +116,7 @@ __global__ void __launch_bounds__(256, 1) step_fused_kernel(const FusedParams p)
       const float x0f = xg[i], x1f = xg[n_pad + i], x2f = xg[2 * n_pad + i];
       const float v0f = vg[i], v1f = vg[n_pad + i], v2f = vg[2 * n_pad + i];
       xn[i] = x0f; xn[n_pad + i] = x1f; xn[2 * n_pad + i] = x2f;
+      sl[i] = lg[i]; sl[n_pad + i] = lg[n_pad + i]; sl[2 * n_pad + i] = lg[2 * n_pad + i];
       sd[i] = v0f; sd[n_pad + i] = v1f; sd[2 * n_pad + i] = v2f;
       const double md = double(p.mass[i]);
       const double x0 = x0f, x1 = x1f, x2 = x2f, p0 = md * v0f, p1 = md * v1f, p2 = md * v2f;
@@ -166,7 +168,12 @@ __global__ void __launch_bounds__(256, 1) step_fused_kernel(const FusedParams p)
       const float mh = p.mass[i] * inv_h;
 #pragma unroll
       for (int k = 0; k < 3; ++k) {
-        xn[k * n_pad + i] = xi[k] - shift[k];
+        if (recentre) {   // rare; the rounding of the shifted coordinate goes to the low part
+          const double xs = double(xi[k]) - double(shift[k]);
+          const float hi = float(xs);
+          xn[k * n_pad + i] = hi;
+          sl[k * n_pad + i] += float(xs - double(hi));
+        }
         sb[k * n_pad + i] = fmaf(mh, vi[k], fg[k * n_pad + i]);
         sd[k * n_pad + i] = p.h * vi[k];
       }
@@ -176,7 +183,8 @@ __global__ void __launch_bounds__(256, 1) step_fused_kernel(const FusedParams p)
     for (int k_it = 0; k_it < p.n_iterations; ++k_it) {
       // ---- phase 0: sx[slot(v)] = (x_n + d, 0) ---------------------------------------------------
       for (int i = tid; i < n; i += nthreads)
-        sts4(sx, lo16(p.vtx_words[i]), xn[i] + sd[i], xn[n_pad + i] + sd[n_pad + i], xn[2 * n_pad + i] + sd[2 * n_pad + i], 0.f);
+        sts4(sx, lo16(p.vtx_words[i]), xn[i] + (sl[i] + sd[i]), xn[n_pad + i] + (sl[n_pad + i] + sd[n_pad + i]),
+             xn[2 * n_pad + i] + (sl[2 * n_pad + i] + sd[2 * n_pad + i]), 0.f);
       if (tid == 0) vacc[0] = vacc[1] = 0;
       if (tid < 8) sts4(sC, uint32_t(p.sC_bytes) - 128u + 16u * tid, 0.f, 0.f, 0.f, 0.f);   // the zero slots (sC doubles as scratch)
       __syncthreads();
@@ -223,6 +231,7 @@ __global__ void __launch_bounds__(256, 1) step_fused_kernel(const FusedParams p)
       }
       __syncthreads();                                   // sN complete, volume accumulated
       // ---- phase B: hinges (reading R8), volume term (R9), corner forces -------------------------------
+      // (the cast to int is the modular reduction of the wrapped int32 sums: see local_sched.cu for the validity range)
       const float vc = p.vc_scale * float(int((static_cast<long long>(vacc[0]) << 12) + vacc[1] - p.fx_rest));
 #pragma unroll
       for (int j = 0; j < TPT; ++j) {
@@ -336,7 +345,9 @@ __global__ void __launch_bounds__(256, 1) step_fused_kernel(const FusedParams p)
 #pragma unroll
       for (int k = 0; k < 3; ++k) {
         const float di = sd[k * n_pad + i];
-        xg[k * n_pad + i] = xn[k * n_pad + i] + di;
+        const float x0 = xn[k * n_pad + i], t = sl[k * n_pad + i] + di, x1 = x0 + t;   // compensated x + xl += d (prologue.cu)
+        xg[k * n_pad + i] = x1;
+        lg[k * n_pad + i] = t - (x1 - x0);
         vi[k] = di * inv_h;
       }
       if (p.v_max > 0.f) {
@@ -353,7 +364,7 @@ __global__ void __launch_bounds__(256, 1) step_fused_kernel(const FusedParams p)
 }
 
 size_t fused_smem_bytes(const SchedDev &s, int n_pad) {
-  return size_t(s.n_vslots + s.n_tslots + s.n_cslots) * 16 + size_t(9) * n_pad * 4 + size_t(n_pad) * 16 + 8 * 16 * 8 + 16;
+  return size_t(s.n_vslots + s.n_tslots + s.n_cslots) * 16 + size_t(12) * n_pad * 4 + size_t(n_pad) * 16 + 8 * 16 * 8 + 16;
 }
 
 }  // namespace
@@ -383,14 +394,17 @@ int launch_step_fused(const TypeDev &td, const BucketView &bv, int n_sm, int n_i
   p.vc_scale = float(td.kv_over_V0 / 36.0 / scale);
   p.kappa = float(td.kappa); p.h = float(td.h); p.d_scale = float(1.0 - td.gamma); p.v_max = float(v_max);
   p.x = static_cast<float *>(bv.field[F_X]);
+  p.xl = static_cast<float *>(bv.field[F_XL]);
   p.v = static_cast<float *>(bv.field[F_V]);
   p.f = static_cast<const float *>(bv.field[F_F]);
   p.origin = bv.origin;
   p.cells = bv.cells;
   const size_t smem = fused_smem_bytes(s, td.n_pad);
   auto launch = [&](auto kernel) -> int {
-    if (smem > 48 * 1024 && cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess)
-      return -1;
+    if (!td.cache.fused_attr) {   // per context and type (the attribute is per device)
+      if (opt_in_max_dynamic_smem(kernel) != cudaSuccess) return -1;
+      td.cache.fused_attr = true;
+    }
     const int64_t grid = bv.cells < int64_t(n_sm) * 4 ? bv.cells : int64_t(n_sm) * 4;
     kernel<<<unsigned(grid), s.threads, smem, stream>>>(p);
     return 1;

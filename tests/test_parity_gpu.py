@@ -1,7 +1,10 @@
 """GPU parity: the CUDA path through the C-ABI against the fp64 oracle, element by element on the
 same seeded inputs.  Tolerances (BASELINE.json north_star): relative L2 on positions 1e-10 (fp64)
-and 1e-4 (fp32); the displacement-relative error (sharper) is checked against looser bars derived
-in DESIGN.md ("Tolerances")."""
+and 1e-4 (fp32).  That bar cannot fail (positions carry the placement offset), so every test also bounds
+the DISPLACEMENT error three ways (aggregate, worst cell, worst vertex: parity_utils.displacement_errors)
+and the velocity error.  fp64: 1e-8.  fp32: per test, at most 2 x the value measured on B200 and (for the
+aggregate) at most 1e-3; the measured values and the emulated fp32 floor they sit on are tabulated in
+DESIGN.md section 5."""
 import numpy as np
 import pytest
 
@@ -12,38 +15,55 @@ from workloads.populations import Population
 pytestmark = pytest.mark.gpu
 
 TOL_POS = {"fp64": 1e-10, "fp32": 1e-4}
-TOL_DISP = {"fp64": 1e-8, "fp32": 5e-3}
+TOL_FP64 = 1e-8          # displacement / velocity, fp64
+# fp32 tests that are not about precision (violent line-search cases, where the cells deform by a good fraction of
+# their size and a different backtracking decision moves the result): the bound of the round-1 suite, kept for those
+TOL_DISP = {"fp64": TOL_FP64, "fp32": 5e-3}
 
 
-def _check(pop, precision, **kw):
+def assert_row(r, precision, fp32):
+    """fp32 = (disp, worst_cell, worst_vertex, vel): <= 2 x the values measured on B200."""
+    assert r["pos"] <= TOL_POS[precision] and r["worst_cell_pos"] <= TOL_POS[precision], r
+    if precision == "fp64":
+        assert r["disp"] <= TOL_FP64 and r["worst_cell"] <= TOL_FP64 and r["worst_vertex"] <= TOL_FP64 and r["vel"] <= TOL_FP64, r
+    else:
+        disp, worst_cell, worst_vertex, vel = fp32
+        assert disp <= 1e-3
+        assert r["disp"] <= disp and r["worst_cell"] <= worst_cell and r["worst_vertex"] <= worst_vertex and r["vel"] <= vel, (r, fp32)
+
+
+def _check(pop, precision, fp32=None, **kw):
     gpu, solver = run_gpu(pop, precision, **kw)
     ref = run_oracle(pop, kw.get("n_steps"), kw.get("n_iterations"))
     rows = compare(pop, gpu, ref)
     solver.close()
     for r in rows:
         print(precision, r)
-        assert r["pos"] <= TOL_POS[precision], r
-        assert r["worst_cell_pos"] <= TOL_POS[precision], r
-        assert r["disp"] <= TOL_DISP[precision], r
-        assert r["vel"] <= TOL_DISP[precision], r
+        assert_row(r, precision, fp32)
     return rows
 
 
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 def test_config1_single_rbc(precision):
-    _check(make_config(1), precision)
+    # one step from rest: the displacement is ~1e-5 um, its fp32 error is the rounding of x + d itself
+    # measured (disp, worst cell, worst vertex, vel): 1.8e-4, 1.8e-4, 5.6e-4, 1.8e-4
+    _check(make_config(1), precision, fp32=(3.7e-4, 3.7e-4, 1.2e-3, 3.7e-4))
 
 
 @pytest.mark.parametrize("precision", ["fp32", "fp64"])
 def test_config2_reduced_70_cells_full_schedule(precision):
     # 70 cells = 210 GEMM rows: several 64-row tiles and a ragged tail; full 10 steps x 10 its
-    _check(make_config(2, n_cells=70), precision)
+    # measured 9.9e-5, 1.1e-4, 6.9e-4, 1.6e-4 (emulated floor of the two-float state 2.2e-5; the rest is the TF32
+    # rounding of H~^-1, DESIGN.md section 5: 2.3e-5 with the split-operator GEMM)
+    _check(make_config(2, n_cells=70), precision, fp32=(2e-4, 2.3e-4, 1.4e-3, 3.2e-4))
 
 
 @pytest.mark.parametrize("precision", ["fp32", "fp64"])
 def test_config3_mixed_types_redrawn_forces(precision):
     pop = make_config(3, n_cells=45)          # 41 RBC-642 + 4 PLT-162, interleaved ids
-    _check(pop, precision, n_steps=4, n_iterations=5)
+    # measured RBC-642 3.7e-5, 4.0e-4, 1.3e-3, 6.5e-5 (floor 3.1e-5, 4.3e-4, 1.5e-3, 6.1e-5: one cell that hardly moves),
+    # PLT-162 1.4e-5, 1.5e-5, 4.4e-5, 1.6e-5
+    _check(pop, precision, fp32=(8e-5, 8e-4, 2.7e-3, 1.4e-4), n_steps=4, n_iterations=5)
 
 
 @pytest.mark.parametrize("precision,impl", [("fp32", 0), ("fp32", 1), ("fp32", 4), ("fp64", 0)])
@@ -51,7 +71,9 @@ def test_config5_level4_mesh(precision, impl):
     # 2562 vertices / 5120 triangles: too large for the scheduled kernel -> large-mesh kernel (fp32 default,
     # corner forces in chunks) or the generic kernel with its global scratch (impl 1, fp64)
     from paper_1911_03062_b200 import binding
-    _check(make_config(5, n_cells=40), precision, n_steps=2, n_iterations=3, options=[(binding.OPT_LOCAL_STEP_IMPL, impl)])
+    # measured 2.4e-4, 2.6e-4, 1.3e-3, 2.5e-4 (large-mesh kernel), 2.1e-4, 2.2e-4, 9.7e-4, 2.1e-4 (generic)
+    _check(make_config(5, n_cells=40), precision, fp32=(5e-4, 5.2e-4, 2.7e-3, 5.1e-4), n_steps=2, n_iterations=3,
+           options=[(binding.OPT_LOCAL_STEP_IMPL, impl)])
 
 
 def test_icosahedron_cell_fp64():
@@ -176,26 +198,26 @@ def test_tf32_tensor_core_global_step_vs_fp32_ffma():
         d_tf32, d_ffma, d_ref = tf32[t][0] - x0, ffma[t][0] - x0, ref[t][0] - x0
         print(pop.types[t].name, "tf32 vs ffma", rel_l2(d_tf32, d_ffma), "tf32 vs oracle", rel_l2(d_tf32, d_ref),
               "ffma vs oracle", rel_l2(d_ffma, d_ref))
-        assert rel_l2(d_tf32, d_ffma) < 2e-3
+        # measured: tf32 vs ffma 4.0e-5 / 1.7e-5, tf32 vs oracle 5.5e-5 / 1.7e-5, ffma vs oracle 4.9e-5 / 6.7e-6
+        assert rel_l2(d_tf32, d_ffma) < 8e-5
         assert rel_l2(tf32[t][0], ref[t][0]) < 1e-4
-        assert rel_l2(d_tf32, d_ref) < 5e-3
+        assert rel_l2(d_tf32, d_ref) < 1.1e-4 and rel_l2(d_ffma, d_ref) < 1e-4
 
 
-@pytest.mark.parametrize("impl,update_mode", [(1, 0), (2, 0), (3, 1), (3, 2)])
-def test_fp32_local_step_implementations(impl, update_mode):
+@pytest.mark.parametrize("impl", [1, 2, 3])
+def test_fp32_local_step_implementations(impl):
     """Every fp32 local-step kernel (1 generic, 2 shared-memory tables, 3 scheduled: register-resident
     topology + colour-assigned conflict-free slots) against the oracle; RBC-642 exercises the second
-    vertex pass of the scheduled kernel (642 vertices on 640 threads).  update_mode 1: the tensor-core GEMM
-    epilogue updates d in place; 2: it writes its product and the next local step / the epilogue applies it."""
+    vertex pass of the scheduled kernel (642 vertices on 640 threads)."""
     from paper_1911_03062_b200 import binding
     pop = make_config(3, n_cells=300)         # 273 RBC + 27 PLT: more cells than one wave of CTAs for PLT
-    gpu, solver = run_gpu(pop, "fp32", n_steps=3, n_iterations=5, options=[(binding.OPT_LOCAL_STEP_IMPL, impl), (binding.OPT_UPDATE_MODE, update_mode)])
+    gpu, solver = run_gpu(pop, "fp32", n_steps=3, n_iterations=5, options=[(binding.OPT_LOCAL_STEP_IMPL, impl)])
     solver.close()
     ref = run_oracle(pop, 3, 5)
     for r in compare(pop, gpu, ref):
         print(impl, r)
-        assert r["pos"] <= TOL_POS["fp32"] and r["worst_cell_pos"] <= TOL_POS["fp32"], r
-        assert r["disp"] <= TOL_DISP["fp32"] and r["vel"] <= TOL_DISP["fp32"], r
+        # measured (all three kernels within 10 %): RBC-642 6.1e-5, 6.5e-4, 2.1e-3, 8.8e-5; PLT-162 2.1e-5, 1.0e-4, 2.5e-4, 2.8e-5
+        assert_row(r, "fp32", (1.3e-4, 1.3e-3, 4.3e-3, 1.8e-4))
 
 
 @pytest.mark.parametrize("precision,impl", [("fp64", 0), ("fp32", 1), ("fp32", 3)])
@@ -219,7 +241,14 @@ def test_irregular_mesh_valence_up_to_8(precision, impl):
     ref = run_oracle(pop)
     for r in compare(pop, gpu, ref):
         print(precision, impl, r)
-        assert r["pos"] <= TOL_POS[precision] and r["disp"] <= TOL_DISP[precision] and r["vel"] <= TOL_DISP[precision], r
+        # An irregular mesh with slivers (valence 4..8 after random edge flips): the strain invariants of its thin
+        # triangles amplify the fp32 rounding.  measured: generic 1.9e-3, 2.7e-3, 6.6e-3, 1.2e-3; scheduled 1.1e-3,
+        # 1.6e-3, 3.8e-3, 6.5e-4 - the one test whose aggregate stays above 1e-3 (bound by hand, not by assert_row)
+        assert r["pos"] <= TOL_POS[precision], r
+        if precision == "fp64":
+            assert r["disp"] <= TOL_FP64 and r["vel"] <= TOL_FP64, r
+        else:
+            assert r["disp"] <= 3.8e-3 and r["worst_cell"] <= 5.4e-3 and r["worst_vertex"] <= 1.4e-2 and r["vel"] <= 2.4e-3, r
 
 
 def _ls_population(n_cells, h, force_sigma, seed, level=2):
@@ -262,8 +291,9 @@ def test_line_search_violent_case_matches_oracle(precision):
     assert np.all(np.isfinite(xg))
     # the cells deform by a good fraction of their size here, so the position-relative error IS the
     # displacement-relative one: the displacement bound of DESIGN.md section 5 applies to both
-    assert rel_l2(xg, xr) <= TOL_DISP[precision]
-    assert rel_l2(xg - x0, xr - x0) <= TOL_DISP[precision]
+    bound = TOL_FP64 if precision == "fp64" else 4e-4               # fp32 measured 1.1e-4 .. 1.6e-4
+    assert rel_l2(xg, xr) <= bound
+    assert rel_l2(xg - x0, xr - x0) <= bound
     if precision == "fp64":
         assert np.array_equal(alpha, hist["alpha"][-1])
     else:
@@ -299,7 +329,7 @@ def test_line_search_large_time_step_rbc642(precision):
     x0 = pop.positions[0]
     print(precision, "disp", rel_l2(xg - x0, xr - x0), "alpha gpu", alpha, "oracle", hist["alpha"][-1])
     assert np.all(np.isfinite(xg))
-    assert rel_l2(xg - x0, xr - x0) <= TOL_DISP[precision]
+    assert rel_l2(xg - x0, xr - x0) <= (TOL_FP64 if precision == "fp64" else 2e-6)   # fp32 measured 7.6e-7 (full steps throughout)
     if precision == "fp64":
         assert np.array_equal(alpha, hist["alpha"][-1])
 
@@ -355,7 +385,7 @@ def test_line_search_fp32_fast_kernels_match_the_generic_full_gradient():
     x0 = pop.positions[0]
     for impl in (0, 1):
         print("impl", impl, "disp error vs oracle", rel_l2(out[impl] - x0, xr - x0))
-        assert rel_l2(out[impl] - x0, xr - x0) <= TOL_DISP["fp32"]
+        assert rel_l2(out[impl] - x0, xr - x0) <= 3.3e-4           # measured 1.1e-4 .. 1.6e-4 (impl 0), 9.1e-5 (impl 1)
     pop = make_config(3, n_cells=40)
     ref = run_oracle(pop, 2, 5)                                      # full steps descend here: plain oracle
     solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision="fp32")
@@ -407,7 +437,7 @@ def test_line_search_with_collisions_is_neutral_when_full_steps_descend(precisio
         x0 = pop.positions[t]
         print(precision, ct.name, rel_l2(xs[t], xr), rel_l2(xs[t] - x0, xr - x0))
         assert rel_l2(xs[t], xr) <= TOL_POS[precision]
-        assert rel_l2(xs[t] - x0, xr - x0) <= TOL_DISP[precision]
+        assert rel_l2(xs[t] - x0, xr - x0) <= (TOL_FP64 if precision == "fp64" else 1.2e-4)   # fp32 measured 5.5e-5 / 2.1e-5
 
 
 def test_line_search_is_neutral_on_a_tame_case_and_freezes_by_tolerance():
@@ -468,8 +498,9 @@ def test_median_filtered_forces_and_velocity_cap(precision):
         assert rel_l2(xr - x0, x_plain - x0) > 0.05                                              # the filter matters
         print(precision, ct.name, rel_l2(xs[t], xr), rel_l2(xs[t] - x0, xr - x0), rel_l2(vs[t], vr))
         assert rel_l2(xs[t], xr) <= TOL_POS[precision]
-        assert rel_l2(xs[t] - x0, xr - x0) <= TOL_DISP[precision]
-        assert rel_l2(vs[t], vr) <= TOL_DISP[precision]
+        # fp32 measured: disp 7.5e-5 / 2.3e-5, vel 3.2e-4 / 3.7e-5 (RBC-642 / PLT-162)
+        assert rel_l2(xs[t] - x0, xr - x0) <= (TOL_FP64 if precision == "fp64" else 1.5e-4)
+        assert rel_l2(vs[t], vr) <= (TOL_FP64 if precision == "fp64" else 6.5e-4)
         assert np.linalg.norm(vs[t], axis=-1).max() <= v_max * (1 + 1e-6)
 
 
@@ -513,7 +544,7 @@ def test_collision_term_matches_oracle(precision, where):
         assert rel_l2(xr - x0, x_plain - x0) > 0.05               # the contacts matter
         print(precision, ct.name, rel_l2(xs[t], xr), rel_l2(xs[t] - x0, xr - x0))
         assert rel_l2(xs[t], xr) <= TOL_POS[precision]
-        assert rel_l2(xs[t] - x0, xr - x0) <= TOL_DISP[precision]
+        assert rel_l2(xs[t] - x0, xr - x0) <= (TOL_FP64 if precision == "fp64" else 2.8e-4)   # fp32 measured 1.4e-4 / 6.6e-5
     # objective of the last step (diagnostics) includes the collision energy
     t = 0
     td = orc.make_type(pop.types[t], pop.dt)
@@ -541,8 +572,9 @@ def test_whole_step_fused_kernel(config, cells, fused):
     ref = run_oracle(pop, 4, 5)
     for r in compare(pop, gpu, ref):
         print(config, fused, r)
-        assert r["pos"] <= TOL_POS["fp32"] and r["worst_cell_pos"] <= TOL_POS["fp32"], r
-        assert r["disp"] <= TOL_DISP["fp32"] and r["vel"] <= TOL_DISP["fp32"], r
+        # measured RBC-258 1.7e-4, 3.1e-4, 9.8e-4, 4.0e-4; PLT-66 4.5e-5, 4.0e-4, 8.1e-4, 1.2e-4 (round 1: 1.0e-3 / 2.0e-3,
+        # the floor of a one-float state: DESIGN.md section 5)
+        assert_row(r, "fp32", (3.4e-4, 8e-4, 2e-3, 8e-4))
 
 
 def test_whole_step_fused_kernel_is_the_one_that_ran():
@@ -567,7 +599,9 @@ def test_paper_resolution_meshes_config6(precision):
     per-GPU load of 114 cells and h = 0.25 us; valence-4 vertices, 2 overflow vertices on a 256-thread CTA."""
     pop = make_config(6)
     assert [ct.n_vertices for ct in pop.types] == [258, 66] and pop.n_cells == 114 and pop.dt == 0.25
-    _check(pop, precision, n_steps=4, n_iterations=5)
+    # batched kernels (114 cells: auto would take the whole-step kernel; run_gpu forces the batched path)
+    # measured RBC-258 2.0e-4, 3.5e-4, 1.1e-3, 4.2e-4; PLT-66 1.5e-4, 9.5e-4, 1.7e-3, 2.0e-4
+    _check(pop, precision, fp32=(4e-4, 1.9e-3, 3.5e-3, 8.4e-4), n_steps=4, n_iterations=5)
 
 
 def _sampled_full_size(config, precision, n_steps, n_iterations, samples_per_type=6):
@@ -606,7 +640,7 @@ def test_full_size_config4_100k_cells_sampled():
     recomputes a seeded sample of ~1,000 cells per type, about a minute of host time."""
     for name, pos, disp, vel in _sampled_full_size(4, "fp32", n_steps=2, n_iterations=10, samples_per_type=1000):
         print(name, pos, disp, vel)
-        assert pos <= TOL_POS["fp32"] and disp <= TOL_DISP["fp32"] and vel <= TOL_DISP["fp32"]
+        assert pos <= TOL_POS["fp32"] and disp <= 1.2e-4 and vel <= 1.4e-4      # measured 5.6e-5 / 2.5e-5 and 7.0e-5 / 2.7e-5
 
 
 @pytest.mark.parametrize("precision", ["fp32", "fp64"])
@@ -614,7 +648,8 @@ def test_full_size_config5_10k_level4_cells_sampled(precision):
     """BASELINE configs[4] at its full 10,000 RBC-2562 cells (generic local step, 11-pass GEMM)."""
     for name, pos, disp, vel in _sampled_full_size(5, precision, n_steps=1, n_iterations=5, samples_per_type=3):
         print(name, pos, disp, vel)
-        assert pos <= TOL_POS[precision] and disp <= TOL_DISP[precision] and vel <= TOL_DISP[precision]
+        bound = TOL_FP64 if precision == "fp64" else 5.6e-4                       # fp32 measured 2.8e-4 (disp = vel: one step)
+        assert pos <= TOL_POS[precision] and disp <= bound and vel <= bound
 
 
 @pytest.mark.parametrize("kappa", [0.7, 0.8, 0.9])
@@ -626,7 +661,8 @@ def test_kappa_damping_sweep_config6(kappa):
     pop.types = [dataclasses.replace(ct, material=dataclasses.replace(ct.material, kappa_damping=kappa))
                  for ct in pop.types]
     _check(pop, "fp64", n_steps=5, n_iterations=5)
-    _check(pop, "fp32", n_steps=5, n_iterations=5, fused_step=2)
+    # measured (all three kappa): RBC-258 1.3e-4, 3.0e-4, 1.1e-3, 3.7e-4; PLT-66 3.5e-5, 7.5e-5, 2.1e-4, 1.3e-4
+    _check(pop, "fp32", fp32=(2.6e-4, 6.1e-4, 2.2e-3, 7.5e-4), n_steps=5, n_iterations=5, fused_step=2)
 
 
 @pytest.mark.parametrize("precision", ["fp32", "fp64"])
@@ -760,7 +796,7 @@ def test_level5_mesh_10242_vertices_runs_from_global_scratch(precision):
     global scratch.  One cell, 1 step x 3 iterations against the oracle."""
     pop = make_config(1, level=5)
     assert pop.types[0].n_vertices == 10242
-    _check(pop, precision, n_steps=1, n_iterations=3)
+    _check(pop, precision, fp32=(5.1e-4, 5.1e-4, 1.7e-3, 5.1e-4), n_steps=1, n_iterations=3)   # measured 2.5e-4, 2.5e-4, 8.4e-4, 2.5e-4
 
 
 @pytest.mark.parametrize("precision", ["fp32", "fp64"])
@@ -796,8 +832,8 @@ def test_drifting_cells_recentre_their_local_frame(precision):
         cerr = np.linalg.norm(centre - expect, axis=1).max() / np.linalg.norm(expect, axis=1).max()
         print(precision, ct.name, "disp", disp, "vel", vel, "centre", cerr, "moved um", np.linalg.norm(expect, axis=1).min())
         assert np.linalg.norm(expect, axis=1).min() > 2.0               # far beyond the 0.5 um threshold
-        assert disp <= TOL_DISP[precision] and vel <= TOL_DISP[precision]
-        assert cerr <= (1e-4 if precision == "fp32" else 1e-9)       # fp32: measured 1.4e-5 (1.3e-3 with truncated TF32 operands)
+        assert disp <= (3.3e-5 if precision == "fp32" else TOL_FP64) and vel <= (3.6e-5 if precision == "fp32" else TOL_FP64)   # fp32 measured 1.6e-5 / 1.8e-5
+        assert cerr <= (2.3e-5 if precision == "fp32" else 1e-9)     # fp32: measured 1.1e-5 (1.3e-3 with truncated TF32 operands)
 
 
 @pytest.mark.parametrize("cells", [600, 1800])
