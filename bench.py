@@ -76,7 +76,11 @@ def load_ncu_raw(kernel: str):
             if h == metric:
                 return float(vals[i]) if vals[i] not in ("", "no data") else None
         return None
-    fadd, fmul, ffma = (col(f"smsp__sass_thread_inst_executed_op_{op}_pred_on.sum") for op in ("fadd", "fmul", "ffma"))
+    # `--set full` keeps the fp32 op counts as chip-wide per-cycle sums: thread instructions = that x the elapsed cycles
+    cycles = col("smsp__cycles_elapsed.avg")
+    fadd, fmul, ffma = (col(f"smsp__sass_thread_inst_executed_op_{op}_pred_on.sum.per_cycle_elapsed") for op in ("fadd", "fmul", "ffma"))
+    if None not in (cycles, fadd, fmul, ffma):
+        fadd, fmul, ffma = fadd * cycles, fmul * cycles, ffma * cycles
     out = {"file": "profiles/" + name,
            "dram_bytes": (col("dram__bytes_read.sum") or 0) + (col("dram__bytes_write.sum") or 0),
            "warp_instructions": col("smsp__inst_executed.sum"),

@@ -226,9 +226,12 @@ __global__ void __launch_bounds__(MAXT, MINB) local_sched_kernel(const SchedPara
   //   corner forces | arrive B3 | phase 0 of the NEXT cell |
   //   arrive B1 | wait B3 | phase C
   // so a warp that is early at a barrier runs ahead into work that does not depend on it.
-  // (Tried in round 2 and dropped, profiles/r2_ncu.md: a two-barrier order with phase C of cell i-1 merged into the
-  // section of phase A of cell i - 1.435 vs 1.369 ms per launch: the six corner-force gathers queue in front of the
-  // vertex gathers that phase A's critical chain starts with.)
+  // Tried in round 2 and dropped (A / B on one box each, profiles/r2_ncu.md): (1) a two-barrier order with phase C of
+  // cell i-1 merged into the section of phase A of cell i: 1.435 vs 1.369 ms per launch - the six corner-force gathers
+  // queue in front of the vertex gathers that phase A's critical chain starts with; (2) phase C of cell i-1
+  // interleaved with the hinge arithmetic of cell i (three gathers in front of each triangle's hinges, summed behind
+  // them, an extra "corner forces consumed" barrier before the next stores): 1.693 vs 1.352 ms - at the 96-register
+  // cap the twelve extra live registers spill, and gathers issued inside the issue-bound section wait behind it.
   if (int64_t(blockIdx.x) < p.cells) {
     phase0(0);
     bar_arrive(0);
