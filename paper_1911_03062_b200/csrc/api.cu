@@ -1012,67 +1012,80 @@ int npfem_step_host(npfem_ctx *c, const void *forces, int32_t n_iterations, void
     c->views = full_views;
     for (size_t t = 0; t < nb; ++t) c->buckets[t].cells = full_cells[t];
   };
-  // the copy-in stream starts after whatever the caller's stream still has in flight on the staging buffers
-  cudaEvent_t ev_start = c->io_events[size_t(2 * n_chunks)];
-  NPFEM_CUDA(c, cudaEventRecord(ev_start, c->stream));
-  NPFEM_CUDA(c, cudaStreamWaitEvent(c->h2d_stream, ev_start, 0));
-  NPFEM_CUDA(c, cudaStreamWaitEvent(c->d2h_stream, ev_start, 0));
-  const unsigned char *f_host = static_cast<const unsigned char *>(forces);
-  unsigned char *x_host = static_cast<unsigned char *>(positions), *v_host = static_cast<unsigned char *>(velocities);
-  unsigned char *sa = static_cast<unsigned char *>(c->stage_a), *sb = static_cast<unsigned char *>(c->stage_b),
-                *sc = static_cast<unsigned char *>(c->stage_c);
-  // all copies in are queued first: the copy engine runs ahead of the solver as far as it can
-  for (int i = 0; i < n_chunks; ++i) {
-    const int64_t c0 = c->n_cells * i / n_chunks, c1 = c->n_cells * (i + 1) / n_chunks;
-    const size_t b0 = size_t(c->user_offset_all[c0]) * es, b1 = size_t(c->user_offset_all[c1]) * es;
-    NPFEM_CUDA(c, cudaMemcpyAsync(sc + b0, f_host + b0, b1 - b0, cudaMemcpyHostToDevice, c->h2d_stream));
-    NPFEM_CUDA(c, cudaEventRecord(c->io_events[size_t(i)], c->h2d_stream));
-  }
-  for (int i = 0; i < n_chunks; ++i) {
-    const int64_t c0 = c->n_cells * i / n_chunks, c1 = c->n_cells * (i + 1) / n_chunks;
-    const size_t b0 = size_t(c->user_offset_all[c0]) * es, b1 = size_t(c->user_offset_all[c1]) * es;
-    std::vector<int64_t> count(nb, 0);
-    for (int64_t cell = c0; cell < c1; ++cell) ++count[size_t(c->type_of_cell[cell])];
-    PackArgs a{};
-    a.refs = c->refs_all_dev + c0;
-    a.n_refs = c1 - c0;
-    a.io_dtype = dtype;
-    a.src_a = sc;
-    NPFEM_CUDA(c, cudaStreamWaitEvent(c->stream, c->io_events[size_t(i)], 0));
-    if ((rc = check_launch(c, launch_set_forces(c->views_dev, a, c->precision, c->stream), "set_forces"))) return rc;
-    for (size_t t = 0; t < nb; ++t) {
-      BucketView bv = full_views[t];
-      const size_t shift = size_t(slot0[t]) * 3 * size_t(bv.n_pad) * esize(c->precision);
-      for (int f = 0; f < F_COUNT; ++f)
-        if (bv.field[f]) bv.field[f] = static_cast<unsigned char *>(bv.field[f]) + shift;   // F_XL is null in fp64 contexts
-      bv.origin += slot0[t] * 3;
-      bv.cells = count[t];
-      c->views[t] = bv;
-      c->buckets[t].cells = count[t];
+  // the pipeline proper; on any failure the copy streams are drained before the call returns (the caller's host
+  // buffers must not have copies in flight once it has the error code in hand) and the views are restored
+  auto pipeline = [&]() -> int {
+    // the copy-in stream starts after whatever the caller's stream still has in flight on the staging buffers
+    cudaEvent_t ev_start = c->io_events[size_t(2 * n_chunks)];
+    NPFEM_CUDA(c, cudaEventRecord(ev_start, c->stream));
+    NPFEM_CUDA(c, cudaStreamWaitEvent(c->h2d_stream, ev_start, 0));
+    NPFEM_CUDA(c, cudaStreamWaitEvent(c->d2h_stream, ev_start, 0));
+    const unsigned char *f_host = static_cast<const unsigned char *>(forces);
+    unsigned char *x_host = static_cast<unsigned char *>(positions), *v_host = static_cast<unsigned char *>(velocities);
+    unsigned char *sa = static_cast<unsigned char *>(c->stage_a), *sb = static_cast<unsigned char *>(c->stage_b),
+                  *sc = static_cast<unsigned char *>(c->stage_c);
+    // all copies in are queued first: the copy engine runs ahead of the solver as far as it can
+    for (int i = 0; i < n_chunks; ++i) {
+      const int64_t c0 = c->n_cells * i / n_chunks, c1 = c->n_cells * (i + 1) / n_chunks;
+      const size_t b0 = size_t(c->user_offset_all[c0]) * es, b1 = size_t(c->user_offset_all[c1]) * es;
+      NPFEM_CUDA(c, cudaMemcpyAsync(sc + b0, f_host + b0, b1 - b0, cudaMemcpyHostToDevice, c->h2d_stream));
+      NPFEM_CUDA(c, cudaEventRecord(c->io_events[size_t(i)], c->h2d_stream));
     }
-    const int64_t keep_fused = c->opt_fused_step;
-    c->opt_fused_step = 1;                       // see small_batch above: chunks take the kernels the whole bucket takes
-    rc = npfem_step(c, n_iterations);
-    c->opt_fused_step = keep_fused;
+    for (int i = 0; i < n_chunks; ++i) {
+      const int64_t c0 = c->n_cells * i / n_chunks, c1 = c->n_cells * (i + 1) / n_chunks;
+      const size_t b0 = size_t(c->user_offset_all[c0]) * es, b1 = size_t(c->user_offset_all[c1]) * es;
+      std::vector<int64_t> count(nb, 0);
+      for (int64_t cell = c0; cell < c1; ++cell) ++count[size_t(c->type_of_cell[cell])];
+      PackArgs a{};
+      a.refs = c->refs_all_dev + c0;
+      a.n_refs = c1 - c0;
+      a.io_dtype = dtype;
+      a.src_a = sc;
+      NPFEM_CUDA(c, cudaStreamWaitEvent(c->stream, c->io_events[size_t(i)], 0));
+      if ((rc = check_launch(c, launch_set_forces(c->views_dev, a, c->precision, c->stream), "set_forces"))) return rc;
+      for (size_t t = 0; t < nb; ++t) {
+        BucketView bv = full_views[t];
+        const size_t shift = size_t(slot0[t]) * 3 * size_t(bv.n_pad) * esize(c->precision);
+        for (int f = 0; f < F_COUNT; ++f)
+          if (bv.field[f]) bv.field[f] = static_cast<unsigned char *>(bv.field[f]) + shift;   // F_XL is null in fp64 contexts
+        bv.origin += slot0[t] * 3;
+        bv.cells = count[t];
+        c->views[t] = bv;
+        c->buckets[t].cells = count[t];
+      }
+      const int64_t keep_fused = c->opt_fused_step;
+      c->opt_fused_step = 1;                       // see small_batch above: chunks take the kernels the whole bucket takes
+      rc = npfem_step(c, n_iterations);
+      c->opt_fused_step = keep_fused;
+      restore();
+      if (rc) return rc;
+      for (size_t t = 0; t < nb; ++t) slot0[t] += count[t];
+      PackArgs g{};
+      g.refs = c->refs_all_dev + c0;
+      g.n_refs = c1 - c0;
+      g.io_dtype = dtype;
+      g.dst_a = sa;
+      g.dst_b = sb;
+      if ((rc = check_launch(c, launch_get_state(c->views_dev, g, c->precision, c->stream), "get_state"))) return rc;
+      cudaEvent_t packed = c->io_events[size_t(n_chunks + i)];
+      NPFEM_CUDA(c, cudaEventRecord(packed, c->stream));
+      NPFEM_CUDA(c, cudaStreamWaitEvent(c->d2h_stream, packed, 0));
+      NPFEM_CUDA(c, cudaMemcpyAsync(x_host + b0, sa + b0, b1 - b0, cudaMemcpyDeviceToHost, c->d2h_stream));
+      NPFEM_CUDA(c, cudaMemcpyAsync(v_host + b0, sb + b0, b1 - b0, cudaMemcpyDeviceToHost, c->d2h_stream));
+    }
+    NPFEM_CUDA(c, cudaStreamSynchronize(c->d2h_stream));
+    NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NPFEM_OK;
+  };
+  rc = pipeline();
+  if (rc) {
     restore();
-    if (rc) return rc;
-    for (size_t t = 0; t < nb; ++t) slot0[t] += count[t];
-    PackArgs g{};
-    g.refs = c->refs_all_dev + c0;
-    g.n_refs = c1 - c0;
-    g.io_dtype = dtype;
-    g.dst_a = sa;
-    g.dst_b = sb;
-    if ((rc = check_launch(c, launch_get_state(c->views_dev, g, c->precision, c->stream), "get_state"))) return rc;
-    cudaEvent_t packed = c->io_events[size_t(n_chunks + i)];
-    NPFEM_CUDA(c, cudaEventRecord(packed, c->stream));
-    NPFEM_CUDA(c, cudaStreamWaitEvent(c->d2h_stream, packed, 0));
-    NPFEM_CUDA(c, cudaMemcpyAsync(x_host + b0, sa + b0, b1 - b0, cudaMemcpyDeviceToHost, c->d2h_stream));
-    NPFEM_CUDA(c, cudaMemcpyAsync(v_host + b0, sb + b0, b1 - b0, cudaMemcpyDeviceToHost, c->d2h_stream));
+    cudaStreamSynchronize(c->h2d_stream);
+    cudaStreamSynchronize(c->d2h_stream);
+    cudaStreamSynchronize(c->stream);
+    cudaGetLastError();
   }
-  NPFEM_CUDA(c, cudaStreamSynchronize(c->d2h_stream));
-  NPFEM_CUDA(c, cudaStreamSynchronize(c->stream));
-  return NPFEM_OK;
+  return rc;
 }
 
 int npfem_set_line_search(npfem_ctx *c, int32_t max_halvings, double armijo_c1, double grad_tol) {
