@@ -70,7 +70,8 @@ extern "C" {
                                          the bias TF32 rounding of H~^-1 leaves in the fixed point) */
 #define NPFEM_OPT_LOCAL_STEP_IMPL  3  /* 0 = auto, 1 = generic kernel, 2 = shared-memory persistent kernel,
                                          3 = scheduled kernel (register-resident topology, conflict-free slots),
-                                         4 = large-mesh kernel (chunked corner forces, e.g. 2562-vertex cells) */
+                                         4 = large-mesh kernel (chunked corner forces, e.g. 2562-vertex cells),
+                                         5 = quad kernel (one thread per pair of adjacent triangles, experimental) */
 
 #define NPFEM_OPT_KERNEL_TIMING    4  /* 1: bracket every kernel of npfem_step with CUDA events */
 #define NPFEM_OPT_FORCE_MEDIAN_FILTER 6  /* 1: npfem_set_forces median-filters F_ext over the one-ring of every vertex

@@ -9,6 +9,7 @@
 
 #include "internal.h"
 #include "local_schedule.hpp"
+#include "quad_schedule.hpp"
 
 using namespace npfem;
 
@@ -19,6 +20,7 @@ struct npfem_ctx {
   int64_t n_cells = 0, total_vertices = 0;
   std::vector<HostTypeData> host_types;
   std::vector<LocalSchedule> sched;       // fp32 contexts: scheduled local step, per type (may be invalid)
+  std::vector<QuadSchedule> quad;         // fp32 contexts: quad local step, per type (may be invalid)
   std::vector<TypeDev> types;
   std::vector<Bucket> buckets;            // one per type
   std::vector<BucketView> views;
@@ -33,7 +35,7 @@ struct npfem_ctx {
   size_t ws_bytes = 0;
   bool ws_owned = false, ready = false;
   struct Layout {
-    std::vector<size_t> type_off[19];     // per type: tri, nbr, rest, hinge, corner, vnbr, w, mass, inv_area, Hinv, Hinv_tf32
+    std::vector<size_t> type_off[23];     // per type: tri, nbr, rest, hinge, corner, vnbr, w, mass, inv_area, Hinv, Hinv_tf32
     std::vector<size_t> field_off[F_COUNT], origin_off, cellid_off, scratch_off;
     size_t views_off = 0, refs_all_off = 0, refs_tmp_off = 0, stage_a_off = 0, stage_b_off = 0, stage_c_off = 0, total = 0;
     // create-time arena (the fp64 H~, its inverse and the Newton-Schulz temporaries of ONE type at a time): starts
@@ -202,6 +204,11 @@ void compute_layout(npfem_ctx *c) {
     L.type_off[16][t] = take(sc.valid ? sc.vtx_words.size() * 4 : 0);
     L.type_off[17][t] = take(sc.valid ? sc.vtx_coef.size() * 4 : 0);
     L.type_off[18][t] = take(f32 ? np * np * 4 : 0);   // W_lo
+    const QuadSchedule &qs = c->quad[t];
+    L.type_off[19][t] = take(qs.valid ? qs.quad_words.size() * 4 : 0);
+    L.type_off[20][t] = take(qs.valid ? qs.quad_consts.size() * 4 : 0);
+    L.type_off[21][t] = take(qs.valid ? qs.vtx_words.size() * 4 : 0);
+    L.type_off[22][t] = take(qs.valid ? qs.vtx_coef.size() * 4 : 0);
     L.setup_bytes = std::max(L.setup_bytes, (2 * n * n + invert_spd_tmp_doubles(h.n)) * sizeof(double));
   }
   L.setup_off = off;
@@ -455,6 +462,22 @@ int ensure_ready(npfem_ctx *c) {
       sd.vtx_words = reinterpret_cast<const uint32_t *>(c->ws + L.type_off[16][t]);
       sd.vtx_coef = reinterpret_cast<const float *>(c->ws + L.type_off[17][t]);
     }
+    if (c->quad[t].valid) {
+      const QuadSchedule &qs = c->quad[t];
+      if ((rc = upload_raw(c, L.type_off[19][t], qs.quad_words))) return rc;
+      if ((rc = upload_raw(c, L.type_off[20][t], qs.quad_consts))) return rc;
+      if ((rc = upload_raw(c, L.type_off[21][t], qs.vtx_words))) return rc;
+      if ((rc = upload_raw(c, L.type_off[22][t], qs.vtx_coef))) return rc;
+      SchedDev &qd = d.quad;
+      qd.valid = true;
+      qd.threads = qs.threads; qd.vstride = qs.vstride; qd.tpt = 1; qd.ttri = qs.qthreads; qd.ttri_used = qs.nq; qd.maxv = qs.maxq;
+      qd.n_vslots = qs.n_vslots; qd.n_tslots = qs.n_tslots; qd.n_cslots = qs.n_cslots;
+      qd.vol_lane_bound = qs.vol_lane_bound;
+      qd.tri_words = reinterpret_cast<const uint32_t *>(c->ws + L.type_off[19][t]);
+      qd.tri_consts = reinterpret_cast<const float *>(c->ws + L.type_off[20][t]);
+      qd.vtx_words = reinterpret_cast<const uint32_t *>(c->ws + L.type_off[21][t]);
+      qd.vtx_coef = reinterpret_cast<const float *>(c->ws + L.type_off[22][t]);
+    }
 
     // dense inverse of H~ on the device (fp64), then cast/pad to the compute type.  H~, the inverse and the
     // Newton-Schulz temporaries sit in the create-time arena of the workspace (overlaid by the state fields, which
@@ -618,6 +641,7 @@ int npfem_create(npfem_ctx **out, const npfem_cell_type *types, int32_t n_types,
   try {
     c->host_types.resize(size_t(n_types));
     c->sched.resize(size_t(n_types));
+    c->quad.resize(size_t(n_types));
     c->buckets.resize(size_t(n_types));
     for (int t = 0; t < n_types; ++t) {
       std::string err;
@@ -631,6 +655,7 @@ int npfem_create(npfem_ctx **out, const npfem_cell_type *types, int32_t n_types,
         const HostTypeData &h = c->host_types[t];
         const int tpt = h.T <= 320 ? 1 : 2;
         build_local_schedule(h, types[t].rest_positions, tpt, c->sched[t]);   // may stay invalid
+        if (h.T <= 2 * 640) build_quad_schedule(h, types[t].rest_positions, c->quad[t]);   // may stay invalid
       }
     }
     c->type_of_cell.assign(type_of_cell, type_of_cell + n_cells);
@@ -742,7 +767,7 @@ int npfem_set_option(npfem_ctx *c, int32_t option, int64_t value) {
       c->opt_global_math = value;
       return NPFEM_OK;
     case NPFEM_OPT_LOCAL_STEP_IMPL:
-      if (value < 0 || value > 4) return fail(c, NPFEM_EINVAL, "local-step impl must be 0 ... 4");
+      if (value < 0 || value > 5) return fail(c, NPFEM_EINVAL, "local-step impl must be 0 ... 5");
       c->opt_local_impl = value;
       return NPFEM_OK;
     case NPFEM_OPT_KERNEL_TIMING: c->timing = value != 0; return NPFEM_OK;
@@ -894,13 +919,15 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
       // damping part to it (launch_damping_grad), fp64 contexts take the generic kernel
       const bool f32 = c->precision == NPFEM_F32 &&
                        (!ls_on || size_t(24) * size_t(c->types[t].n) <= size_t(200) * 1024);
-      const bool sched = f32 && (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]);
-      const bool fast = f32 && !sched && (c->opt_local_impl == 0 || c->opt_local_impl == 2) && local_smem_supported(c->types[t]);
-      const bool big = f32 && !sched && !fast && (c->opt_local_impl == 0 || c->opt_local_impl == 4) && local_big_supported(c->types[t]);
-      const bool reduced = sched || fast || big;
+      const bool quad = f32 && c->opt_local_impl == 5 && local_quad_supported(c->types[t]);
+      const bool sched = f32 && !quad && (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]);
+      const bool fast = f32 && !quad && !sched && (c->opt_local_impl == 0 || c->opt_local_impl == 2) && local_smem_supported(c->types[t]);
+      const bool big = f32 && !quad && !sched && !fast && (c->opt_local_impl == 0 || c->opt_local_impl == 4) && local_big_supported(c->types[t]);
+      const bool reduced = quad || sched || fast || big;
       const double d_scale = reduced && !ls_on ? 1.0 - c->types[t].gamma : 1.0;
       const BucketView &lv = c->views[t];
       if ((rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "local step", [&] {
+             if (quad) return launch_local_quad(c->types[t], lv, c->n_sm, c->stream);
              if (sched) return launch_local_sched(c->types[t], lv, c->n_sm, c->stream);
              if (fast) return launch_local_smem(c->types[t], lv, c->n_sm, c->stream);
              if (big) return launch_local_big(c->types[t], lv, c->n_sm, c->stream);

@@ -23,6 +23,7 @@ enum Field { F_X = 0, F_V, F_F, F_B, F_D, F_G, F_XL, F_COUNT };
 struct SchedDev {
   bool valid = false;
   int threads = 0, vstride = 0, tpt = 0, ttri = 0, maxv = 0, n_vslots = 0, n_tslots = 0, n_cslots = 0;
+  int ttri_used = 0;           // quad schedule: number of quads (threads below it own one)
   const uint32_t *tri_words = nullptr;
   const float *tri_consts = nullptr;
   const uint32_t *vtx_words = nullptr;
@@ -45,8 +46,8 @@ inline cudaError_t opt_in_max_dynamic_smem(K kernel) {
 }
 
 struct KernelCache {
-  size_t sched_smem = 0;
-  int sched_per_sm = 0;
+  size_t sched_smem = 0, quad_smem = 0;
+  int sched_per_sm = 0, quad_per_sm = 0;
   int tc_smem = 0;
   bool generic_attr[2] = {false, false}, smem_attr = false, big_attr = false, fused_attr = false, objective_attr = false,
        damping_attr = false;
@@ -77,6 +78,7 @@ struct TypeDev {
   double inertia_coef = 0;           // (1 + h alpha) / h^2, multiplies m_v
   double kappa = 0;
   SchedDev sched;                    // fp32 contexts: scheduled local step (may be invalid)
+  SchedDev quad;                     // fp32 contexts: quad local step (quad_schedule.hpp / local_quad.cu; may be invalid)
   mutable KernelCache cache;
 };
 
@@ -207,6 +209,10 @@ int launch_local_smem(const TypeDev &td, const BucketView &bv, int n_sm, cudaStr
 // reduced-gradient convention as launch_local_smem
 bool local_sched_supported(const TypeDev &td);
 int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
+
+// fp32 quad local step: one thread per pair of adjacent triangles; same reduced-gradient convention
+bool local_quad_supported(const TypeDev &td);
+int launch_local_quad(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
 
 // fp32 reduced-gradient local step for types too large for the scheduled kernel (chunked corner forces)
 bool local_big_supported(const TypeDev &td);
