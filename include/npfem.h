@@ -287,6 +287,34 @@ int npfem_local_schedule_stats(const npfem_cell_type *type, double dt, double *s
 int npfem_probe_fma_peak(void *cuda_stream, int32_t precision, int32_t grid_ctas, int32_t iterations, void *sink_dev,
                          double *flops_out);
 
+/*
+ * The fp64 inverse of one SPD matrix on the device: what npfem_create runs once per cell type on H~ (Eq. (4),
+ * the global step applies H~^-1, constant per type), exposed on its own.  H_dev, Hinv_dev: DEVICE,
+ * row-major [n][n] doubles, caller-owned, must not overlap; the result is symmetrised.  Newton-Schulz iteration
+ * X <- X (2 I - H X), X0 = I / ||H||_inf, to ||I - H X||_F <= 1e-13 sqrt(n) (*residual_out, HOST, may be NULL).  The
+ * call synchronises `cuda_stream` (it reads the residual back every iteration).
+ *
+ * npfem_invert_spd: the 3 n^2 + 32 doubles of scratch come from the caller (tmp_dev: DEVICE, 256-byte aligned,
+ * tmp_bytes >= npfem_invert_spd_tmp_bytes(n)).
+ *
+ * npfem_invert_spd_static: for callers that cannot allocate device memory (CUDA graph capture around the call site,
+ * serving loops, harnesses that forbid cudaMalloc): the scratch is a file-scope `static __device__` array inside the
+ * library, 3 * NPFEM_INVERT_STATIC_MAX_N^2 + 32 doubles = 1.6 MB, which every device that loads the library holds
+ * until the process exits.  n > NPFEM_INVERT_STATIC_MAX_N is refused (NPFEM_EINVAL).  All calls on a device share that
+ * one array: calls that overlap on the GPU (two streams, two host threads) race - serialise them.  Neither entry point
+ * calls cudaMalloc / cudaFree or an allocating library routine.
+ *
+ * Errors (message via npfem_invert_spd_last_error(), per host thread): NPFEM_EINVAL (NULL pointer, n, alignment,
+ * n above the static maximum, non-positive diagonal), NPFEM_ENOMEM (tmp_bytes), NPFEM_ESTATE (no convergence: not SPD
+ * or too ill-conditioned), NPFEM_ECUDA.
+ */
+#define NPFEM_INVERT_STATIC_MAX_N 258
+size_t npfem_invert_spd_tmp_bytes(int32_t n);
+int npfem_invert_spd(const double *H_dev, double *Hinv_dev, int32_t n, void *tmp_dev, size_t tmp_bytes, void *cuda_stream,
+                     double *residual_out);
+int npfem_invert_spd_static(const double *H_dev, double *Hinv_dev, int32_t n, void *cuda_stream, double *residual_out);
+const char *npfem_invert_spd_last_error(void);
+
 /* Message of the last failure on `ctx` (ctx == NULL: of the last failed npfem_create). */
 const char *npfem_last_error(const npfem_ctx *ctx);
 

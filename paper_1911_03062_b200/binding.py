@@ -26,6 +26,7 @@ EXPORTED_SYMBOLS = (
     "npfem_get_kernel_times", "npfem_launch_count", "npfem_last_error", "npfem_version", "npfem_destroy",
     "npfem_local_schedule_stats", "npfem_set_line_search", "npfem_get_step_lengths", "npfem_set_velocity_cap", "npfem_set_collisions",
     "npfem_clear_collisions", "npfem_probe_fma_peak",
+    "npfem_invert_spd_tmp_bytes", "npfem_invert_spd", "npfem_invert_spd_static", "npfem_invert_spd_last_error",
 )
 
 
@@ -115,6 +116,14 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.npfem_local_schedule_stats.restype = C.c_int
     lib.npfem_probe_fma_peak.argtypes = [vp, i32, i32, i32, vp, C.POINTER(C.c_double)]
     lib.npfem_probe_fma_peak.restype = C.c_int
+    lib.npfem_invert_spd_tmp_bytes.argtypes = [i32]
+    lib.npfem_invert_spd_tmp_bytes.restype = sz
+    lib.npfem_invert_spd.argtypes = [vp, vp, i32, vp, sz, vp, C.POINTER(C.c_double)]
+    lib.npfem_invert_spd.restype = C.c_int
+    lib.npfem_invert_spd_static.argtypes = [vp, vp, i32, vp, C.POINTER(C.c_double)]
+    lib.npfem_invert_spd_static.restype = C.c_int
+    lib.npfem_invert_spd_last_error.argtypes = []
+    lib.npfem_invert_spd_last_error.restype = C.c_char_p
     _LIB = lib
     return lib
 
@@ -142,6 +151,52 @@ def local_schedule_stats(cell_type, dt: float) -> dict:
     if rc != 0:
         raise NpfemError(rc, lib.npfem_last_error(None).decode())
     return dict(zip(SCHEDULE_STAT_NAMES, [float(v) for v in out]))
+
+
+INVERT_STATIC_MAX_N = 258        # NPFEM_INVERT_STATIC_MAX_N of include/npfem.h
+
+
+def invert_spd(H, out=None, tmp=None, stream=None):
+    """npfem_invert_spd: fp64 inverse of the SPD matrix H (torch CUDA tensor [n][n], float64, contiguous) with
+    caller-owned scratch `tmp` (torch uint8 CUDA tensor of >= npfem_invert_spd_tmp_bytes(n); torch allocates one if
+    None).  Returns (inverse, residual).  Argument marshalling only."""
+    import torch
+    lib = load_library()
+    n = _check_square_f64(H)
+    out = torch.empty_like(H) if out is None else out
+    need = lib.npfem_invert_spd_tmp_bytes(n)
+    tmp = torch.empty(need, dtype=torch.uint8, device=H.device) if tmp is None else tmp
+    res = C.c_double(0.0)
+    st = torch.cuda.current_stream(H.device) if stream is None else stream
+    rc = lib.npfem_invert_spd(C.c_void_p(H.data_ptr()), C.c_void_p(out.data_ptr()), n, C.c_void_p(tmp.data_ptr()), tmp.numel(),
+                              C.c_void_p(st.cuda_stream), C.byref(res))
+    if rc != 0:
+        raise NpfemError(rc, lib.npfem_invert_spd_last_error().decode())
+    return out, res.value
+
+
+def invert_spd_static(H, out, stream=None):
+    """npfem_invert_spd_static: the same inverse with the library's static device scratch (n <= INVERT_STATIC_MAX_N):
+    no device allocation on this path, `out` is the caller's.  Returns the residual.  Calls that overlap on the GPU
+    race on the shared scratch."""
+    import torch
+    lib = load_library()
+    n = _check_square_f64(H)
+    _check_square_f64(out)
+    res = C.c_double(0.0)
+    st = torch.cuda.current_stream(H.device) if stream is None else stream
+    rc = lib.npfem_invert_spd_static(C.c_void_p(H.data_ptr()), C.c_void_p(out.data_ptr()), n, C.c_void_p(st.cuda_stream),
+                                     C.byref(res))
+    if rc != 0:
+        raise NpfemError(rc, lib.npfem_invert_spd_last_error().decode())
+    return res.value
+
+
+def _check_square_f64(H) -> int:
+    import torch
+    if not (H.is_cuda and H.dtype == torch.float64 and H.dim() == 2 and H.shape[0] == H.shape[1] and H.is_contiguous()):
+        raise ValueError("expected a contiguous float64 CUDA tensor [n][n]")
+    return int(H.shape[0])
 
 
 class Solver:
