@@ -53,7 +53,7 @@ def parse_args():
 
 
 NCU_RAW = {   # kernel of the bench line -> committed raw export of ONE launch of it on the bench workload
-    "local:RBC-642": "r2_ncu_local_sched_rbc642_raw.csv",
+    "local:RBC-642": "r2_ncu_local_quad_rbc642_raw.csv",     # the default (quad) kernel; r2_ncu_local_sched_* = --local-impl 3
     "global:RBC-642": "r2_ncu_global_tcgen05_rbc642_raw.csv",
 }
 NCU_WORKLOAD = {"cells": 100000, "precision": "fp32"}   # what the exports were captured on (profiles/r2_ncu.md)

@@ -71,7 +71,8 @@ extern "C" {
 #define NPFEM_OPT_LOCAL_STEP_IMPL  3  /* 0 = auto, 1 = generic kernel, 2 = shared-memory persistent kernel,
                                          3 = scheduled kernel (register-resident topology, conflict-free slots),
                                          4 = large-mesh kernel (chunked corner forces, e.g. 2562-vertex cells),
-                                         5 = quad kernel (one thread per pair of adjacent triangles, experimental) */
+                                         5 = quad kernel (one thread per pair of adjacent triangles).  auto = 5 where the type
+                                         allows it, else 3, else 2, else 4, else 1 */
 
 #define NPFEM_OPT_KERNEL_TIMING    4  /* 1: bracket every kernel of npfem_step with CUDA events */
 #define NPFEM_OPT_FORCE_MEDIAN_FILTER 6  /* 1: npfem_set_forces median-filters F_ext over the one-ring of every vertex
@@ -276,6 +277,20 @@ int64_t npfem_launch_count(const npfem_ctx *ctx);
  * Returns NPFEM_OK, NPFEM_EINVAL or NPFEM_EMESH (message via npfem_last_error(NULL)).
  */
 int npfem_local_schedule_stats(const npfem_cell_type *type, double dt, double *stats, int32_t n_stats);
+
+/*
+ * The same for the schedule of the QUAD local step (one thread per pair of adjacent triangles T0 = (p, q, r),
+ * T1 = (p, s, q); the default fp32 local step of types with an even triangle count <= 1,280): host-only.
+ *   [0] 1 if the type takes the quad kernel (a perfect matching of the dual graph exists and it fits), else 0
+ *   [1] CTA threads (= quad slots, one vertex per thread)   [2] corner-force reads per vertex (6 or 8)
+ *   [3] predicted wavefronts per vertex-gather instruction   [4] per normal-gather instruction   (ideal 4.0)
+ *   [5] / [6] worst wavefronts of a corner-force STORE / GATHER instruction quarter (exactly 1.0 expected)
+ *   [7] 1 if the tables decode to the mesh's own connectivity: every triangle in exactly one quad, both triangles of a
+ *       quad adjacent across p-q and correctly oriented, the four neighbour-normal slots those of the triangles across
+ *       q-r, r-p, p-s, s-q, every slot unique, every vertex reading exactly the corner slots written for it; else 0
+ *   [8] shared-memory bytes of the kernel's per-cell arrays  [9] host milliseconds to build
+ */
+int npfem_quad_schedule_stats(const npfem_cell_type *type, double dt, double *stats, int32_t n_stats);
 
 /*
  * Measurement aid (not on the solver's path; SURVEY.md 8(d) "measure an FFMA peak on the box"): enqueues on

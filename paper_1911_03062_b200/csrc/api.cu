@@ -919,7 +919,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
       // damping part to it (launch_damping_grad), fp64 contexts take the generic kernel
       const bool f32 = c->precision == NPFEM_F32 &&
                        (!ls_on || size_t(24) * size_t(c->types[t].n) <= size_t(200) * 1024);
-      const bool quad = f32 && c->opt_local_impl == 5 && local_quad_supported(c->types[t]);
+      const bool quad = f32 && (c->opt_local_impl == 0 || c->opt_local_impl == 5) && local_quad_supported(c->types[t]);
       const bool sched = f32 && !quad && (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]);
       const bool fast = f32 && !quad && !sched && (c->opt_local_impl == 0 || c->opt_local_impl == 2) && local_smem_supported(c->types[t]);
       const bool big = f32 && !quad && !sched && !fast && (c->opt_local_impl == 0 || c->opt_local_impl == 4) && local_big_supported(c->types[t]);
@@ -1317,6 +1317,120 @@ int npfem_local_schedule_stats(const npfem_cell_type *type, double dt, double *s
     ok &= reads == corner_slots[v];
   }
   (void)vwords;
+  stats[5] = worst_store;
+  stats[6] = worst_gather;
+  stats[7] = ok ? 1 : 0;
+  return NPFEM_OK;
+}
+
+int npfem_quad_schedule_stats(const npfem_cell_type *type, double dt, double *stats, int32_t n_stats) {
+  if (!type || !stats || n_stats < 10 || !(dt > 0)) return fail(nullptr, NPFEM_EINVAL, "type/stats missing, n_stats < 10 or dt <= 0");
+  std::fill(stats, stats + n_stats, 0.0);
+  HostTypeData h;
+  std::string err;
+  const int rc = build_host_type(*type, dt, h, err);
+  if (rc != NPFEM_OK) return fail(nullptr, rc, err);
+  QuadSchedule qs;
+  const auto t0 = std::chrono::steady_clock::now();
+  if (!build_quad_schedule(h, type->rest_positions, qs)) return NPFEM_OK;
+  stats[9] = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  stats[0] = 1;
+  stats[1] = qs.threads;
+  stats[2] = qs.maxq;
+  stats[3] = qs.wf_vertex;
+  stats[4] = qs.wf_normal;
+  stats[8] = double(qs.n_vslots + qs.n_tslots + qs.n_cslots) * 16.0;
+  // ---- decode the tables and check them against the mesh's own connectivity (nothing of the builder is reused) ----
+  auto lo = [](uint32_t w) { return int(w & 0xffffu) / 16; };
+  auto hi = [](uint32_t w) { return int(w >> 16) / 16; };
+  bool ok = qs.nq * 2 == h.T;
+  std::vector<int> vertex_of_slot(size_t(qs.n_vslots), -1);
+  for (int v = 0; v < h.n; ++v) {
+    const int sl = lo(qs.vtx_words[v]);
+    ok &= sl < qs.n_vslots && vertex_of_slot[sl] < 0;
+    if (sl < qs.n_vslots) vertex_of_slot[sl] = v;
+  }
+  // directed edge (a, b) -> the triangle that runs a -> b (closed oriented manifold: exactly one)
+  std::vector<int> tri_of_edge(size_t(h.n) * h.n, -1);
+  for (int t = 0; t < h.T; ++t)
+    for (int k = 0; k < 3; ++k) tri_of_edge[size_t(h.tri[4 * t + k]) * h.n + h.tri[4 * t + (k + 1) % 3]] = t;
+  auto tri_at = [&](int a, int b) { return a >= 0 && b >= 0 ? tri_of_edge[size_t(a) * h.n + b] : -1; };
+  auto W = [&](int k, int q) { return qs.quad_words[size_t(q) * qs.threads + k]; };
+  std::vector<int> quad_of_tri(size_t(h.T), -1), tslot_of_tri(size_t(h.T), -1), seen_t(size_t(qs.n_tslots), 0),
+      seen_c(size_t(qs.n_cslots), 0);
+  std::vector<std::vector<int>> corner_slots(size_t(h.n));
+  struct Dec { int p, q, r, s, A, B; };
+  std::vector<Dec> dec(size_t(qs.nq), Dec{-1, -1, -1, -1, -1, -1});
+  for (int k = 0; k < qs.nq && ok; ++k) {
+    const int sl[4] = {lo(W(k, 0)), hi(W(k, 0)), lo(W(k, 1)), hi(W(k, 1))};
+    int v[4];
+    for (int i = 0; i < 4; ++i) v[i] = sl[i] < qs.n_vslots ? vertex_of_slot[sl[i]] : -1;
+    Dec &d = dec[k];
+    d.p = v[0]; d.q = v[1]; d.r = v[2]; d.s = v[3];
+    d.A = tri_at(d.p, d.q);                     // T0 = (p, q, r)
+    d.B = tri_at(d.q, d.p);                     // T1 = (p, s, q)
+    ok &= d.A >= 0 && d.B >= 0 && d.A != d.B && tri_at(d.q, d.r) == d.A && tri_at(d.r, d.p) == d.A &&
+          tri_at(d.p, d.s) == d.B && tri_at(d.s, d.q) == d.B;
+    if (!ok) break;
+    ok &= quad_of_tri[d.A] < 0 && quad_of_tri[d.B] < 0;
+    quad_of_tri[d.A] = quad_of_tri[d.B] = k;
+    const int ta = lo(W(k, 4)), tb = hi(W(k, 4));
+    ok &= ta < qs.n_tslots && tb < qs.n_tslots && ta != tb && !seen_t[ta]++ && !seen_t[tb]++;
+    tslot_of_tri[d.A] = ta;
+    tslot_of_tri[d.B] = tb;
+    const int cs[4] = {lo(W(k, 5)), hi(W(k, 5)), lo(W(k, 6)), hi(W(k, 6))};
+    for (int i = 0; i < 4; ++i) {
+      ok &= cs[i] < qs.n_cslots - 8 && !seen_c[cs[i]]++;
+      corner_slots[v[i]].push_back(cs[i]);
+    }
+  }
+  for (int t = 0; t < h.T; ++t) ok &= quad_of_tri[t] >= 0;
+  // neighbour normals across the four outer edges q-r, r-p (of T0), p-s, s-q (of T1)
+  for (int k = 0; k < qs.nq && ok; ++k) {
+    const Dec &d = dec[k];
+    const int ns[4] = {lo(W(k, 2)), hi(W(k, 2)), lo(W(k, 3)), hi(W(k, 3))};
+    const int nb[4] = {tri_at(d.r, d.q), tri_at(d.p, d.r), tri_at(d.s, d.p), tri_at(d.q, d.s)};
+    for (int i = 0; i < 4; ++i) ok &= nb[i] >= 0 && ns[i] == tslot_of_tri[nb[i]];
+  }
+  // stores: quarter warps of 8 consecutive quad threads, per corner role (one STS.128 each)
+  double worst_store = 0, worst_gather = 0;
+  for (int k0 = 0; k0 < qs.nq; k0 += 8)
+    for (int role = 0; role < 4; ++role) {
+      int mult[8] = {0, 0, 0, 0, 0, 0, 0, 0}, w = 0;
+      for (int k = k0; k < std::min(k0 + 8, qs.nq); ++k) {
+        const uint32_t word = W(k, 5 + role / 2);
+        w = std::max(w, ++mult[((role & 1) ? hi(word) : lo(word)) % 8]);
+      }
+      worst_store = std::max(worst_store, double(w));
+    }
+  // gathers: quarter warps of 8 consecutive vertices, per read position; a vertex reads exactly the slots its quads
+  // write for it (any order) and zero slots otherwise
+  auto read_slot = [&](int v, int k) {
+    const uint32_t w = qs.vtx_words[size_t(1 + k / 2) * qs.vstride + v];
+    return (k & 1) ? hi(w) : lo(w);
+  };
+  for (int v0 = 0; v0 < h.n; v0 += 8)
+    for (int k = 0; k < qs.maxq; ++k) {
+      int mult[8] = {0, 0, 0, 0, 0, 0, 0, 0}, w = 0;
+      std::vector<int> slots;
+      for (int v = v0; v < std::min(v0 + 8, h.n); ++v) {
+        const int sl = read_slot(v, k);
+        if (std::find(slots.begin(), slots.end(), sl) == slots.end()) w = std::max(w, ++mult[sl % 8]);
+        slots.push_back(sl);
+      }
+      worst_gather = std::max(worst_gather, double(w));
+    }
+  for (int v = 0; v < h.n; ++v) {
+    std::vector<int> reads;
+    for (int k = 0; k < qs.maxq; ++k) {
+      const int sl = read_slot(v, k);
+      if (sl < qs.n_cslots - 8) reads.push_back(sl);
+      else ok &= sl < qs.n_cslots;
+    }
+    std::sort(reads.begin(), reads.end());
+    std::sort(corner_slots[v].begin(), corner_slots[v].end());
+    ok &= reads == corner_slots[v];
+  }
   stats[5] = worst_store;
   stats[6] = worst_gather;
   stats[7] = ok ? 1 : 0;

@@ -204,11 +204,12 @@ def test_tf32_tensor_core_global_step_vs_fp32_ffma():
         assert rel_l2(d_tf32, d_ref) < 1.1e-4 and rel_l2(d_ffma, d_ref) < 1e-4
 
 
-@pytest.mark.parametrize("impl", [1, 2, 3])
+@pytest.mark.parametrize("impl", [1, 2, 3, 5])
 def test_fp32_local_step_implementations(impl):
     """Every fp32 local-step kernel (1 generic, 2 shared-memory tables, 3 scheduled: register-resident
-    topology + colour-assigned conflict-free slots) against the oracle; RBC-642 exercises the second
-    vertex pass of the scheduled kernel (642 vertices on 640 threads)."""
+    topology + colour-assigned conflict-free slots, 5 quad: one thread per pair of adjacent triangles, the default
+    where the type allows it) against the oracle; RBC-642 exercises the second vertex pass of the scheduled and quad
+    kernels (642 vertices on 640 threads)."""
     from paper_1911_03062_b200 import binding
     pop = make_config(3, n_cells=300)         # 273 RBC + 27 PLT: more cells than one wave of CTAs for PLT
     gpu, solver = run_gpu(pop, "fp32", n_steps=3, n_iterations=5, options=[(binding.OPT_LOCAL_STEP_IMPL, impl)])
@@ -220,7 +221,7 @@ def test_fp32_local_step_implementations(impl):
         assert_row(r, "fp32", (1.3e-4, 1.3e-3, 4.3e-3, 1.8e-4))
 
 
-@pytest.mark.parametrize("precision,impl", [("fp64", 0), ("fp32", 1), ("fp32", 3)])
+@pytest.mark.parametrize("precision,impl", [("fp64", 0), ("fp32", 1), ("fp32", 3), ("fp32", 5)])
 def test_irregular_mesh_valence_up_to_8(precision, impl):
     """A mesh that is not an icosphere (flipped edges, valences 4..8): generic kernels and the
     8-read variant of the scheduled kernel against the oracle."""

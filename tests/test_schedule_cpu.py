@@ -49,3 +49,31 @@ def test_schedule_is_deterministic():
     a, b = local_schedule_stats(rbc_cell_type(2), 0.1), local_schedule_stats(rbc_cell_type(2), 0.1)
     a.pop("build_ms"), b.pop("build_ms")
     assert a == b
+
+
+# ---- quad local step (one thread per pair of adjacent triangles; csrc/quad_schedule.hpp) --------------------------
+from paper_1911_03062_b200.binding import quad_schedule_stats  # noqa: E402
+
+
+@pytest.mark.parametrize("make,threads", [(lambda: rbc_cell_type(3), 640), (lambda: platelet_cell_type(2), 160),
+                                          (lambda: rbc_cell_type(3, base="octa"), 256),
+                                          (lambda: platelet_cell_type(2, base="octa"), 64)])
+def test_quad_schedule_of_the_baseline_and_paper_cell_types(make, threads):
+    """A perfect matching of the dual graph exists for these meshes (T even, bridgeless cubic graph: Petersen), the
+    tables decode to the mesh's connectivity, and the corner-force traffic is conflict-free."""
+    st = quad_schedule_stats(make(), 0.1)
+    assert st["valid"] == 1 and st["threads"] == threads and st["consistent"] == 1
+    assert st["reads_per_vertex"] == 6                      # every vertex lies in at most 6 quads (of its <= 6 triangles)
+    assert st["worst_store_quarter"] == 1 and st["worst_gather_quarter"] == 1
+    assert 4.0 <= st["wf_vertex_gather"] <= 6.0 and 4.0 <= st["wf_normal_gather"] <= 6.0
+    assert st["smem_bytes"] < 100 * 1024
+
+
+def test_quad_schedule_irregular_mesh_and_rejections():
+    st = quad_schedule_stats(irregular_cell_type(2, 40, seed=3), 0.1)       # valence up to 8
+    assert st["valid"] == 1 and st["consistent"] == 1
+    assert st["worst_store_quarter"] == 1 and st["worst_gather_quarter"] == 1
+    assert quad_schedule_stats(rbc_cell_type(4), 0.1)["valid"] == 0          # 5,120 triangles: other kernels
+    a, b = quad_schedule_stats(rbc_cell_type(2), 0.1), quad_schedule_stats(rbc_cell_type(2), 0.1)
+    a.pop("build_ms"), b.pop("build_ms")
+    assert a == b                                                            # deterministic
