@@ -767,7 +767,7 @@ int npfem_set_option(npfem_ctx *c, int32_t option, int64_t value) {
       c->opt_global_math = value;
       return NPFEM_OK;
     case NPFEM_OPT_LOCAL_STEP_IMPL:
-      if (value < 0 || value > 6) return fail(c, NPFEM_EINVAL, "local-step impl must be 0 ... 6");
+      if (value < 0 || value > 5) return fail(c, NPFEM_EINVAL, "local-step impl must be 0 ... 5");
       c->opt_local_impl = value;
       return NPFEM_OK;
     case NPFEM_OPT_KERNEL_TIMING: c->timing = value != 0; return NPFEM_OK;
@@ -919,16 +919,14 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
       // damping part to it (launch_damping_grad), fp64 contexts take the generic kernel
       const bool f32 = c->precision == NPFEM_F32 &&
                        (!ls_on || size_t(24) * size_t(c->types[t].n) <= size_t(200) * 1024);
-      const bool ws = f32 && c->opt_local_impl == 6 && local_ws_supported(c->types[t]);
-      const bool quad = f32 && !ws && (c->opt_local_impl == 0 || c->opt_local_impl == 5) && local_quad_supported(c->types[t]);
+      const bool quad = f32 && (c->opt_local_impl == 0 || c->opt_local_impl == 5) && local_quad_supported(c->types[t]);
       const bool sched = f32 && !quad && (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]);
       const bool fast = f32 && !quad && !sched && (c->opt_local_impl == 0 || c->opt_local_impl == 2) && local_smem_supported(c->types[t]);
       const bool big = f32 && !quad && !sched && !fast && (c->opt_local_impl == 0 || c->opt_local_impl == 4) && local_big_supported(c->types[t]);
-      const bool reduced = ws || quad || sched || fast || big;
+      const bool reduced = quad || sched || fast || big;
       const double d_scale = reduced && !ls_on ? 1.0 - c->types[t].gamma : 1.0;
       const BucketView &lv = c->views[t];
       if ((rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "local step", [&] {
-             if (ws) return launch_local_ws(c->types[t], lv, c->n_sm, c->stream);
              if (quad) return launch_local_quad(c->types[t], lv, c->n_sm, c->stream);
              if (sched) return launch_local_sched(c->types[t], lv, c->n_sm, c->stream);
              if (fast) return launch_local_smem(c->types[t], lv, c->n_sm, c->stream);

@@ -46,7 +46,7 @@ inline cudaError_t opt_in_max_dynamic_smem(K kernel) {
 }
 
 struct KernelCache {
-  size_t sched_smem = 0, quad_smem = 0, ws_smem = 0;
+  size_t sched_smem = 0, quad_smem = 0;
   int sched_per_sm = 0, quad_per_sm = 0;
   int tc_smem = 0;
   bool generic_attr[2] = {false, false}, smem_attr = false, big_attr = false, fused_attr = false, objective_attr = false,
@@ -213,9 +213,6 @@ int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, cudaSt
 // fp32 quad local step: one thread per pair of adjacent triangles; same reduced-gradient convention
 bool local_quad_supported(const TypeDev &td);
 int launch_local_quad(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
-// the same arithmetic, warp-specialised (quad warps + vertex warps, local_ws.cu): types whose quad schedule has 640 threads
-bool local_ws_supported(const TypeDev &td);
-int launch_local_ws(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
 
 // fp32 reduced-gradient local step for types too large for the scheduled kernel (chunked corner forces)
 bool local_big_supported(const TypeDev &td);
