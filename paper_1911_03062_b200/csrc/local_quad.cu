@@ -145,8 +145,8 @@ __global__ void __launch_bounds__(MAXT, MINB) local_quad_kernel(const QuadParams
     uint32_t done;
     do {
       asm volatile(
-          "{\n.reg .pred q;\nmbarrier.try_wait.parity.shared::cta.b64 q, [%1], %2;\nselp.u32 %0, 1, 0, q;\n}\n"
-          : "=r"(done) : "r"(smem_u32(bars + which)), "r"(parity) : "memory");
+          "{\n.reg .pred q;\nmbarrier.try_wait.parity.shared::cta.b64 q, [%1], %2, %3;\nselp.u32 %0, 1, 0, q;\n}\n"
+          : "=r"(done) : "r"(smem_u32(bars + which)), "r"(parity), "r"(20000u) : "memory");   // suspend-time hint, ns
     } while (!done);
   };
   // phase 0 of this CTA's it0-th cell (ring slot it0 % NSTAGE): sx[slot(v)] = (x + (xl + d), 0), the current
@@ -295,17 +295,7 @@ __global__ void __launch_bounds__(MAXT, MINB) local_quad_kernel(const QuadParams
       r22 = fmaf(W2, ff, W1 * R22);
       r12 = fmaf(-W2, fe, W1 * R12);
     }
-    bar_wait(1, par);                                  // B2: sN complete
-    if (tid == 0) {
-      // every thread is past phase C of the previous cell: its ring slot and the other volume
-      // accumulator are free
-      vacc[2 * ((it + 1) & 1)] = vacc[2 * ((it + 1) & 1) + 1] = 0;
-      const int64_t nxt = cell + int64_t(NSTAGE - 1) * gridDim.x;
-      if (nxt < p.cells) prefetch(nxt, (it + NSTAGE - 1) % NSTAGE);
-    }
-    // ---- phase B ----------------------------------------------------------------------------
-    // the four neighbour normals first (independent loads in flight together), then the five hinges
-    const float4 NB0 = lds4(sN, lo16(qw[2])), NB1 = lds4(sN, hi16(qw[2])), NB2 = lds4(sN, lo16(qw[3])), NB3 = lds4(sN, hi16(qw[3]));
+    // the shared hinge needs this thread's own two normals only: it too runs ahead of the wait for B2
     // hinge weights on the corners of T0 = (p, q, r): w0..w2, and of T1 = (p, s, q): z0..z2 (reading R8; side k of a
     // triangle with edges (a1, a2) runs from corner k to k+1: a1, a2 - a1, -a2)
     float w0, w1, w2, z0, z1, z2;
@@ -319,6 +309,17 @@ __global__ void __launch_bounds__(MAXT, MINB) local_quad_kernel(const QuadParams
       w0 = D * q; w1 = (L - D) * q; w2 = -L * q;
       z2 = fe * q; z0 = (L - fe) * q; z1 = -L * q;               // T1, side 2: L = |a2|^2 = e11, D = a1 . a2 = fe
     }
+    bar_wait(1, par);                                  // B2: sN complete
+    if (tid == 0) {
+      // every thread is past phase C of the previous cell: its ring slot and the other volume
+      // accumulator are free
+      vacc[2 * ((it + 1) & 1)] = vacc[2 * ((it + 1) & 1) + 1] = 0;
+      const int64_t nxt = cell + int64_t(NSTAGE - 1) * gridDim.x;
+      if (nxt < p.cells) prefetch(nxt, (it + NSTAGE - 1) % NSTAGE);
+    }
+    // ---- phase B ----------------------------------------------------------------------------
+    // the four neighbour normals first (independent loads in flight together), then the five hinges
+    const float4 NB0 = lds4(sN, lo16(qw[2])), NB1 = lds4(sN, hi16(qw[2])), NB2 = lds4(sN, lo16(qw[3])), NB3 = lds4(sN, hi16(qw[3]));
     {   // T0 side 1: q -> r, neighbour NB0
       const float4 B = NB0;
       const float crx = n0[1] * B.z - n0[2] * B.y, cry = n0[2] * B.x - n0[0] * B.z, crz = n0[0] * B.y - n0[1] * B.x;
