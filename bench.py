@@ -40,7 +40,7 @@ def parse_args():
     ap.add_argument("--iterations", type=int, default=None, help="solver iterations per step")
     ap.add_argument("--precision", default="fp32", choices=["fp32", "fp64"])
     ap.add_argument("--global-math", default="tf32", choices=["tf32", "fp32", "tf32x2"])
-    ap.add_argument("--local-impl", type=int, default=0, choices=[0, 1, 2, 3, 4, 5])
+    ap.add_argument("--local-impl", type=int, default=0, choices=[0, 1, 2, 3, 4, 5, 6])
     ap.add_argument("--line-search", type=int, default=0, help="Armijo backtracking with this many halvings (0 = off)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-chunks", type=int, default=0, help="npfem_step_host chunks (0 = library's choice, 1 = unpipelined)")

@@ -71,8 +71,9 @@ extern "C" {
 #define NPFEM_OPT_LOCAL_STEP_IMPL  3  /* 0 = auto, 1 = generic kernel, 2 = shared-memory persistent kernel,
                                          3 = scheduled kernel (register-resident topology, conflict-free slots),
                                          4 = large-mesh kernel (chunked corner forces, e.g. 2562-vertex cells),
-                                         5 = quad kernel (one thread per pair of adjacent triangles).  auto = 5 where the type
-                                         allows it, else 3, else 2, else 4, else 1 */
+                                         5 = quad kernel (one thread per pair of adjacent triangles),
+                                         6 = multi-pass quad kernel (meshes of 1,282 ... 5,120 triangles).  auto = 5 where the
+                                         type allows it, else 6, else 3, else 2, else 4, else 1 */
 
 #define NPFEM_OPT_KERNEL_TIMING    4  /* 1: bracket every kernel of npfem_step with CUDA events */
 #define NPFEM_OPT_FORCE_MEDIAN_FILTER 6  /* 1: npfem_set_forces median-filters F_ext over the one-ring of every vertex
@@ -291,6 +292,13 @@ int npfem_local_schedule_stats(const npfem_cell_type *type, double dt, double *s
  *   [8] shared-memory bytes of the kernel's per-cell arrays  [9] host milliseconds to build
  */
 int npfem_quad_schedule_stats(const npfem_cell_type *type, double dt, double *stats, int32_t n_stats);
+
+/*
+ * The same for the MULTI-PASS quad local step (meshes of 1,282 ... 5,120 triangles, e.g. RBC-2562: the quads in up to 4
+ * passes of 640, one quad per thread and pass): [1] = passes, the rest as for npfem_quad_schedule_stats; [7] also checks
+ * that every pass's vertex list names each vertex the pass touches exactly once with exactly the slots written for it.
+ */
+int npfem_quadmp_schedule_stats(const npfem_cell_type *type, double dt, double *stats, int32_t n_stats);
 
 /*
  * Measurement aid (not on the solver's path; SURVEY.md 8(d) "measure an FFMA peak on the box"): enqueues on

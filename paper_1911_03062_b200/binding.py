@@ -26,7 +26,7 @@ EXPORTED_SYMBOLS = (
     "npfem_get_kernel_times", "npfem_launch_count", "npfem_last_error", "npfem_version", "npfem_destroy",
     "npfem_local_schedule_stats", "npfem_set_line_search", "npfem_get_step_lengths", "npfem_set_velocity_cap", "npfem_set_collisions",
     "npfem_clear_collisions", "npfem_probe_fma_peak",
-    "npfem_quad_schedule_stats", "npfem_invert_spd_tmp_bytes", "npfem_invert_spd", "npfem_invert_spd_static", "npfem_invert_spd_last_error",
+    "npfem_quad_schedule_stats", "npfem_quadmp_schedule_stats", "npfem_invert_spd_tmp_bytes", "npfem_invert_spd", "npfem_invert_spd_static", "npfem_invert_spd_last_error",
 )
 
 
@@ -116,6 +116,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.npfem_local_schedule_stats.restype = C.c_int
     lib.npfem_quad_schedule_stats.argtypes = [C.POINTER(_CellType), C.c_double, C.POINTER(C.c_double), i32]
     lib.npfem_quad_schedule_stats.restype = C.c_int
+    lib.npfem_quadmp_schedule_stats.argtypes = [C.POINTER(_CellType), C.c_double, C.POINTER(C.c_double), i32]
+    lib.npfem_quadmp_schedule_stats.restype = C.c_int
     lib.npfem_probe_fma_peak.argtypes = [vp, i32, i32, i32, vp, C.POINTER(C.c_double)]
     lib.npfem_probe_fma_peak.restype = C.c_int
     lib.npfem_invert_spd_tmp_bytes.argtypes = [i32]
@@ -159,16 +161,18 @@ QUAD_STAT_NAMES = ("valid", "threads", "reads_per_vertex", "wf_vertex_gather", "
                    "worst_gather_quarter", "consistent", "smem_bytes", "build_ms")
 
 
-def quad_schedule_stats(cell_type, dt: float) -> dict:
-    """npfem_quad_schedule_stats (host-only): the create-time schedule of the quad local step, decoded and checked
-    against the mesh by the library."""
+def quad_schedule_stats(cell_type, dt: float, multipass: bool = False) -> dict:
+    """npfem_quad_schedule_stats / npfem_quadmp_schedule_stats (host-only): the create-time schedule of the quad local
+    step (multipass: of its multi-pass variant; "threads" is then the number of passes), decoded and checked against
+    the mesh by the library."""
     lib = load_library()
     rest = np.ascontiguousarray(cell_type.rest_positions, dtype=np.float64)
     tri = np.ascontiguousarray(cell_type.triangles, dtype=np.int32)
     ct = _CellType(rest.shape[0], tri.shape[0], rest.ctypes.data_as(C.POINTER(C.c_double)),
                    tri.ctypes.data_as(C.POINTER(C.c_int32)), _material_struct(cell_type.material))
     out = (C.c_double * len(QUAD_STAT_NAMES))()
-    rc = lib.npfem_quad_schedule_stats(C.byref(ct), float(dt), out, len(QUAD_STAT_NAMES))
+    fn = lib.npfem_quadmp_schedule_stats if multipass else lib.npfem_quad_schedule_stats
+    rc = fn(C.byref(ct), float(dt), out, len(QUAD_STAT_NAMES))
     if rc != 0:
         raise NpfemError(rc, lib.npfem_last_error(None).decode())
     return dict(zip(QUAD_STAT_NAMES, [float(v) for v in out]))

@@ -10,6 +10,7 @@
 #include "internal.h"
 #include "local_schedule.hpp"
 #include "quad_schedule.hpp"
+#include "quadmp_schedule.hpp"
 
 using namespace npfem;
 
@@ -21,6 +22,7 @@ struct npfem_ctx {
   std::vector<HostTypeData> host_types;
   std::vector<LocalSchedule> sched;       // fp32 contexts: scheduled local step, per type (may be invalid)
   std::vector<QuadSchedule> quad;         // fp32 contexts: quad local step, per type (may be invalid)
+  std::vector<QuadMpSchedule> quadmp;     // fp32 contexts: multi-pass quad local step of larger meshes (may be invalid)
   std::vector<TypeDev> types;
   std::vector<Bucket> buckets;            // one per type
   std::vector<BucketView> views;
@@ -35,7 +37,7 @@ struct npfem_ctx {
   size_t ws_bytes = 0;
   bool ws_owned = false, ready = false;
   struct Layout {
-    std::vector<size_t> type_off[23];     // per type: tri, nbr, rest, hinge, corner, vnbr, w, mass, inv_area, Hinv, Hinv_tf32
+    std::vector<size_t> type_off[28];     // per type: tri, nbr, rest, hinge, corner, vnbr, w, mass, inv_area, Hinv, Hinv_tf32
     std::vector<size_t> field_off[F_COUNT], origin_off, cellid_off, scratch_off;
     size_t views_off = 0, refs_all_off = 0, refs_tmp_off = 0, stage_a_off = 0, stage_b_off = 0, stage_c_off = 0, total = 0;
     // create-time arena (the fp64 H~, its inverse and the Newton-Schulz temporaries of ONE type at a time): starts
@@ -209,6 +211,12 @@ void compute_layout(npfem_ctx *c) {
     L.type_off[20][t] = take(qs.valid ? qs.quad_consts.size() * 4 : 0);
     L.type_off[21][t] = take(qs.valid ? qs.vtx_words.size() * 4 : 0);
     L.type_off[22][t] = take(qs.valid ? qs.vtx_coef.size() * 4 : 0);
+    const QuadMpSchedule &qm = c->quadmp[t];
+    L.type_off[23][t] = take(qm.valid ? qm.quad_words.size() * 4 : 0);
+    L.type_off[24][t] = take(qm.valid ? qm.quad_consts.size() * 4 : 0);
+    L.type_off[25][t] = take(qm.valid ? qm.list_words.size() * 4 : 0);
+    L.type_off[26][t] = take(qm.valid ? qm.vtx_slot.size() * 4 : 0);
+    L.type_off[27][t] = take(qm.valid ? qm.vtx_coef.size() * 4 : 0);
     L.setup_bytes = std::max(L.setup_bytes, (2 * n * n + invert_spd_tmp_doubles(h.n)) * sizeof(double));
   }
   L.setup_off = off;
@@ -478,6 +486,25 @@ int ensure_ready(npfem_ctx *c) {
       qd.vtx_words = reinterpret_cast<const uint32_t *>(c->ws + L.type_off[21][t]);
       qd.vtx_coef = reinterpret_cast<const float *>(c->ws + L.type_off[22][t]);
     }
+    if (c->quadmp[t].valid) {
+      const QuadMpSchedule &qm = c->quadmp[t];
+      if ((rc = upload_raw(c, L.type_off[23][t], qm.quad_words))) return rc;
+      if ((rc = upload_raw(c, L.type_off[24][t], qm.quad_consts))) return rc;
+      if ((rc = upload_raw(c, L.type_off[25][t], qm.list_words))) return rc;
+      if ((rc = upload_raw(c, L.type_off[26][t], qm.vtx_slot))) return rc;
+      if ((rc = upload_raw(c, L.type_off[27][t], qm.vtx_coef))) return rc;
+      QuadMpDev &md = d.quadmp;
+      md.valid = true;
+      md.passes = qm.passes; md.nq = qm.nq; md.maxv = qm.maxq; md.lstride = qm.lstride;
+      md.n_vslots = qm.n_vslots; md.n_tslots = qm.n_tslots; md.n_cslots = qm.n_cslots;
+      for (int i = 0; i < qm.passes && i < 4; ++i) md.list_len[i] = qm.list_len[i];
+      md.vol_lane_bound = qm.vol_lane_bound;
+      md.quad_words = reinterpret_cast<const uint32_t *>(c->ws + L.type_off[23][t]);
+      md.quad_consts = reinterpret_cast<const float *>(c->ws + L.type_off[24][t]);
+      md.list_words = reinterpret_cast<const uint32_t *>(c->ws + L.type_off[25][t]);
+      md.vtx_slot = reinterpret_cast<const uint32_t *>(c->ws + L.type_off[26][t]);
+      md.vtx_coef = reinterpret_cast<const float *>(c->ws + L.type_off[27][t]);
+    }
 
     // dense inverse of H~ on the device (fp64), then cast/pad to the compute type.  H~, the inverse and the
     // Newton-Schulz temporaries sit in the create-time arena of the workspace (overlaid by the state fields, which
@@ -642,6 +669,7 @@ int npfem_create(npfem_ctx **out, const npfem_cell_type *types, int32_t n_types,
     c->host_types.resize(size_t(n_types));
     c->sched.resize(size_t(n_types));
     c->quad.resize(size_t(n_types));
+    c->quadmp.resize(size_t(n_types));
     c->buckets.resize(size_t(n_types));
     for (int t = 0; t < n_types; ++t) {
       std::string err;
@@ -656,6 +684,7 @@ int npfem_create(npfem_ctx **out, const npfem_cell_type *types, int32_t n_types,
         const int tpt = h.T <= 320 ? 1 : 2;
         build_local_schedule(h, types[t].rest_positions, tpt, c->sched[t]);   // may stay invalid
         if (h.T <= 2 * 640) build_quad_schedule(h, types[t].rest_positions, c->quad[t]);   // may stay invalid
+        else if (h.T <= 2 * QMP_THREADS * QMP_MAX_PASSES) build_quadmp_schedule(h, types[t].rest_positions, c->quadmp[t]);
       }
     }
     c->type_of_cell.assign(type_of_cell, type_of_cell + n_cells);
@@ -767,7 +796,7 @@ int npfem_set_option(npfem_ctx *c, int32_t option, int64_t value) {
       c->opt_global_math = value;
       return NPFEM_OK;
     case NPFEM_OPT_LOCAL_STEP_IMPL:
-      if (value < 0 || value > 5) return fail(c, NPFEM_EINVAL, "local-step impl must be 0 ... 5");
+      if (value < 0 || value > 6) return fail(c, NPFEM_EINVAL, "local-step impl must be 0 ... 6");
       c->opt_local_impl = value;
       return NPFEM_OK;
     case NPFEM_OPT_KERNEL_TIMING: c->timing = value != 0; return NPFEM_OK;
@@ -920,14 +949,16 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
       const bool f32 = c->precision == NPFEM_F32 &&
                        (!ls_on || size_t(24) * size_t(c->types[t].n) <= size_t(200) * 1024);
       const bool quad = f32 && (c->opt_local_impl == 0 || c->opt_local_impl == 5) && local_quad_supported(c->types[t]);
-      const bool sched = f32 && !quad && (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]);
-      const bool fast = f32 && !quad && !sched && (c->opt_local_impl == 0 || c->opt_local_impl == 2) && local_smem_supported(c->types[t]);
-      const bool big = f32 && !quad && !sched && !fast && (c->opt_local_impl == 0 || c->opt_local_impl == 4) && local_big_supported(c->types[t]);
-      const bool reduced = quad || sched || fast || big;
+      const bool quadmp = f32 && !quad && (c->opt_local_impl == 0 || c->opt_local_impl == 6) && local_quadmp_supported(c->types[t]);
+      const bool sched = f32 && !quad && !quadmp && (c->opt_local_impl == 0 || c->opt_local_impl == 3) && local_sched_supported(c->types[t]);
+      const bool fast = f32 && !quad && !quadmp && !sched && (c->opt_local_impl == 0 || c->opt_local_impl == 2) && local_smem_supported(c->types[t]);
+      const bool big = f32 && !quad && !quadmp && !sched && !fast && (c->opt_local_impl == 0 || c->opt_local_impl == 4) && local_big_supported(c->types[t]);
+      const bool reduced = quad || quadmp || sched || fast || big;
       const double d_scale = reduced && !ls_on ? 1.0 - c->types[t].gamma : 1.0;
       const BucketView &lv = c->views[t];
       if ((rc = timed_launch(c, NPFEM_KIND_LOCAL, int(t), "local step", [&] {
              if (quad) return launch_local_quad(c->types[t], lv, c->n_sm, c->stream);
+             if (quadmp) return launch_local_quadmp(c->types[t], lv, c->n_sm, c->stream);
              if (sched) return launch_local_sched(c->types[t], lv, c->n_sm, c->stream);
              if (fast) return launch_local_smem(c->types[t], lv, c->n_sm, c->stream);
              if (big) return launch_local_big(c->types[t], lv, c->n_sm, c->stream);
@@ -1430,6 +1461,127 @@ int npfem_quad_schedule_stats(const npfem_cell_type *type, double dt, double *st
     std::sort(reads.begin(), reads.end());
     std::sort(corner_slots[v].begin(), corner_slots[v].end());
     ok &= reads == corner_slots[v];
+  }
+  stats[5] = worst_store;
+  stats[6] = worst_gather;
+  stats[7] = ok ? 1 : 0;
+  return NPFEM_OK;
+}
+
+int npfem_quadmp_schedule_stats(const npfem_cell_type *type, double dt, double *stats, int32_t n_stats) {
+  if (!type || !stats || n_stats < 10 || !(dt > 0)) return fail(nullptr, NPFEM_EINVAL, "type/stats missing, n_stats < 10 or dt <= 0");
+  std::fill(stats, stats + n_stats, 0.0);
+  HostTypeData h;
+  std::string err;
+  const int rc = build_host_type(*type, dt, h, err);
+  if (rc != NPFEM_OK) return fail(nullptr, rc, err);
+  QuadMpSchedule qs;
+  const auto t0 = std::chrono::steady_clock::now();
+  if (!build_quadmp_schedule(h, type->rest_positions, qs)) return NPFEM_OK;
+  stats[9] = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  stats[0] = 1;
+  stats[1] = qs.passes;
+  stats[2] = qs.maxq;
+  stats[3] = qs.wf_vertex;
+  stats[4] = qs.wf_normal;
+  stats[8] = double(qs.n_vslots + qs.n_tslots + qs.n_cslots) * 16.0 + 12.0 * ((h.n + 15) / 16 * 16);
+  // ---- decode the tables and check them against the mesh's own connectivity ---------------------------------------
+  auto lo = [](uint32_t w) { return int(w & 0xffffu); };
+  auto hi = [](uint32_t w) { return int(w >> 16); };
+  const int TH = qs.threads, vwords = 1 + qs.maxq / 2;
+  bool ok = qs.nq * 2 == h.T && qs.passes * TH >= qs.nq;
+  std::vector<int> vertex_of_slot(size_t(qs.n_vslots), -1);
+  for (int v = 0; v < h.n; ++v) {
+    const int sl = int(qs.vtx_slot[v]);
+    ok &= sl < qs.n_vslots && vertex_of_slot[sl] < 0;
+    if (sl < qs.n_vslots) vertex_of_slot[sl] = v;
+  }
+  std::vector<int> tri_of_edge(size_t(h.n) * h.n, -1);
+  for (int t = 0; t < h.T; ++t)
+    for (int k = 0; k < 3; ++k) tri_of_edge[size_t(h.tri[4 * t + k]) * h.n + h.tri[4 * t + (k + 1) % 3]] = t;
+  auto tri_at = [&](int a, int b) { return a >= 0 && b >= 0 ? tri_of_edge[size_t(a) * h.n + b] : -1; };
+  auto W = [&](int k, int q) { return qs.quad_words[(size_t(k / TH) * 7 + q) * TH + k % TH]; };
+  std::vector<int> quad_of_tri(size_t(h.T), -1), tslot_of_tri(size_t(h.T), -1), seen_t(size_t(qs.n_tslots), 0);
+  struct Dec { int p, q, r, s, A, B; };
+  std::vector<Dec> dec(size_t(qs.nq), Dec{-1, -1, -1, -1, -1, -1});
+  double worst_store = 0, worst_gather = 0;
+  for (int ps = 0; ps < qs.passes && ok; ++ps) {
+    const int k0 = ps * TH, k1 = std::min(qs.nq, k0 + TH);
+    std::vector<int> seen_c(size_t(qs.n_cslots), 0);
+    std::vector<std::vector<int>> corner_slots(size_t(h.n));
+    for (int k = k0; k < k1 && ok; ++k) {
+      const int sl[4] = {lo(W(k, 0)), hi(W(k, 0)), lo(W(k, 1)), hi(W(k, 1))};
+      int v[4];
+      for (int i = 0; i < 4; ++i) v[i] = sl[i] < qs.n_vslots ? vertex_of_slot[sl[i]] : -1;
+      Dec &d = dec[k];
+      d.p = v[0]; d.q = v[1]; d.r = v[2]; d.s = v[3];
+      d.A = tri_at(d.p, d.q);
+      d.B = tri_at(d.q, d.p);
+      ok &= d.A >= 0 && d.B >= 0 && d.A != d.B && tri_at(d.q, d.r) == d.A && tri_at(d.r, d.p) == d.A &&
+            tri_at(d.p, d.s) == d.B && tri_at(d.s, d.q) == d.B;
+      if (!ok) break;
+      ok &= quad_of_tri[d.A] < 0 && quad_of_tri[d.B] < 0;
+      quad_of_tri[d.A] = quad_of_tri[d.B] = k;
+      const int ta = lo(W(k, 4)), tb = hi(W(k, 4));
+      ok &= ta < qs.n_tslots && tb < qs.n_tslots && ta != tb && !seen_t[ta]++ && !seen_t[tb]++;
+      tslot_of_tri[d.A] = ta;
+      tslot_of_tri[d.B] = tb;
+      const int cs[4] = {lo(W(k, 5)), hi(W(k, 5)), lo(W(k, 6)), hi(W(k, 6))};
+      for (int i = 0; i < 4; ++i) {
+        ok &= cs[i] < qs.n_cslots - 8 && !seen_c[cs[i]]++;
+        corner_slots[v[i]].push_back(cs[i]);
+      }
+    }
+    // stores: quarter warps of 8 consecutive quad threads, per corner role
+    for (int k = k0; k < k1; k += 8)
+      for (int role = 0; role < 4; ++role) {
+        int mult[8] = {0, 0, 0, 0, 0, 0, 0, 0}, w = 0;
+        for (int kk = k; kk < std::min(k + 8, k1); ++kk) {
+          const uint32_t word = W(kk, 5 + role / 2);
+          w = std::max(w, ++mult[((role & 1) ? hi(word) : lo(word)) % 8]);
+        }
+        worst_store = std::max(worst_store, double(w));
+      }
+    // the pass's vertex list: every vertex touched by the pass exactly once, reading exactly its slots
+    const int len = qs.list_len[ps];
+    ok &= len <= qs.lstride;
+    auto LW = [&](int q, int e) { return qs.list_words[(size_t(ps) * vwords + q) * qs.lstride + e]; };
+    auto read_slot = [&](int e, int q) { const uint32_t w = LW(1 + q / 2, e); return (q & 1) ? hi(w) : lo(w); };
+    std::vector<int> listed(size_t(h.n), 0);
+    for (int e = 0; e < len && ok; ++e) {
+      const int v = int(LW(0, e));
+      ok &= v >= 0 && v < h.n && !listed[v]++;
+      if (!ok) break;
+      std::vector<int> reads;
+      for (int q = 0; q < qs.maxq; ++q) {
+        const int sl = read_slot(e, q);
+        if (sl < qs.n_cslots - 8) reads.push_back(sl);
+        else ok &= sl < qs.n_cslots;
+      }
+      std::sort(reads.begin(), reads.end());
+      std::sort(corner_slots[v].begin(), corner_slots[v].end());
+      ok &= reads == corner_slots[v];
+    }
+    for (int e = len; e < qs.lstride; ++e) ok &= LW(0, e) == 0xffffffffu;
+    for (int v = 0; v < h.n; ++v) ok &= listed[v] || corner_slots[v].empty();
+    for (int e0 = 0; e0 < len; e0 += 8)
+      for (int q = 0; q < qs.maxq; ++q) {
+        int mult[8] = {0, 0, 0, 0, 0, 0, 0, 0}, w = 0;
+        std::vector<int> slots;
+        for (int e = e0; e < std::min(e0 + 8, len); ++e) {
+          const int sl = read_slot(e, q);
+          if (std::find(slots.begin(), slots.end(), sl) == slots.end()) w = std::max(w, ++mult[sl % 8]);
+          slots.push_back(sl);
+        }
+        worst_gather = std::max(worst_gather, double(w));
+      }
+  }
+  for (int t = 0; t < h.T; ++t) ok &= quad_of_tri[t] >= 0;
+  for (int k = 0; k < qs.nq && ok; ++k) {
+    const Dec &d = dec[k];
+    const int ns[4] = {lo(W(k, 2)), hi(W(k, 2)), lo(W(k, 3)), hi(W(k, 3))};
+    const int nb[4] = {tri_at(d.r, d.q), tri_at(d.p, d.r), tri_at(d.s, d.p), tri_at(d.q, d.s)};
+    for (int i = 0; i < 4; ++i) ok &= nb[i] >= 0 && ns[i] == tslot_of_tri[nb[i]];
   }
   stats[5] = worst_store;
   stats[6] = worst_gather;

@@ -31,6 +31,19 @@ struct SchedDev {
   double vol_lane_bound = 0;   // max over threads of sum_j |x0| 2A_t of the rest shape (6V partial per lane)
 };
 
+// Device tables of the multi-pass quad local step (quadmp_schedule.hpp / local_quadmp.cu)
+struct QuadMpDev {
+  bool valid = false;
+  int passes = 0, nq = 0, maxv = 0, lstride = 0, n_vslots = 0, n_tslots = 0, n_cslots = 0;
+  int list_len[4] = {0, 0, 0, 0};
+  const uint32_t *quad_words = nullptr;
+  const float *quad_consts = nullptr;
+  const uint32_t *list_words = nullptr;
+  const uint32_t *vtx_slot = nullptr;
+  const float *vtx_coef = nullptr;
+  double vol_lane_bound = 0;
+};
+
 // Per-context launch state of the kernels that opt in to more than 48 KB of dynamic shared memory: the attribute
 // is per device and function, the occupancy depends on it, so both are cached per context and cell type (a
 // process-wide static would be wrong for two devices in one process).
@@ -50,7 +63,7 @@ struct KernelCache {
   int sched_per_sm = 0, quad_per_sm = 0;
   int tc_smem = 0;
   bool generic_attr[2] = {false, false}, smem_attr = false, big_attr = false, fused_attr = false, objective_attr = false,
-       damping_attr = false;
+       damping_attr = false, quadmp_attr = false;
 };
 
 // Device view of one cell type (pointers into the workspace; element type = compute type).
@@ -79,6 +92,7 @@ struct TypeDev {
   double kappa = 0;
   SchedDev sched;                    // fp32 contexts: scheduled local step (may be invalid)
   SchedDev quad;                     // fp32 contexts: quad local step (quad_schedule.hpp / local_quad.cu; may be invalid)
+  QuadMpDev quadmp;                  // fp32 contexts, meshes beyond one pass: multi-pass quad local step (may be invalid)
   mutable KernelCache cache;
 };
 
@@ -213,6 +227,9 @@ int launch_local_sched(const TypeDev &td, const BucketView &bv, int n_sm, cudaSt
 // fp32 quad local step: one thread per pair of adjacent triangles; same reduced-gradient convention
 bool local_quad_supported(const TypeDev &td);
 int launch_local_quad(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
+// the same for meshes of up to 4 x 640 quads (RBC-2562): the quads in passes, per-vertex accumulators in shared memory
+bool local_quadmp_supported(const TypeDev &td);
+int launch_local_quadmp(const TypeDev &td, const BucketView &bv, int n_sm, cudaStream_t s);
 
 // fp32 reduced-gradient local step for types too large for the scheduled kernel (chunked corner forces)
 bool local_big_supported(const TypeDev &td);

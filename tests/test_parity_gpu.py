@@ -66,10 +66,11 @@ def test_config3_mixed_types_redrawn_forces(precision):
     _check(pop, precision, fp32=(8e-5, 8e-4, 2.7e-3, 1.4e-4), n_steps=4, n_iterations=5)
 
 
-@pytest.mark.parametrize("precision,impl", [("fp32", 0), ("fp32", 1), ("fp32", 4), ("fp64", 0)])
+@pytest.mark.parametrize("precision,impl", [("fp32", 0), ("fp32", 1), ("fp32", 4), ("fp32", 6), ("fp64", 0)])
 def test_config5_level4_mesh(precision, impl):
-    # 2562 vertices / 5120 triangles: too large for the scheduled kernel -> large-mesh kernel (fp32 default,
-    # corner forces in chunks) or the generic kernel with its global scratch (impl 1, fp64)
+    # 2562 vertices / 5120 triangles: too large for one pass of the quad kernel -> multi-pass quad kernel (fp32 default
+    # = impl 6: 4 passes of 640 quads), the large-mesh kernel of round 1 (impl 4: corner forces in chunks) or the
+    # generic kernel with its global scratch (impl 1, fp64)
     from paper_1911_03062_b200 import binding
     # measured 2.4e-4, 2.6e-4, 1.3e-3, 2.5e-4 (large-mesh kernel), 2.1e-4, 2.2e-4, 9.7e-4, 2.1e-4 (generic)
     _check(make_config(5, n_cells=40), precision, fp32=(5e-4, 5.2e-4, 2.7e-3, 5.1e-4), n_steps=2, n_iterations=3,

@@ -77,3 +77,17 @@ def test_quad_schedule_irregular_mesh_and_rejections():
     a, b = quad_schedule_stats(rbc_cell_type(2), 0.1), quad_schedule_stats(rbc_cell_type(2), 0.1)
     a.pop("build_ms"), b.pop("build_ms")
     assert a == b                                                            # deterministic
+
+
+def test_multipass_quad_schedule_of_the_level4_mesh():
+    """RBC-2562 (BASELINE configs[4]): 2,560 quads in 4 passes of 640; global vertex / normal slots, per-pass corner
+    slots and per-pass vertex lists, all decoded and checked against the mesh by the library."""
+    st = quad_schedule_stats(rbc_cell_type(4), 0.1, multipass=True)
+    assert st["valid"] == 1 and st["threads"] == 4 and st["consistent"] == 1      # "threads" = passes here
+    assert st["reads_per_vertex"] == 6
+    assert st["worst_store_quarter"] == 1 and st["worst_gather_quarter"] == 1
+    assert 4.0 <= st["wf_vertex_gather"] <= 6.0 and 4.0 <= st["wf_normal_gather"] <= 6.0
+    assert st["smem_bytes"] <= 227 * 1024
+    # one pass suffices for the smaller meshes (the one-pass kernel takes them); too many passes are refused
+    assert quad_schedule_stats(rbc_cell_type(3), 0.1, multipass=True)["threads"] == 1
+    assert quad_schedule_stats(rbc_cell_type(5), 0.1, multipass=True)["valid"] == 0
