@@ -73,9 +73,31 @@ __global__ void __launch_bounds__(TH, 1) local_quadmp_kernel(const QuadMpParams 
   unsigned char *sC = sN + p.sN_bytes;
   float *acc = reinterpret_cast<float *>(sC + p.sC_bytes);     // [3][n_pad] corner-force sums per vertex
   int *vacc = reinterpret_cast<int *>(acc + 3 * n_pad);        // [hi, lo] base-2^12 digits of 6V (fixed point)
+  uint64_t *bar_acc = reinterpret_cast<uint64_t *>(vacc + 2);  // split barrier "accumulators of the pass updated"
   const int tid = threadIdx.x, lane = tid & 31;
 
   if (tid < 8) sts4(sC, uint32_t(p.sC_bytes) - 128u + 16u * tid, 0.f, 0.f, 0.f, 0.f);   // the zero slots
+  if (tid == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(uint32_t(__cvta_generic_to_shared(bar_acc))), "r"(TH / 32));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  // arrive early (after the pass's accumulation), wait late (before the next corner-force stores / before phase C):
+  // the threads with two list entries no longer hold up the others at a second block barrier per pass
+  auto acc_arrive = [&]() {
+    __syncwarp();
+    if (lane == 0)
+      asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(uint32_t(__cvta_generic_to_shared(bar_acc))) : "memory");
+  };
+  auto acc_wait = [&](uint32_t parity) {
+    uint32_t done;
+    do {
+      asm volatile(
+          "{\n.reg .pred q;\nmbarrier.try_wait.parity.shared::cta.b64 q, [%1], %2, %3;\nselp.u32 %0, 1, 0, q;\n}\n"
+          : "=r"(done) : "r"(uint32_t(__cvta_generic_to_shared(bar_acc))), "r"(parity), "r"(20000u) : "memory");
+    } while (!done);
+  };
+  uint32_t acc_phase = 0;      // completed phases of bar_acc (one per pass)
   uint32_t qw[QW];
   float qk[QK];
   auto load_pass = [&](int ps) {   // this thread's quad of pass ps (zeros beyond the last quad: nothing is stored then)
@@ -290,6 +312,7 @@ __global__ void __launch_bounds__(TH, 1) local_quadmp_kernel(const QuadMpParams 
           cs4[k] = t1;
         }
       }
+      if (ps > 0) acc_wait((acc_phase - 1) & 1u);     // the previous pass's gathers from sC are done
       if (act) {
         sts4(sC, (lo16(qw[5]) << 4), cp[0], cp[1], cp[2], 0.f);
         sts4(sC, (hi16(qw[5]) << 4), cq[0], cq[1], cq[2], 0.f);
@@ -328,9 +351,11 @@ __global__ void __launch_bounds__(TH, 1) local_quadmp_kernel(const QuadMpParams 
           acc[2 * n_pad + vid] += az;
         }
       }
-      __syncthreads();
+      acc_arrive();
+      ++acc_phase;
     }
     // ---- phase C: r = coef d - b + the vertex's corner forces -> global -----------------------------------------
+    // (merging it with phase 0 of the CTA's next cell, loads of both issued together, was tried: 0.99 vs 0.94 ms)
 #pragma unroll
     for (int j0 = 0; j0 < NV; j0 += 3) {
       float dd[3][3], bb[3][3], coef[3];
@@ -345,6 +370,7 @@ __global__ void __launch_bounds__(TH, 1) local_quadmp_kernel(const QuadMpParams 
           bb[jj][c] = a ? __ldcs(p.b + base + c * n_pad + v) : 0.f;
         }
       }
+      if (j0 == 0) acc_wait((acc_phase - 1) & 1u);    // every accumulator is final (the loads above are in flight)
 #pragma unroll
       for (int jj = 0; jj < 3; ++jj) {
         const int v = tid + (j0 + jj) * TH;
@@ -360,13 +386,13 @@ __global__ void __launch_bounds__(TH, 1) local_quadmp_kernel(const QuadMpParams 
         }
       }
     }
-    // the next cell's phase 0 rewrites sx (last read before the last pass's first barrier) and zeroes acc[v] in the
-    // thread that has just read it
+    // the next cell's phase 0 rewrites sx (last read in the last pass's arithmetic, which every warp has left: the wait
+    // above) and zeroes acc[v] in the thread that has just read it
   }
 }
 
 size_t quadmp_smem_bytes(const QuadMpDev &s, int n_pad) {
-  return size_t(s.n_vslots + s.n_tslots + s.n_cslots) * 16 + size_t(3) * n_pad * 4 + 16;
+  return size_t(s.n_vslots + s.n_tslots + s.n_cslots) * 16 + size_t(3) * n_pad * 4 + 8 + 8;
 }
 
 }  // namespace
