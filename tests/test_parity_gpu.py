@@ -222,6 +222,33 @@ def test_fp32_local_step_implementations(impl):
         assert_row(r, "fp32", (1.3e-4, 1.3e-3, 4.3e-3, 1.8e-4))
 
 
+def test_two_pass_mesh_with_a_partly_filled_last_pass():
+    """An octahedral RBC mesh of 1,026 vertices / 2,048 triangles: 1,024 quads = one full pass of the multi-pass quad
+    kernel + one pass of 384 quads (threads without a quad, vertices listed in both passes)."""
+    from paper_1911_03062_b200 import binding
+    from workloads.meshes import rbc_cell_type
+    ct = rbc_cell_type(4, base="octa")
+    assert ct.rest_positions.shape[0] == 1026 and binding.quad_schedule_stats(ct, 0.1, multipass=True)["threads"] == 2
+    rng = np.random.default_rng(5)
+    n_cells = 170                               # more cells than CTAs: the persistent loop wraps
+    pos = ct.rest_positions[None] + rng.uniform(0, 120, (n_cells, 1, 3))
+    pop = Population(name="octa4", types=[ct], type_of_cell=np.zeros(n_cells, np.int32), positions=[pos],
+                     velocities=[0.01 * rng.standard_normal(pos.shape)], dt=0.1, n_steps=2, n_iterations=4,
+                     box=(120.0,) * 3, force_sigma=1.0, shear_gamma=0.0, redraw_noise_each_step=False,
+                     _force_seed=np.random.SeedSequence(6), _shear_height=[pos[..., 2]])
+    ref = run_oracle(pop)
+    out = {}
+    for impl in (6, 1):
+        gpu, solver = run_gpu(pop, "fp32", options=[(binding.OPT_LOCAL_STEP_IMPL, impl), (binding.OPT_GLOBAL_STEP_MATH, 1)])
+        solver.close()
+        out[impl] = compare(pop, gpu, ref)[0]
+        print(impl, out[impl])
+    # the generic kernel (impl 1) is the yardstick on the same inputs: the multi-pass kernel sits at the same fp32 floor
+    for k in ("disp", "worst_cell", "worst_vertex", "vel"):
+        assert out[6][k] <= 1.5 * out[1][k] + 1e-6, (k, out[6][k], out[1][k])
+    assert out[6]["pos"] <= TOL_POS["fp32"] and out[6]["disp"] <= 5e-4
+
+
 @pytest.mark.parametrize("precision,impl", [("fp64", 0), ("fp32", 1), ("fp32", 3), ("fp32", 5)])
 def test_irregular_mesh_valence_up_to_8(precision, impl):
     """A mesh that is not an icosphere (flipped edges, valences 4..8): generic kernels and the

@@ -88,6 +88,10 @@ def test_multipass_quad_schedule_of_the_level4_mesh():
     assert st["worst_store_quarter"] == 1 and st["worst_gather_quarter"] == 1
     assert 4.0 <= st["wf_vertex_gather"] <= 6.0 and 4.0 <= st["wf_normal_gather"] <= 6.0
     assert st["smem_bytes"] <= 227 * 1024
+    # 1,024 quads: one full pass and one of 384 (threads without a quad in the last pass)
+    st2 = quad_schedule_stats(rbc_cell_type(4, base="octa"), 0.1, multipass=True)
+    assert st2["valid"] == 1 and st2["threads"] == 2 and st2["consistent"] == 1
+    assert st2["worst_store_quarter"] == 1 and st2["worst_gather_quarter"] == 1
     # one pass suffices for the smaller meshes (the one-pass kernel takes them); too many passes are refused
     assert quad_schedule_stats(rbc_cell_type(3), 0.1, multipass=True)["threads"] == 1
     assert quad_schedule_stats(rbc_cell_type(5), 0.1, multipass=True)["valid"] == 0
