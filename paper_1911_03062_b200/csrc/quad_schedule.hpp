@@ -294,9 +294,6 @@ inline void repair_matching(const HostTypeData &h, const std::vector<std::array<
           int w2;
           long n2, e2;
           cost(bl.match, w2, n2, e2);
-#ifdef QUAD_DEBUG
-          printf("round %d v %d pair (%d,%d): worst %d->%d n %ld->%ld excess %ld->%ld\n", round, v, a, b, worst, w2, n_worst, n2, excess, e2);
-#endif
           if (w2 < worst || (w2 == worst && (n2 < n_worst || (n2 == n_worst && e2 < excess)))) {
             mate = bl.match;
             improved = true;
