@@ -42,6 +42,8 @@ def parse_args():
     ap.add_argument("--global-math", default="tf32", choices=["tf32", "fp32", "tf32x2"])
     ap.add_argument("--local-impl", type=int, default=0, choices=[0, 1, 2, 3, 4, 5, 6])
     ap.add_argument("--line-search", type=int, default=0, help="Armijo backtracking with this many halvings (0 = off)")
+    ap.add_argument("--graph", action="store_true",
+                    help="capture one npfem_step in a CUDA graph and time replays of it (pays off at small cell counts)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-chunks", type=int, default=0, help="npfem_step_host chunks (0 = library's choice, 1 = unpipelined)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -370,6 +372,8 @@ def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: 
     np_io = np.float32 if args.precision == "fp32" else np.float64
     peaks = load_peaks()
 
+    if args.graph:      # a graph cannot be captured on the legacy default stream: the whole run moves to a side stream
+        torch.cuda.set_stream(torch.cuda.Stream(device=local_rank))
     solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision=args.precision, device=local_rank)
     solver.set_option(binding.OPT_GLOBAL_STEP_MATH, {"tf32": 0, "fp32": 1, "tf32x2": 2}[args.global_math])
     solver.set_option(binding.OPT_LOCAL_STEP_IMPL, args.local_impl)
@@ -389,17 +393,30 @@ def run_b200(args, pop, n_iterations: int, config_desc: dict, rank: int, world: 
     for _ in range(args.warmup):
         solver.step(n_iterations)
     barrier()
+    graph, launches_per_step = None, None
+    if args.graph:
+        # npfem_step allocates nothing and never synchronises (include/npfem.h): one step = one capturable sequence
+        l0 = solver.launch_count
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=torch.cuda.current_stream(local_rank)):
+            solver.step(n_iterations)
+        launches_per_step = solver.launch_count - l0
+        graph.replay()
+        barrier()
     launches0 = solver.launch_count
     marks = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     with ClockSampler(local_rank) as clocks:
         marks[0].record()
         for k in range(args.steps):
-            solver.step(n_iterations)
+            if graph is not None:
+                graph.replay()
+            else:
+                solver.step(n_iterations)
             marks[k + 1].record()                     # one event between steps: per-step times for median / best
         barrier()
     elapsed_ms = marks[0].elapsed_time(marks[-1])
     step_ms = sorted(marks[k].elapsed_time(marks[k + 1]) for k in range(args.steps))
-    launches = solver.launch_count - launches0
+    launches = launches_per_step * args.steps if graph is not None else solver.launch_count - launches0
     # per-kernel breakdown: the same K steps again with a CUDA-event pair around every launch (kept out of
     # the timed region above: the events cost as much as a small kernel in the small-batch regime)
     solver.set_option(binding.OPT_KERNEL_TIMING, 1)
@@ -562,7 +579,7 @@ def config_description(args, pop, n_cells: int, n_iterations: int) -> dict:
     return {"workload": f"{label}: {CONFIG_NAMES[args.config]}",
             "cells": int(n_cells), "cell_types_vertices": mix, "iterations_per_step": int(n_iterations),
             "dt_us": pop.dt, "precision": args.precision, "global_step_math": args.global_math,
-            "line_search_halvings": int(args.line_search),
+            "line_search_halvings": int(args.line_search), "cuda_graph": bool(args.graph),
             "l2": ("no flush needed: the state touched per iteration (>= 2.9 GB at 100k cells) exceeds the 126 MB L2"
                    if n_cells >= 20000 else "state fits the 126 MB L2: small-batch latency regime, no flush")}
 

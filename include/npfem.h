@@ -181,6 +181,8 @@ int npfem_set_forces(npfem_ctx *ctx, const int64_t *cell_ids, int64_t n_ids,
  * ONE time step h for every cell: prologue (PBD damping, rhs), `n_iterations`
  * quasi-Newton iterations of Eq. (4) (local step = grad g, global step = apply H~^-1),
  * epilogue (Eq. 1).  1 <= n_iterations <= NPFEM_MAX_ITERATIONS.  Asynchronous.
+ * The call only enqueues kernels on the context's stream: no allocation, no synchronisation, no host read-back.  With
+ * a caller-owned workspace (and scratch for the optional features) it can be captured in a CUDA graph and replayed.
  */
 int npfem_step(npfem_ctx *ctx, int32_t n_iterations);
 

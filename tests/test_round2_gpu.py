@@ -245,3 +245,39 @@ def test_config4_full_size_all_10_steps_sampled_cells():
         print("config 4 full size, 10 x 10:", r)
         assert r["pos"] <= 1e-4 and r["worst_cell_pos"] <= 1e-4
         assert r["disp"] <= 1e-4 and r["worst_cell"] <= 1e-3 and r["vel"] <= 3e-4, r
+
+
+def test_step_is_capturable_in_a_cuda_graph_and_replays_bit_identically():
+    """npfem_step allocates nothing and never synchronises (the memory contract of include/npfem.h), so a whole time
+    step - prologue, K x (local step, tensor-core global step), epilogue - is ONE capturable launch sequence: captured
+    once, replayed, the state equals the eagerly stepped one bit for bit (bench.py --graph times the replays)."""
+    import torch
+    from paper_1911_03062_b200 import Solver
+    pop = make_config(3, n_cells=330)
+    side = torch.cuda.Stream()
+    x0 = torch.from_numpy(pop.packed(pop.positions)).cuda()
+    f0 = torch.from_numpy(pop.packed(pop.forces(0), dtype=np.float32)).cuda()
+    torch.cuda.synchronize()
+    states = {}
+    with torch.cuda.stream(side):
+        for mode in ("eager", "graph"):
+            solver = Solver(pop.types, pop.type_of_cell, pop.dt, precision="fp32")
+            solver.set_state(x0)
+            solver.set_forces(f0)
+            solver.step(5)                                     # first step eagerly in both runs: attributes, module loads
+            if mode == "eager":
+                for _ in range(3):
+                    solver.step(5)
+            else:
+                side.synchronize()
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=side):
+                    solver.step(5)                             # captured, not run
+                for _ in range(3):
+                    g.replay()
+            x, v = solver.get_state()
+            side.synchronize()
+            states[mode] = (x.cpu().numpy(), v.cpu().numpy())
+            solver.close()
+    assert np.array_equal(states["eager"][0], states["graph"][0]) and np.array_equal(states["eager"][1], states["graph"][1])
+    assert np.abs(states["graph"][0] - pop.packed(pop.positions)).max() > 0
