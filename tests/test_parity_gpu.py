@@ -249,6 +249,34 @@ def test_two_pass_mesh_with_a_partly_filled_last_pass():
     assert out[6]["pos"] <= TOL_POS["fp32"] and out[6]["disp"] <= 5e-4
 
 
+def test_multipass_kernel_on_an_irregular_level4_mesh_valence_up_to_8():
+    """2,562 vertices after 400 random edge flips (valences 4 .. 8): the 8-read variant of the multi-pass quad kernel
+    against the generic kernel on the same inputs and against the oracle."""
+    from paper_1911_03062_b200 import binding
+    from workloads.meshes import irregular_cell_type
+    ct = irregular_cell_type(4, 400, seed=5)
+    assert np.bincount(ct.triangles.ravel()).max() == 8
+    st = binding.quad_schedule_stats(ct, 0.1, multipass=True)
+    assert st["valid"] == 1 and st["threads"] == 4 and st["reads_per_vertex"] == 8 and st["consistent"] == 1
+    rng = np.random.default_rng(17)
+    n_cells = 12
+    pos = ct.rest_positions[None] + rng.uniform(0, 90, (n_cells, 1, 3))
+    pop = Population(name="irr4", types=[ct], type_of_cell=np.zeros(n_cells, np.int32), positions=[pos],
+                     velocities=[0.01 * rng.standard_normal(pos.shape)], dt=0.1, n_steps=2, n_iterations=3,
+                     box=(90.0,) * 3, force_sigma=1.0, shear_gamma=0.0, redraw_noise_each_step=False,
+                     _force_seed=np.random.SeedSequence(18), _shear_height=[pos[..., 2]])
+    ref = run_oracle(pop)
+    out = {}
+    for impl in (6, 1):
+        gpu, solver = run_gpu(pop, "fp32", options=[(binding.OPT_LOCAL_STEP_IMPL, impl), (binding.OPT_GLOBAL_STEP_MATH, 1)])
+        solver.close()
+        out[impl] = compare(pop, gpu, ref)[0]
+        print(impl, out[impl])
+    for k in ("disp", "worst_cell", "worst_vertex", "vel"):
+        assert out[6][k] <= 1.5 * out[1][k] + 1e-6, (k, out[6][k], out[1][k])
+    assert out[6]["pos"] <= TOL_POS["fp32"] and out[6]["disp"] <= TOL_DISP["fp32"]
+
+
 @pytest.mark.parametrize("precision,impl", [("fp64", 0), ("fp32", 1), ("fp32", 3), ("fp32", 5)])
 def test_irregular_mesh_valence_up_to_8(precision, impl):
     """A mesh that is not an icosphere (flipped edges, valences 4..8): generic kernels and the
