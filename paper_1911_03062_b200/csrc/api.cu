@@ -258,7 +258,7 @@ size_t feature_bytes(const npfem_ctx *c, int f) {
   for (size_t t = 0; t < nb; ++t) {
     const size_t cells = size_t(c->buckets[t].cells), np = size_t(c->host_types[t].n_pad);
     if (f == FEAT_LS) {
-      total += align_up(4 * cells * sizeof(double)) + align_up(cells * sizeof(int)) + align_up(cells * 3 * np * es);
+      total += align_up(4 * cells * sizeof(double)) + align_up((cells + 1) * sizeof(int)) + align_up(cells * 3 * np * es);
       if (c->precision == NPFEM_F32) total += align_up(cells * 3 * np * 4);   // g_lo of the 3xTF32 product
     } else {
       total += align_up(cells * 3 * np * sizeof(double)) + align_up(cells * np * es);
@@ -304,7 +304,7 @@ int materialise_feature(npfem_ctx *c, int f) {
       l.obj1 = l.obj0 + cells;
       l.slope = l.obj1 + cells;
       l.alpha = l.slope + cells;
-      l.done = reinterpret_cast<int *>(take(cells * sizeof(int)));
+      l.done = reinterpret_cast<int *>(take((cells + 1) * sizeof(int)));   // + done[cells]: cells still searching
       l.d_old = take(cells * 3 * np * es);
       if (c->precision == NPFEM_F32) {
         float *g_lo = reinterpret_cast<float *>(take(cells * 3 * np * 4));
@@ -1005,6 +1005,7 @@ int npfem_step(npfem_ctx *c, int32_t n_iterations) {
       if (ls_on && c->buckets[t].cells) {
         if ((rc = timed_launch(c, NPFEM_KIND_LINE_SEARCH, int(t), "line search", [&] {
                int nl = launch_ls_init(c->views[t], c->ls[t], c->ls_tol, c->precision, c->stream);
+               if (nl < 0) return nl;
                for (int l = 0; l <= c->ls_max_halvings; ++l) {
                  nl += launch_objective(c->types[t], c->views[t], nullptr, c->ls[t].obj1, c->ls[t].done, c->precision, c->n_sm, c->stream);
                  if (c->col_active)

@@ -109,6 +109,7 @@ collision_energy_kernel(BucketView bv, CollisionDev col, const int64_t *__restri
   const int64_t warp0 = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) >> 5;
   const int64_t n_warps = (int64_t(gridDim.x) * blockDim.x) >> 5;
   const int n = bv.n, n_pad = bv.n_pad;
+  if (skip && skip[bv.cells] == 0) return;              // line search: skip[cells] = cells still searching
   for (int64_t cell = warp0; cell < bv.cells; cell += n_warps) {
     if (skip && skip[cell]) continue;
     const size_t base = size_t(cell) * 3 * n_pad;

@@ -187,7 +187,8 @@ int launch_objective(const TypeDev &td, const BucketView &bv, const int64_t *cel
 // Armijo backtracking line search, per-cell state of one bucket
 struct LineSearchDev {
   double *obj0 = nullptr, *obj1 = nullptr, *slope = nullptr, *alpha = nullptr;   // [cells]
-  int *done = nullptr;                                                            // [cells]
+  int *done = nullptr;   // [cells + 1]: 1 = step length settled; done[cells] = number of cells still searching (kernels
+                         // that are given `done` as their skip list return at once when it is 0)
   void *d_old = nullptr;                                                          // [cells][3][n_pad] d before the global step
   // fp32 contexts whose global step runs on the TF32 tensor cores: the search direction comes from a 3xTF32
   // product (g = g_hi + g_lo, H~^-1 = W_hi + W_lo, the lo x lo term dropped), see launch_ls_split_g

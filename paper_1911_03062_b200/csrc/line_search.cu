@@ -70,6 +70,7 @@ ls_init_kernel(BucketView bv, LineSearchDev ls, double grad_tol) {
       ls.slope[cell] = slope;
       ls.alpha[cell] = frozen ? 0.0 : 1.0;
       ls.done[cell] = frozen ? 1 : 0;
+      if (!frozen) atomicAdd(ls.done + bv.cells, 1);     // cells still searching (zeroed by launch_ls_init)
     }
   }
 }
@@ -81,6 +82,7 @@ ls_accept_kernel(BucketView bv, LineSearchDev ls, double c1, int last) {
   const int64_t warp0 = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) >> 5;
   const int64_t n_warps = (int64_t(gridDim.x) * blockDim.x) >> 5;
   const int n = bv.n, n_pad = bv.n_pad;
+  if (*static_cast<volatile const int *>(ls.done + bv.cells) == 0) return;   // every cell has settled: nothing to do
   for (int64_t cell = warp0; cell < bv.cells; cell += n_warps) {
     if (ls.done[cell]) continue;                // warp-uniform
     const double alpha = ls.alpha[cell];
@@ -92,6 +94,7 @@ ls_accept_kernel(BucketView bv, LineSearchDev ls, double c1, int last) {
       if (lane == 0) {
         ls.done[cell] = 1;
         ls.obj0[cell] = ls.obj1[cell];
+        atomicSub(ls.done + bv.cells, 1);
       }
       continue;
     }
@@ -234,6 +237,7 @@ int launch_ls_split_w(const float *w, const float *w_hi, float *w_lo, size_t cou
 
 int launch_ls_init(const BucketView &bv, const LineSearchDev &ls, double grad_tol, int precision, cudaStream_t s) {
   if (bv.cells == 0) return 0;
+  if (cudaMemsetAsync(ls.done + bv.cells, 0, sizeof(int), s) != cudaSuccess) return -2;
   if (precision == NPFEM_F32)
     ls_init_kernel<float><<<warp_grid(bv.cells), 128, 0, s>>>(bv, ls, grad_tol);
   else

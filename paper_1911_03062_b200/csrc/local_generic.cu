@@ -226,6 +226,7 @@ objective_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_id, do
   // cell_id == nullptr: out_row is indexed by the bucket slot; skip[slot] != 0: leave that cell alone
   __shared__ double red[8];
   const int n = p.n, n_pad = p.n_pad, nt = p.T_;
+  if (skip && skip[p.cells] == 0) return;               // line search: skip[cells] = cells still searching
   for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x) {
     if (skip && skip[cell]) continue;
     const size_t base = size_t(cell) * 3 * n_pad;
@@ -332,6 +333,7 @@ objective_smem_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_i
   const int n = p.n, n_pad = p.n_pad, nt = p.T_;
   double *sp = reinterpret_cast<double *>(smem_raw);   // [3][n] x_n + d
   double *sn = sp + 3 * n;                              // [T][3] unit normals
+  if (skip && skip[p.cells] == 0) return;               // line search: skip[cells] = cells still searching
   for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x) {
     if (skip && skip[cell]) continue;                   // uniform over the CTA
     const size_t base = size_t(cell) * 3 * n_pad;
