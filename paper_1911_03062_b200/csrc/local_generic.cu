@@ -323,7 +323,10 @@ __device__ __forceinline__ void load_pair(const double *p, double &a, double &b)
 // ---- objective, shared-memory version (line search): the same sum as objective_kernel
 // with x_n + d and the UNIT triangle normals of the cell staged once in shared memory in fp64, so a hinge
 // costs one rsqrt (1/|e|) instead of three neighbour-normal cross products, two sqrt and a division.
-// Shared memory: 8 (3 n + 3 T) bytes (RBC-642: 46 KB, RBC-2562: 184 KB); larger meshes keep objective_kernel.
+// d itself is staged too (compute type): the damping part's one-ring stencil then gathers from shared memory instead
+// of issuing ~20 scattered global loads per vertex.
+// Shared memory: 8 (3 n + 3 T) + 3 n sizeof(T) bytes (RBC-642 fp32: 54 KB, RBC-2562: 215 KB); larger meshes keep
+// objective_kernel.
 template <typename T, int NT>
 __global__ void __launch_bounds__(NT)
 objective_smem_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_id, double *__restrict__ out_row,
@@ -333,14 +336,17 @@ objective_smem_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_i
   const int n = p.n, n_pad = p.n_pad, nt = p.T_;
   double *sp = reinterpret_cast<double *>(smem_raw);   // [3][n] x_n + d
   double *sn = sp + 3 * n;                              // [T][3] unit normals
+  T *sd = reinterpret_cast<T *>(sn + 3 * nt);           // [3][n] d
   if (skip && skip[p.cells] == 0) return;               // line search: skip[cells] = cells still searching
   for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x) {
     if (skip && skip[cell]) continue;                   // uniform over the CTA
     const size_t base = size_t(cell) * 3 * n_pad;
     for (int k = 0; k < 3; ++k)
-      for (int i = threadIdx.x; i < n; i += NT)
-        sp[k * n + i] = double(p.x[base + k * n_pad + i]) +
-                        ((p.xl ? double(p.xl[base + k * n_pad + i]) : 0.0) + double(p.d[base + k * n_pad + i]));
+      for (int i = threadIdx.x; i < n; i += NT) {
+        const T di = p.d[base + k * n_pad + i];
+        sd[k * n + i] = di;
+        sp[k * n + i] = double(p.x[base + k * n_pad + i]) + ((p.xl ? double(p.xl[base + k * n_pad + i]) : 0.0) + double(di));
+      }
     __syncthreads();
     double acc = 0.0, vol = 0.0;
     for (int t = threadIdx.x; t < nt; t += NT) {
@@ -385,13 +391,13 @@ objective_smem_kernel(const LocalParams<T> p, const int64_t *__restrict__ cell_i
       double di[3], u[3];
       const double w0 = p.vtx_w[i];
       for (int k = 0; k < 3; ++k) {
-        di[k] = double(p.d[base + k * n_pad + i]);
+        di[k] = double(sd[k * n + i]);
         u[k] = w0 * di[k];
       }
       for (int q = 0; q < p.valence_max; ++q) {
         const int j = p.vtx_nbr[q * n + i];
         const double w = p.vtx_w[(q + 1) * n + i];
-        for (int k = 0; k < 3; ++k) u[k] += w * double(p.d[base + k * n_pad + j]);
+        for (int k = 0; k < 3; ++k) u[k] += w * double(sd[k * n + j]);
       }
       const double dd = dot3(di, di), du = dot3(di, u), uu = dot3(u, u);
       acc += 0.5 * (double(p.inertia_coef) * double(p.vtx_mass[i]) * dd +
@@ -503,11 +509,11 @@ template <typename T>
 int launch_objective_T(const TypeDev &td, const BucketView &bv, const int64_t *cell_id_dev, double *objective_row,
                        const int *skip_dev, int n_sm, cudaStream_t s) {
   const LocalParams<T> p = make_params<T>(td, bv);
-  const size_t smem = sizeof(double) * (size_t(3) * td.n + size_t(3) * td.T);
-  if (smem <= 56 * 1024) {                    // 4 CTAs of 256 threads per SM (RBC-642: 46 KB each)
-    if (!td.cache.objective_attr) cudaFuncSetAttribute(objective_smem_kernel<T, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 56 * 1024);
+  const size_t smem = sizeof(double) * (size_t(3) * td.n + size_t(3) * td.T) + sizeof(T) * size_t(3) * td.n;
+  if (smem <= 74 * 1024) {                    // 4 (fp32 RBC-642: 54 KB each) or 3 (fp64: 62 KB) CTAs of 256 threads per SM
+    if (!td.cache.objective_attr) cudaFuncSetAttribute(objective_smem_kernel<T, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 74 * 1024);
     td.cache.objective_attr = true;
-    const int64_t cap = int64_t(n_sm) * 4 * 4;
+    const int64_t cap = int64_t(n_sm) * (smem <= 56 * 1024 ? 4 : 3) * 4;
     objective_smem_kernel<T, 256><<<unsigned(bv.cells < cap ? bv.cells : cap), 256, smem, s>>>(p, cell_id_dev, objective_row, skip_dev);
   } else if (smem <= kMaxSmem) {              // one CTA of 1024 threads per SM (RBC-2562: 184 KB)
     if (!td.cache.objective_attr) cudaFuncSetAttribute(objective_smem_kernel<T, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kMaxSmem));
