@@ -12,6 +12,9 @@
 #include "quad_schedule.hpp"
 #include "quadmp_schedule.hpp"
 
+static_assert(npfem::QMP_MAX_PASSES == 4 && npfem::QMP_THREADS == 640,
+              "local_quadmp.cu (NP, TH) and QuadMpDev::list_len are written for 4 passes of 640 quads");
+
 using namespace npfem;
 
 struct npfem_ctx {
