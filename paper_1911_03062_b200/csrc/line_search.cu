@@ -176,6 +176,99 @@ damping_grad_kernel(const DampingParams p) {
   }
 }
 
+// The same for cells of at most 768 vertices (RBC-642, PLT-162): persistent CTAs, the one-ring tables of the thread's
+// <= 3 vertices (neighbour ids packed in pairs, weights, inverse area, mass) live in REGISTERS for the whole launch
+// instead of coming from L1 / L2 twice per cell, and the cell's g is requested together with its d at the top of the
+// cell, so its latency runs under the two stencil passes (ncu on the plain kernel: long-scoreboard 15 per issue).
+// Same arithmetic in the same order: bit-identical to damping_grad_kernel.
+template <int MAXQ>
+__global__ void __launch_bounds__(256, 2)
+damping_grad_reg_kernel(const DampingParams p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int VPT = 3;
+  const int n = p.n, n_pad = p.n_pad;
+  float *sd = reinterpret_cast<float *>(smem_raw);   // [3][n]
+  float *sz = sd + 3 * n;                             // [3][n]
+  uint32_t nb[VPT][MAXQ / 2];
+  float w[VPT][MAXQ + 1], ks[VPT], mi[VPT];
+#pragma unroll
+  for (int v = 0; v < VPT; ++v) {
+    const int i = threadIdx.x + 256 * v;
+    const bool a = i < n;
+    w[v][0] = a ? p.vtx_w[i] : 0.f;
+#pragma unroll
+    for (int q = 0; q < MAXQ; q += 2) {
+      const int j0 = a && q < p.valence_max ? p.vtx_nbr[q * n + i] : 0;
+      const int j1 = a && q + 1 < p.valence_max ? p.vtx_nbr[(q + 1) * n + i] : 0;
+      nb[v][q / 2] = uint32_t(j0) | (uint32_t(j1) << 16);
+      w[v][q + 1] = a && q < p.valence_max ? p.vtx_w[(q + 1) * n + i] : 0.f;
+      w[v][q + 2] = a && q + 1 < p.valence_max ? p.vtx_w[(q + 2) * n + i] : 0.f;
+    }
+    ks[v] = a ? p.k_b * p.vtx_inv_area[i] : 0.f;
+    mi[v] = a ? p.gamma_inertia * p.vtx_mass[i] : 0.f;
+  }
+  for (int64_t cell = blockIdx.x; cell < p.cells; cell += gridDim.x) {
+    const size_t base = size_t(cell) * 3 * n_pad;
+    float gk[VPT][3];
+#pragma unroll
+    for (int v = 0; v < VPT; ++v) {
+      const int i = threadIdx.x + 256 * v;
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        if (i < n) sd[k * n + i] = p.d[base + k * n_pad + i];
+        gk[v][k] = i < n ? p.g[base + k * n_pad + i] : 0.f;
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int v = 0; v < VPT; ++v) {
+      const int i = threadIdx.x + 256 * v;
+      if (i < n) {
+        float u[3] = {w[v][0] * sd[i], w[v][0] * sd[n + i], w[v][0] * sd[2 * n + i]};
+#pragma unroll
+        for (int q = 0; q < MAXQ; ++q)
+          if (q < p.valence_max) {
+            const int j = int((q & 1) ? nb[v][q / 2] >> 16 : nb[v][q / 2] & 0xffffu);
+            const float wq = w[v][q + 1];
+            u[0] += wq * sd[j];
+            u[1] += wq * sd[n + j];
+            u[2] += wq * sd[2 * n + j];
+          }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) sz[k * n + i] = p.k_mem * sd[k * n + i] + ks[v] * u[k];
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int v = 0; v < VPT; ++v) {
+      const int i = threadIdx.x + 256 * v;
+      if (i < n) {
+        float lz[3] = {w[v][0] * sz[i], w[v][0] * sz[n + i], w[v][0] * sz[2 * n + i]};
+#pragma unroll
+        for (int q = 0; q < MAXQ; ++q)
+          if (q < p.valence_max) {
+            const int j = int((q & 1) ? nb[v][q / 2] >> 16 : nb[v][q / 2] & 0xffffu);
+            const float wq = w[v][q + 1];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) lz[k] += wq * sz[k * n + j];
+          }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+          const float g = gk[v][k] + mi[v] * sd[k * n + i] + p.beta_over_h * lz[k];
+          if (p.g_lo) {
+            const float hi = tf32_rn(g);
+            p.g[base + k * n_pad + i] = hi;
+            p.g_lo[base + k * n_pad + i] = tf32_rn(g - hi);
+          } else {
+            p.g[base + k * n_pad + i] = p.g_tf32 ? tf32_rn(g) : g;
+          }
+        }
+      }
+    }
+    __syncthreads();
+  }
+}
+
 __global__ void __launch_bounds__(256) split_g_kernel(float *__restrict__ g, float *__restrict__ g_lo, size_t count) {
   for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < count; i += size_t(gridDim.x) * blockDim.x) {
     const float v = g[i], hi = tf32_rn(v);
@@ -216,6 +309,11 @@ int launch_damping_grad(const TypeDev &td, const BucketView &bv, float *g_lo, in
   if (smem > 200 * 1024) return -1;
   if (!td.cache.damping_attr) cudaFuncSetAttribute(damping_grad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   td.cache.damping_attr = true;
+  if (td.n <= 768 && td.valence_max <= 8) {   // tables in registers, persistent: 2 CTAs per SM (registers)
+    const int64_t capr = int64_t(n_sm) * 2;
+    damping_grad_reg_kernel<8><<<unsigned(bv.cells < capr ? bv.cells : capr), 256, smem, s>>>(p);
+    return 1;
+  }
   const int64_t cap = int64_t(n_sm) * 8 * 2;
   damping_grad_kernel<<<unsigned(bv.cells < cap ? bv.cells : cap), 256, smem, s>>>(p);
   return 1;
